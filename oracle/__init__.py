@@ -1,0 +1,189 @@
+"""CPU oracle for the UltraEP balance-planning path — TEST INFRASTRUCTURE ONLY.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It shares no code with the CUDA
+path (``paper_2606_04101_b200``) and never imports it.
+
+The arithmetic lives in ``uep_oracle.cpp`` (plain single-threaded C++, written from
+reference/PAPER.md Algorithm 1 and §5.2); this module only compiles it with g++ and
+marshals numpy arrays through ctypes.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "uep_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+FLOOR_STRICT = 0
+FLOOR_TOLERANT = 1
+N_SCALARS = 16
+SC_TAU, SC_N_REPLICAS, SC_MAX_LOAD, SC_MAX_FANOUT, SC_N_PROBES, SC_N_INVALID, SC_TAU_LO0, \
+    SC_TAU_HI0, SC_N_GROUPS = range(9)
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle (g++ -O2, single translation unit). Returns the .so path."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    tmp = _LIB + f".tmp{os.getpid()}"
+    subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-o", tmp, _SRC])
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        for name in ("uep_oracle_histogram", "uep_oracle_layout", "uep_oracle_plan",
+                     "uep_oracle_remap", "uep_oracle_pack"):
+            getattr(_lib, name).restype = ctypes.c_int
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+@dataclass
+class Plan:
+    """Host copy of every plan array (names as in include/uep.h / DESIGN.md)."""
+    E: int
+    R: int
+    n_slot: int
+    M: int
+    P: int
+    home: np.ndarray
+    main_phys: np.ndarray
+    slot_expert: np.ndarray   # [R, n_slot]
+    inst_off: np.ndarray      # [E+1]
+    inst_rank: np.ndarray     # [E + R*n_slot]
+    inst_phys: np.ndarray
+    inst_cum: np.ndarray
+    phys_count: np.ndarray    # [R, P]
+    phys_base: np.ndarray     # [R, P]
+    rank_load: np.ndarray     # [R]
+    rank_base: np.ndarray     # [R+1]
+    U: np.ndarray             # [E, R]
+    scalars: np.ndarray       # [16]
+    trace: list               # [(tau, feasible)] bisection sequence
+
+    @property
+    def tau(self):
+        return int(self.scalars[SC_TAU])
+
+    @property
+    def n_replicas(self):
+        return int(self.scalars[SC_N_REPLICAS])
+
+
+def histogram(ids: np.ndarray, E: int):
+    """O-1. Returns (count[E] int32, n_invalid)."""
+    ids = _i32(ids).reshape(-1)
+    count = np.zeros(E, dtype=np.int32)
+    bad = ctypes.c_int64(0)
+    rc = _load().uep_oracle_histogram(_p(ids), ctypes.c_int64(ids.size), ctypes.c_int32(E),
+                                      _p(count), ctypes.byref(bad))
+    assert rc == 0
+    return count, int(bad.value)
+
+
+def layout(E: int, R: int, home=None):
+    """Static layout: (home[E], main_phys[E], M)."""
+    home_in = None if home is None else _i32(home)
+    home_out = np.zeros(E, dtype=np.int32)
+    main_phys = np.zeros(E, dtype=np.int32)
+    M = ctypes.c_int32(0)
+    rc = _load().uep_oracle_layout(ctypes.c_int32(E), ctypes.c_int32(R), _p(home_in),
+                                   _p(home_out), _p(main_phys), ctypes.byref(M))
+    if rc != 0:
+        raise ValueError("home rank outside [0, R)")
+    return home_out, main_phys, int(M.value)
+
+
+def plan(lam: np.ndarray, R: int, n_slot: int, u_min: int, beta_num: int = 101,
+         beta_den: int = 100, floor_mode: int = FLOOR_TOLERANT, home=None,
+         S_total: int | None = None) -> Plan:
+    """O-2 SolveReplication (Alg. 1 lines 1-25)."""
+    lam = _i32(lam).reshape(-1)
+    E = lam.size
+    home_arr, main_phys, M = layout(E, R, home)
+    P = M + n_slot
+    cap = E + R * n_slot
+    z = lambda n: np.zeros(n, dtype=np.int32)
+    slot_expert, inst_off = z(max(R * n_slot, 1)), z(E + 1)
+    inst_rank, inst_phys, inst_cum = z(cap), z(cap), z(cap)
+    phys_count, phys_base = z(R * P), z(R * P)
+    rank_load, rank_base, U, scalars = z(R), z(R + 1), z(E * R), z(N_SCALARS)
+    trace_tau = np.zeros(128, dtype=np.int64)
+    trace_feas = z(128)
+    home_in = None if home is None else _i32(home)
+    if S_total is None:
+        S_total = int(lam.astype(np.int64).sum())
+    rc = _load().uep_oracle_plan(
+        _p(lam), ctypes.c_int32(E), ctypes.c_int32(R), ctypes.c_int32(n_slot),
+        ctypes.c_int32(u_min), ctypes.c_int32(beta_num), ctypes.c_int32(beta_den),
+        ctypes.c_int32(floor_mode), _p(home_in), ctypes.c_int64(S_total),
+        _p(slot_expert), _p(inst_off), _p(inst_rank), _p(inst_phys), _p(inst_cum),
+        _p(phys_count), _p(phys_base), _p(rank_load), _p(rank_base), _p(U), _p(scalars),
+        _p(trace_tau), _p(trace_feas), ctypes.c_int32(128))
+    if rc != 0:
+        raise ValueError(f"uep_oracle_plan rc={rc}")
+    n = int(scalars[SC_N_PROBES])
+    trace = [(int(trace_tau[i]), bool(trace_feas[i])) for i in range(min(n, 128))]
+    return Plan(E, R, n_slot, M, P, home_arr, main_phys,
+                slot_expert[:R * n_slot].reshape(R, n_slot), inst_off, inst_rank, inst_phys,
+                inst_cum, phys_count.reshape(R, P), phys_base.reshape(R, P), rank_load,
+                rank_base, U.reshape(E, R), scalars, trace)
+
+
+def remap(ids: np.ndarray, gate: np.ndarray | None, pl: Plan):
+    """O-3 token assignment. gate is any array with 2- or 4-byte items (raw byte copy).
+    Returns (replica, rank, offset, out_gate) with the shapes of ids / a flat gate array."""
+    ids32 = _i32(ids)
+    flat = ids32.reshape(-1)
+    S = flat.size
+    rep, rnk, off = (np.empty(S, dtype=np.int32) for _ in range(3))
+    if gate is not None:
+        gate = np.ascontiguousarray(gate).reshape(-1)
+        assert gate.size == S and gate.itemsize in (2, 4)
+        out_gate = np.zeros(S, dtype=gate.dtype)
+        gbytes = gate.itemsize
+    else:
+        out_gate, gbytes = None, 0
+    rc = _load().uep_oracle_remap(
+        _p(flat), _p(gate), ctypes.c_int32(gbytes), ctypes.c_int64(S), ctypes.c_int32(pl.E),
+        ctypes.c_int32(pl.P), _p(pl.inst_off), _p(pl.inst_rank), _p(pl.inst_phys),
+        _p(pl.inst_cum), _p(np.ascontiguousarray(pl.phys_base).reshape(-1)), _p(pl.rank_base),
+        _p(rep), _p(rnk), _p(off), _p(out_gate))
+    if rc != 0:
+        raise ValueError(f"uep_oracle_remap rc={rc}")
+    shp = ids32.shape
+    return rep.reshape(shp), rnk.reshape(shp), off.reshape(shp), out_gate
+
+
+def pack(slot_expert: np.ndarray, src: np.ndarray, dst: np.ndarray) -> None:
+    """O-4. src: [E, ...] contiguous per expert; dst: [R, n_slot, ...] written in place."""
+    se = _i32(slot_expert)
+    R, n_slot = se.shape
+    assert src.flags.c_contiguous and dst.flags.c_contiguous and dst.flags.writeable
+    B = src.nbytes // src.shape[0]
+    assert dst.nbytes == R * n_slot * B
+    rc = _load().uep_oracle_pack(_p(se.reshape(-1)), ctypes.c_int32(R), ctypes.c_int32(n_slot),
+                                 _p(src), ctypes.c_int64(B), _p(dst))
+    assert rc == 0

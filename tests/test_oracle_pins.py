@@ -1,0 +1,297 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU, no CUDA path).
+
+Every test here would fail on a plausible oracle mistake (dropped term, wrong tie-break,
+wrong rounding, wrong floor predicate, transposed index):
+  * hand-worked examples A/B (tests/golden, derived by hand from Alg. 1)
+  * closed form for all-slots-to-one-expert
+  * identity / degenerate cases, strict == tolerant at u_min = 1
+  * the paper's constraints as invariants on Zipf workloads over a shape grid
+  * numpy bincount (histogram), numpy STABLE argsort (remap), numpy fancy indexing (pack)
+  * exhaustive optimum over all placements on the tiny config (Hall bound, cross-checked
+    against scipy max-flow)
+"""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_04101_b200 import synth
+import uep_checks as ck
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _read_golden(name):
+    d = {}
+    with open(os.path.join(GOLD, name)) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            k, v = line.split(":", 1)
+            d[k.strip()] = v.strip()
+    return d
+
+
+@pytest.mark.parametrize("name", ["example_A.txt", "example_B_strict.txt",
+                                  "example_B_tolerant.txt"])
+def test_worked_examples(name):
+    g = _read_golden(name)
+    lam = np.array(g["lambda"].split(), dtype=np.int32)
+    bn, bd = (int(x) for x in g["beta"].split("/"))
+    probes = [(int(a), b == "F") for a, b in (x.split(":") for x in g["probes"].split())]
+    transfers = []
+    for x in g["transfers"].split():
+        et, d = x.split(":")
+        e, t = et.split(">")
+        transfers.append((int(e), int(t), int(d)))
+    for mode in g["modes"].split():
+        fm = oracle.FLOOR_STRICT if mode == "strict" else oracle.FLOOR_TOLERANT
+        p = oracle.plan(lam, int(g["R"]), int(g["n_slot"]), int(g["u_min"]), bn, bd, fm)
+        assert p.trace == probes
+        assert p.tau == int(g["tau"])
+        assert p.rank_load.tolist() == [int(x) for x in g["rank_load"].split()]
+        got = []
+        for e in range(p.E):
+            lo, hi = p.inst_off[e], p.inst_off[e + 1]
+            q = np.diff(np.concatenate([[0], p.inst_cum[lo:hi]]))
+            got += [(e, int(p.inst_rank[lo + i]), int(q[i])) for i in range(1, hi - lo)]
+        assert got == transfers
+        assert p.inst_cum[p.inst_off[0]:p.inst_off[1]].tolist() == \
+            [int(x) for x in g["cum_e0"].split()]
+        ck.check_plan(lam, p, int(g["u_min"]), bn, bd, fm)
+
+
+def test_all_to_one_closed_form():
+    """All S slots on one expert: the other R-1 ranks have slack tau each, so the probe takes
+    tau-sized bites, lowest rank id first.  S=2^21, R=64, beta=1.01, u_min=1024:
+    tau = floor(1.01*32768) = 33095, 63 replicas: 62 of 33095 and one of 12167."""
+    E, R, S = 256, 64, 2097152
+    for hot in (0, 37, 255):
+        lam = np.zeros(E, dtype=np.int32)
+        lam[hot] = S
+        p = oracle.plan(lam, R, 2, 1024)
+        h = hot * R // E
+        assert p.tau == 33095 and p.n_replicas == 63 and int(p.scalars[3]) == 64
+        lo, hi = p.inst_off[hot], p.inst_off[hot + 1]
+        q = np.diff(np.concatenate([[0], p.inst_cum[lo:hi]]))
+        assert q[0] == 33095 and (q[1:63] == 33095).all() and q[63] == 12167
+        assert 63 * 33095 + 12167 == S
+        others = [t for t in range(R) if t != h]
+        assert p.inst_rank[lo + 1:hi].tolist() == others          # lowest rank id first
+        assert all(ok for _, ok in p.trace)                       # monotone: every mid feasible
+        ck.check_plan(lam, p, 1024)
+    # general closed form (tolerant): tau = tau_lo whenever tau_lo >= ceil(S/R)
+    for S2, R2, um in [(100000, 8, 100), (999983, 16, 500), (4096, 4, 64)]:
+        lam = np.zeros(32, dtype=np.int32)
+        lam[5] = S2
+        p = oracle.plan(lam, R2, 1, um)
+        tau = (-(-S2 // R2)) * 101 // 100
+        assert p.tau == tau
+        bites = (S2 - tau) // tau
+        rem = (S2 - tau) - bites * tau
+        assert p.n_replicas == bites + (1 if rem >= um else 0)
+        ck.check_plan(lam, p, um)
+
+
+def test_identity_and_degenerate_cases():
+    rng = np.random.default_rng(0)
+    # balanced: max l <= tau_lo -> loop never runs (S4)
+    lam = np.full(64, 1000, dtype=np.int32)
+    p = oracle.plan(lam, 16, 2, 16)
+    assert p.n_replicas == 0 and p.trace == [] and p.tau == 4000 and (p.slot_expert == -1).all()
+    assert (p.rank_load == 4000).all()
+    # n_slot = 0: probes run, none can move load -> identity, tau = max l
+    lam = rng.integers(0, 5000, 64).astype(np.int32)
+    p = oracle.plan(lam, 16, 0, 16, floor_mode=oracle.FLOOR_STRICT)
+    ell = ck.initial_rank_load(lam, p.home, 16)
+    assert p.n_replicas == 0 and p.tau == ell.max() and (p.rank_load == ell).all()
+    ck.check_plan(lam, p, 16, floor_mode=ck.STRICT)
+    # tolerant (S8): with no transfer possible a probe is feasible iff max l - tau < u_min,
+    # which is monotone, so bisection must find exactly max l - u_min + 1
+    p = oracle.plan(lam, 16, 0, 16)
+    assert p.n_replicas == 0 and p.tau == ell.max() - 16 + 1 and (p.rank_load == ell).all()
+    ck.check_plan(lam, p, 16)
+    # R = 1
+    p = oracle.plan(lam, 1, 2, 16)
+    assert p.n_replicas == 0 and p.rank_load[0] == lam.sum()
+    # empty load
+    p = oracle.plan(np.zeros(16, np.int32), 4, 1, 8)
+    assert p.n_replicas == 0 and p.tau == 0 and (p.rank_load == 0).all()
+    # E < R (S2): ranks without a main expert are pure absorbers
+    lam = rng.integers(1000, 90000, 64).astype(np.int32)
+    p = oracle.plan(lam, 256, 1, 64)
+    assert p.M == 1 and (np.bincount(p.home, minlength=256) <= 1).all()
+    ck.check_plan(lam, p, 64)
+    assert p.n_replicas > 0
+    # explicit home map
+    home = rng.integers(0, 8, 64).astype(np.int32)
+    p = oracle.plan(lam, 8, 3, 256, home=home)
+    assert (p.home == home).all()
+    ck.check_plan(lam, p, 256)
+
+
+def test_strict_equals_tolerant_at_u_min_1():
+    for seed in range(6):
+        ids = synth.zipf_topk_ids(2048, 4, 64, 0.6 + 0.3 * seed, seed).numpy()
+        lam, _ = oracle.histogram(ids, 64)
+        a = oracle.plan(lam, 16, 2, 1, floor_mode=oracle.FLOOR_STRICT)
+        b = oracle.plan(lam, 16, 2, 1, floor_mode=oracle.FLOOR_TOLERANT)
+        assert a.trace == b.trace and (a.U == b.U).all() and (a.slot_expert == b.slot_expert).all()
+        ck.check_plan(lam, a, 1, floor_mode=ck.STRICT)
+        # with u_min = 1 every overloaded rank that can be drained is: load <= tau exactly
+        assert a.rank_load.max() <= a.tau
+
+
+GRID = [  # (T, k, E, R, n_slot, s)
+    (4096, 2, 16, 4, 1, 1.2), (8192, 8, 128, 32, 2, 0.6), (8192, 8, 128, 32, 2, 1.4),
+    (16384, 8, 256, 64, 2, 1.0), (16384, 4, 512, 256, 4, 2.0), (4096, 1, 64, 8, 1, 0.0),
+    (8192, 8, 160, 40, 4, 1.0), (2048, 4, 64, 256, 1, 1.0), (16384, 8, 512, 8, 3, 1.6),
+]
+
+
+@pytest.mark.parametrize("T,k,E,R,n_slot,s", GRID)
+@pytest.mark.parametrize("mode", [oracle.FLOOR_STRICT, oracle.FLOOR_TOLERANT])
+def test_plan_invariants_and_remap_on_zipf(T, k, E, R, n_slot, s, mode):
+    ids = synth.zipf_topk_ids(T, k, E, s, seed=T + E + R).numpy()
+    lam, bad = oracle.histogram(ids, E)
+    assert bad == 0 and (lam == np.bincount(ids.ravel(), minlength=E)).all()   # library pin
+    u_min = synth.stress_u_min(T * k, R)
+    p = oracle.plan(lam, R, n_slot, u_min, floor_mode=mode)
+    ck.check_plan(lam, p, u_min, floor_mode=mode)
+    gate = synth.gates_uniform_renorm(T, k, 3).numpy()
+    rep, rnk, off, og = oracle.remap(ids, gate, p)
+    ck.check_remap(ids, p, rep, rnk, off, gate, og)
+
+
+def test_histogram_invalid_ids_and_remap_skip():
+    rng = np.random.default_rng(5)
+    ids = rng.integers(-3, 20, size=(3000, 4)).astype(np.int32)       # ids in [-3, 19], E = 16
+    lam, bad = oracle.histogram(ids, 16)
+    valid = (ids >= 0) & (ids < 16)
+    assert bad == (~valid).sum() and (lam == np.bincount(ids[valid], minlength=16)).all()
+    p = oracle.plan(lam, 4, 1, 32, S_total=ids.size)
+    assert int(p.scalars[5]) == bad
+    gate = rng.standard_normal(ids.shape).astype(np.float32)
+    rep, rnk, off, og = oracle.remap(ids, gate, p)
+    ck.check_remap(ids, p, rep, rnk, off, gate, og)
+
+
+def test_remap_duplicate_ids_in_token_and_gate_bits():
+    """S15 duplicates inside a token; S17 gates are raw bit copies (NaN payloads, -0.0, denormals)."""
+    ids = synth.one_expert_ids(2048, 4, 3).numpy()
+    lam, _ = oracle.histogram(ids, 16)
+    p = oracle.plan(lam, 4, 1, 64)
+    bits = np.arange(ids.size, dtype=np.uint32) * np.uint32(2654435761)
+    bits[:8] = [0x7FC00001, 0xFFC12345, 0x80000000, 0x00000001, 0x807FFFFF, 0x7F800000,
+                0xFF800000, 0x7FA00000]
+    gate = bits.view(np.float32).reshape(ids.shape)
+    rep, rnk, off, og = oracle.remap(ids, gate, p)
+    pos = ck.check_remap(ids, p, rep, rnk, off, gate, og)
+    assert sorted(og.view(np.uint32).tolist()) == sorted(bits.tolist())
+    # contiguous ranges in global stable order: slot j of expert 3 -> instance by cum
+    cum = p.inst_cum[p.inst_off[3]:p.inst_off[4]]
+    j = np.arange(ids.size)
+    assert (rep.ravel() == np.searchsorted(cum, j, side="right")).all()
+    # bf16-sized gates
+    g16 = (np.arange(ids.size) % 65536).astype(np.uint16)
+    _, _, _, og16 = oracle.remap(ids, g16, p)
+    assert (og16[pos] == g16).all()
+
+
+def test_pack_matches_numpy_indexing():
+    rng = np.random.default_rng(1)
+    ids = synth.zipf_topk_ids(4096, 2, 16, 1.2, 9).numpy()
+    lam, _ = oracle.histogram(ids, 16)
+    p = oracle.plan(lam, 4, 2, 64)
+    assert p.n_replicas > 0
+    src = rng.integers(0, 65536, size=(16, 1000)).astype(np.uint16)
+    sent = rng.integers(0, 65536, size=(4, 2, 1000)).astype(np.uint16)
+    dst = sent.copy()
+    oracle.pack(p.slot_expert, src, dst)
+    X = p.slot_expert
+    ref = np.where((X >= 0)[..., None], src[np.maximum(X, 0)], sent)
+    assert np.array_equal(dst, ref)
+    ck.check_pack(X, src, dst, sent)
+
+
+def _hall_min_max(lam, home, placements, R):
+    """Exact optimum of min-max rank load with splittable expert load for each placement:
+    max over non-empty rank subsets B of ceil(load confined to B / |B|) (max-flow/min-cut)."""
+    lam = np.asarray(lam, dtype=np.int64)
+    E = lam.size
+    N = placements.shape[0]
+    best = np.zeros(N, dtype=np.int64)
+    e_idx = np.arange(E)
+    for mask in range(1, 1 << R):
+        inB = np.array([(mask >> t) & 1 for t in range(R)], dtype=bool)
+        conf = np.broadcast_to(inB[home][None, :], (N, E)).copy()      # home in B
+        for t in range(R):
+            if not inB[t]:                                             # replica outside B
+                conf &= placements[:, t][:, None] != e_idx[None, :]
+        load = (conf * lam[None, :]).sum(axis=1)
+        nb = int(inB.sum())
+        best = np.maximum(best, -(-load // nb))
+    return best
+
+
+def test_tiny_config_bruteforce_optimum_bound():
+    """tiny config: enumerate all 13^4 placements (each rank's slot: empty or one of the 12
+    non-home experts); OPT (ignoring u_min, hence a lower bound) <= oracle's max load."""
+    from scipy.sparse import csr_matrix
+    from scipy.sparse.csgraph import maximum_flow
+    c = synth.CONFIGS["tiny"]
+    E, R = c["E"], c["R"]
+    ids = synth.zipf_topk_ids(c["T"], c["k"], E, c["zipf_s"], 2024).numpy()
+    lam, _ = oracle.histogram(ids, E)
+    home, _, _ = oracle.layout(E, R)
+    opts = []
+    for t in range(R):
+        opts.append([-1] + [e for e in range(E) if home[e] != t])
+    placements = np.array(list(itertools.product(*opts)), dtype=np.int64)
+    assert placements.shape == (13 ** 4, 4)
+    best = _hall_min_max(lam, home, placements, R)
+    # cross-check the Hall formula against scipy max-flow on a few placements
+    rng = np.random.default_rng(0)
+    for i in rng.integers(0, placements.shape[0], 12):
+        tau = int(best[i])
+        for cap, want in ((tau, True), (tau - 1, False)):
+            n = E + R + 2
+            g = np.zeros((n, n), dtype=np.int32)
+            for e in range(E):
+                g[0, 1 + e] = lam[e]
+                g[1 + e, 1 + E + home[e]] = lam[e]
+                for t in range(R):
+                    if placements[i, t] == e:
+                        g[1 + e, 1 + E + t] = lam[e]
+            for t in range(R):
+                g[1 + E + t, n - 1] = cap
+            flow = maximum_flow(csr_matrix(g), 0, n - 1).flow_value
+            assert (flow == lam.sum()) == want
+    opt = int(best.min())
+    mean_ceil = -(-int(lam.sum()) // R)
+    assert opt >= mean_ceil
+    for mode in (oracle.FLOOR_STRICT, oracle.FLOOR_TOLERANT):
+        p = oracle.plan(lam, R, c["n_slot"], c["u_min"], floor_mode=mode)
+        ck.check_plan(lam, p, c["u_min"], floor_mode=mode)
+        assert opt <= int(p.rank_load.max())
+        # the heuristic should land close to the optimum on this instance (plausibility)
+        assert int(p.rank_load.max()) <= opt + c["u_min"] + mean_ceil // 50
+
+
+def test_dsv3_shape_plausibility_against_table3():
+    """Table 3 aggregates are plausibility only: post-balance imbalance
+    within [1.00, beta + u_min/mean], a few dozen replicas, single-digit-ish fan-out."""
+    c = synth.CONFIGS["dsv3_prefill"]
+    for seed in (1, 2):
+        ids = synth.zipf_topk_ids(c["T"], c["k"], c["E"], 1.0, seed).numpy()
+        lam, _ = oracle.histogram(ids, c["E"])
+        p = oracle.plan(lam, c["R"], c["n_slot"], c["u_min"])
+        ck.check_plan(lam, p, c["u_min"])
+        mean = lam.sum() / c["R"]
+        imb = p.rank_load.max() / mean
+        assert 1.0 <= imb <= 1.01 + 1024 / mean + 1e-9
+        assert 20 <= p.n_replicas <= 128 and int(p.scalars[3]) <= 16
+        assert 12 <= int(p.scalars[4]) <= 24
