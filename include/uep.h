@@ -1,0 +1,196 @@
+/* uep.h — C ABI of libuep: the post-gating, exact-load balance-planning step of UltraEP
+ * (arxiv 2606.04101), emulated for R virtual expert-parallel ranks on ONE B200 (sm_100a).
+ *
+ *   uep_histogram : lambda_e, the per-expert token load              (Alg. 1 line 2)
+ *   uep_plan      : SolveReplication, quota-driven planner           (Alg. 1 lines 1-25, PAPER.md:247-297;
+ *                                                                     §5.1; §5.3)
+ *   uep_remap     : token assignment by cumulative-quota lookup      (§5.2 "Token Assignment")
+ *   uep_pack      : weight distribution main -> redundant slot,      (§4.2, §6.1)
+ *                   single-GPU part: pack into per-destination buffers
+ *   uep_balance   : the four chained on one stream, capturable in a CUDA graph
+ *                   ("fully on-device ... preserves the graph capture")
+ *
+ * Conventions (all entry points)
+ *   - plain C; every pointer argument says HOST or DEVICE below; `stream` is a cudaStream_t
+ *     passed as void* so that this header needs no CUDA include.
+ *   - return 0 (UEP_OK) or a negative UEP_ERR_*; uep_strerror() gives the text.
+ *   - after uep_create: asynchronous on `stream`, no host synchronisation, no allocation,
+ *     no host memory touched => every compute call can be stream-captured.
+ *   - ownership: the library never frees or retains caller pointers beyond the call.
+ *     Outputs and workspace are caller-allocated DEVICE memory.  A context may be shared by
+ *     concurrent calls; a workspace may not (one per in-flight call).
+ *   - data faults that would need a sync to report (an id outside [0,E)) are counted on the
+ *     device (scalars[UEP_SC_N_INVALID]) and the slot is skipped (S14).
+ *   - all DEVICE pointers must be 16-byte aligned.
+ *
+ * Notation (Table 1): E logical experts, R ranks, N_slot redundant slots per
+ * rank, h(e) home rank, lambda_e load, l_r initial rank load, U quotas, X slot assignment.
+ * S = T*k routed slots; M = max_r |E_r| main slots per rank; P = M + N_slot physical slots.
+ */
+#ifndef UEP_H_
+#define UEP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define UEP_MAX_E 512        /* shared-memory histogram / planner tables are sized for this */
+#define UEP_MAX_R 256
+#define UEP_MAX_NSLOT 4
+#define UEP_MAX_TENSORS 8
+
+enum { UEP_FLOOR_STRICT = 0,     /* Alg. 1 line 20 verbatim: feasible iff sum_r exc_r == 0      */
+       UEP_FLOOR_TOLERANT = 1 }; /* DESIGN.md S8 (default): feasible iff every exc_r < u_min    */
+enum { UEP_GATE_F32 = 0, UEP_GATE_BF16 = 1, UEP_GATE_NONE = 2 };
+
+enum { UEP_OK = 0,
+       UEP_ERR_INVALID_ARG = -1,   /* NULL / misaligned pointer, bad size                        */
+       UEP_ERR_UNSUPPORTED = -2,   /* shape outside the limits above                             */
+       UEP_ERR_CUDA = -3,          /* a CUDA runtime call or launch failed                       */
+       UEP_ERR_NO_DEVICE = -4 };
+
+/* plan->scalars[] indices (int32 each, UEP_N_SCALARS entries) */
+enum { UEP_SC_TAU = 0,           /* final threshold tau (Alg. 1: tau_hi on exit)                 */
+       UEP_SC_N_REPLICAS = 1,    /* number of redundant slots used, sum_e (|H(e)|-1)             */
+       UEP_SC_MAX_LOAD = 2,      /* max_r sum_e u_{e,r}                      (Eq. 3) */
+       UEP_SC_MAX_FANOUT = 3,    /* max_e |H(e)|                              (Table 3)           */
+       UEP_SC_N_PROBES = 4,      /* probes on the sequential bisection path                      */
+       UEP_SC_N_INVALID = 5,     /* T*k - sum_e lambda_e                                         */
+       UEP_SC_TAU_LO0 = 6,       /* tau_lo on entry                                              */
+       UEP_SC_TAU_HI0 = 7,       /* tau_hi on entry = max_r l_r                                  */
+       UEP_SC_N_GROUPS = 8,      /* number of experts with at least one replica                  */
+       UEP_N_SCALARS = 16 };
+
+typedef struct uep_ctx uep_ctx;  /* opaque; immutable after uep_create */
+
+typedef struct uep_config {
+  int32_t T, k;                  /* tokens and top-k; S = T*k < 2^24 slots                       */
+  int32_t E, R, n_slot;          /* 1<=E<=512, 1<=R<=256, 0<=n_slot<=4                            */
+  int32_t u_min;                 /* quota floor u_min >= 1 (paper: 1024)           */
+  int32_t beta_num, beta_den;    /* balancing target beta as a rational (paper: 101/100)         */
+  int32_t floor_mode;            /* UEP_FLOOR_*                                                   */
+  int32_t gate_dtype;            /* UEP_GATE_*                                                    */
+  const int32_t* home_rank;      /* HOST [E] or NULL => h(e) = floor(e*R/E)        (S2) */
+} uep_config;
+
+/* element counts (int32 elements) of every plan array, plus the derived M and P */
+typedef struct uep_plan_sizes {
+  int32_t slot_expert;           /* R*n_slot (>=1 allocated)                                      */
+  int32_t inst_off;              /* E+1                                                           */
+  int32_t inst_cap;              /* E + R*n_slot : inst_rank / inst_phys / inst_cum               */
+  int32_t phys;                  /* R*P : phys_count / phys_base                                  */
+  int32_t rank_load;             /* R                                                             */
+  int32_t rank_base;             /* R+1                                                           */
+  int32_t U;                     /* E*R (optional dense quota table)                              */
+  int32_t scalars;               /* UEP_N_SCALARS                                                 */
+  int32_t M, P;
+} uep_plan_sizes;
+
+/* The plan: a struct (in HOST memory) of DEVICE pointers, all int32.
+ *   slot_expert[R][n_slot]  X: expert replicated in redundant slot s of rank t, -1 = empty;
+ *                           used slots of a rank are a prefix, in acceptance order (S10)
+ *   inst_off[E+1]           CSR over logical experts into the instance arrays
+ *   inst_rank/phys/cum[]    instances of e in order [main, replicas in acceptance order] (S11):
+ *                           host rank, local physical slot on that rank (main e -> its index
+ *                           among E_{h(e)} ascending; redundant slot s -> M+s), and the
+ *                           INCLUSIVE cumulative quota (last = lambda_e)
+ *   phys_count/base[R][P]   tokens received per local physical slot and their exclusive prefix
+ *   rank_load[R]            sum_e u_{e,t};  rank_base[R+1] its exclusive prefix (last = #valid)
+ *   scalars[UEP_N_SCALARS]  see UEP_SC_*
+ *   U[E][R]                 dense quota table, may be NULL (tests / inspection only)        */
+typedef struct uep_plan_out {
+  int32_t* slot_expert;
+  int32_t* inst_off;
+  int32_t* inst_rank;
+  int32_t* inst_phys;
+  int32_t* inst_cum;
+  int32_t* phys_count;
+  int32_t* phys_base;
+  int32_t* rank_load;
+  int32_t* rank_base;
+  int32_t* scalars;
+  int32_t* U;
+} uep_plan_out;
+
+/* Create a context for fixed shapes (validates limits, uploads the static layout h(e), E_r,
+ * main slot indices).  cfg: HOST.  Uses the current CUDA device.  Allocates a few KB of
+ * device memory, freed by uep_destroy. */
+int uep_create(const uep_config* cfg, uep_ctx** out);
+void uep_destroy(uep_ctx* ctx);
+
+/* Bytes of DEVICE workspace one in-flight call needs.  It carries the per-chunk expert counts
+ * from uep_histogram to uep_remap (their exclusive prefix over chunks gives each slot's global
+ * stable rank).  uep_workspace_init must be called once (async on `stream`) before first use. */
+size_t uep_workspace_bytes(const uep_ctx* ctx);
+int uep_workspace_init(const uep_ctx* ctx, void* ws, void* stream);
+int uep_plan_bytes(const uep_ctx* ctx, uep_plan_sizes* out);      /* out: HOST */
+
+/* lambda_e = #{slots s : topk_ids[s] == e} (Alg. 1 line 2).
+ *   topk_ids      DEVICE int32 [T,k] row-major (slot s = i*k + kk)
+ *   expert_count  DEVICE int32 [E], overwritten
+ *   ws            DEVICE workspace; afterwards holds the chunk prefix table for uep_remap    */
+int uep_histogram(const uep_ctx* ctx, const int32_t* topk_ids, int32_t* expert_count, void* ws,
+                  void* stream);
+
+/* SolveReplication (Alg. 1 lines 1-25) under the readings of DESIGN.md §3; emits X, U (as CSR
+ * cumulative quotas) and the receive layout.  expert_count: DEVICE int32 [E].  plan: HOST struct
+ * of DEVICE pointers (U may be NULL).  ws is not modified. */
+int uep_plan(const uep_ctx* ctx, const int32_t* expert_count, const uep_plan_out* plan, void* ws,
+             void* stream);
+
+/* Token assignment (§5.2): slot s of expert e with global stable rank j goes to the first
+ * instance whose cumulative quota exceeds j.
+ *   gate          DEVICE [T,k] of cfg.gate_dtype, or NULL
+ *   out_replica/out_rank/out_offset  DEVICE int32 [T,k]; (-1,-1,-1) for an invalid id
+ *   out_gate      DEVICE [T*k] gate dtype, written at rank_base[rank]+offset (raw bit copy);
+ *                 positions past the number of valid slots are not written
+ *   ws            must come from uep_histogram on the SAME topk_ids                          */
+int uep_remap(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
+              const uep_plan_out* plan, int32_t* out_replica, int32_t* out_rank,
+              int32_t* out_offset, void* out_gate, void* ws, void* stream);
+
+/* Pack the state of every replicated expert into its destination slot:
+ *   dst[j][(t*n_slot+s)*B_j .. +B_j) = src[j][e*B_j .. +B_j)  for x_{t,s} = e != empty.
+ * Empty slots are not touched.  src/dst/bytes_per_expert: HOST arrays [n_tensors] of DEVICE
+ * pointers / sizes; B_j % 16 == 0; n_tensors <= UEP_MAX_TENSORS. */
+int uep_pack(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,
+             const void* const* src, const size_t* bytes_per_expert, void* const* dst,
+             void* stream);
+
+/* histogram -> plan -> remap and pack, chained on `stream` (pack runs on an internal side
+ * stream forked/joined with events, so that it overlaps the remap as in Eq. 1,
+ * max(T_reroute, T_w_distr)).  Capturable.  n_tensors may be 0. */
+int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
+                int32_t* expert_count, const uep_plan_out* plan, int32_t* out_replica,
+                int32_t* out_rank, int32_t* out_offset, void* out_gate, int32_t n_tensors,
+                const void* const* src, const size_t* bytes_per_expert, void* const* dst,
+                void* ws, void* stream);
+
+/* Convenience for callers with HOST buffers (the bench's end-to-end leg): copies ids/gate to
+ * the device buffers in `dev_*`, runs uep_balance, copies the remap outputs and the scalars
+ * back, and synchronises `stream`.  Host buffers should be pinned.  Expert state stays resident. */
+int uep_balance_host(const uep_ctx* ctx, const int32_t* topk_ids_host, const void* gate_host,
+                     int32_t* dev_topk_ids, void* dev_gate, int32_t* expert_count,
+                     const uep_plan_out* plan, int32_t* out_replica, int32_t* out_rank,
+                     int32_t* out_offset, void* out_gate, int32_t* out_replica_host,
+                     int32_t* out_rank_host, int32_t* out_offset_host, void* out_gate_host,
+                     int32_t* scalars_host, int32_t n_tensors, const void* const* src,
+                     const size_t* bytes_per_expert, void* const* dst, void* ws, void* stream);
+
+const char* uep_strerror(int code);
+const char* uep_last_cuda_error(void);   /* text of the last CUDA error seen on this thread */
+
+/* Launch geometry chosen at create time, for the bench's roofline arithmetic. */
+typedef struct uep_launch_info {
+  int32_t n_chunks, chunk_len;   /* histogram / remap: CTAs and slots per CTA                   */
+  int32_t hist_threads, remap_threads, plan_threads, pack_ctas, pack_tile_bytes, sm_count;
+} uep_launch_info;
+int uep_get_launch_info(const uep_ctx* ctx, uep_launch_info* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UEP_H_ */

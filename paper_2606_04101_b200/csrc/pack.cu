@@ -1,0 +1,173 @@
+// pack.cu — uep_pack: forward weight distribution main -> redundant slot (§4.2),
+// single-GPU part: copy the state of every replicated expert into the destination
+// rank's slot buffer.  dst[j][(t*n_slot+s)*B_j ..) = src[j][e*B_j ..) for x_{t,s} = e.
+//
+// HBM-bound byte movement.  Kept from the paper's tile streaming (§6.1): fixed
+// tiles, a persistent grid, and "each source tile is staged once into shared memory and stored
+// to all replica destinations" — so an expert with f replicas costs 1 read + f writes.
+// B200 form: the staging is done by the TMA engine, not by threads.  One elected thread per
+// CTA drives a ring of kPackStages shared-memory tiles: cp.async.bulk global->shared
+// (complete_tx on an mbarrier), then one cp.async.bulk shared->global per destination,
+// committed as a bulk group; a stage is refilled once the group that read it has drained
+// (cp.async.bulk.wait_group.read).  The grid is static (graph-capturable); the work list is
+// read from the plan on the device: CTA c takes tiles c, c+G, ... of every replicated expert,
+// rotated per (expert, tensor) so that remainders spread evenly.
+#include "uep_internal.cuh"
+
+namespace uep {
+
+constexpr int kPackThreads = 32;
+constexpr int kPackPending = 1;          // store groups allowed in flight when a stage is reused
+constexpr int kPackAhead = kPackStages - 1 - kPackPending;   // loads issued ahead of the stores
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          smem_u32(dst_smem)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst),
+               "r"(smem_u32(src_smem)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+// Enumerates this CTA's units in a fixed order: experts ascending (only those with replicas),
+// tensors ascending, tiles c' , c'+G, ...   A unit = one source tile and its destinations.
+struct UnitIter {
+  int e, j;
+  long long tile;        // tile index inside tensor j of expert e
+  unsigned rot;          // running rotation so that tile remainders spread over CTAs
+  __device__ void init() { e = -1; j = 0; tile = 0; rot = 0; }
+};
+
+struct Unit {
+  const unsigned char* src;
+  unsigned long long dst_off;   // byte offset of the tile inside a slot of tensor j
+  uint32_t bytes;
+  int e, j;
+};
+
+__global__ void __launch_bounds__(kPackThreads, 1)
+pack_kernel(PackArgs a, int E, int n_slot, int M, const int32_t* __restrict__ inst_off,
+            const int32_t* __restrict__ inst_rank, const int32_t* __restrict__ inst_phys) {
+  extern __shared__ __align__(128) unsigned char pack_smem[];
+  __shared__ __align__(8) uint64_t full[kPackStages];
+  __shared__ Unit ring[kPackStages];
+  if (threadIdx.x != 0) return;                         // one elected thread drives the TMA engine
+  const int G = gridDim.x, c = blockIdx.x;
+  for (int s = 0; s < kPackStages; ++s) mbar_init(&full[s], 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+
+  UnitIter it;
+  it.init();
+  // advance the iterator to this CTA's next unit; false when exhausted
+  auto next = [&](Unit& u) -> bool {
+    while (true) {
+      if (it.e >= 0 && it.e < E) {
+        while (it.j < a.n_tensors) {
+          const unsigned long long B = a.bytes[it.j];
+          const long long tiles = (long long)((B + kPackTile - 1) / kPackTile);
+          if (it.tile < tiles) {
+            const unsigned long long off = (unsigned long long)it.tile * kPackTile;
+            u.src = a.src[it.j] + (unsigned long long)it.e * B + off;
+            u.dst_off = off;
+            u.bytes = (uint32_t)min((unsigned long long)kPackTile, B - off);
+            u.e = it.e; u.j = it.j;
+            it.tile += G;
+            return true;
+          }
+          it.rot = (unsigned)((it.rot + tiles) % (unsigned)G);
+          it.j += 1;
+          it.tile = (c + G - (int)it.rot) % G;
+        }
+      }
+      // next replicated expert
+      int e = it.e + 1;
+      while (e < E && inst_off[e + 1] - inst_off[e] <= 1) ++e;
+      if (e >= E) { it.e = E; return false; }
+      it.e = e; it.j = 0;
+      it.tile = (c + G - (int)it.rot) % G;
+    }
+  };
+
+  long long n_loaded = 0, n_stored = 0;
+  bool more = true;
+  auto issue_load = [&]() {
+    Unit u;
+    if (!more || !(more = next(u))) return;
+    const int st = (int)(n_loaded % kPackStages);
+    ring[st] = u;
+    mbar_expect_tx(&full[st], u.bytes);
+    bulk_g2s(pack_smem + (size_t)st * kPackTile, u.src, u.bytes, &full[st]);
+    ++n_loaded;
+  };
+  for (int i = 0; i < kPackAhead; ++i) issue_load();
+  while (n_stored < n_loaded) {
+    // refill: the stage to be overwritten was read by the store group of unit n_loaded-kPackStages,
+    // which is at least kPackPending+1 groups old
+    if (more) {
+      if (n_loaded >= kPackStages) bulk_wait_read<kPackPending>();
+      issue_load();
+    }
+    const int st = (int)(n_stored % kPackStages);
+    mbar_wait(&full[st], (uint32_t)((n_stored / kPackStages) & 1));
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    const Unit u = ring[st];
+    const int lo = inst_off[u.e], hi = inst_off[u.e + 1];
+    const unsigned long long B = a.bytes[u.j];
+    for (int p = lo + 1; p < hi; ++p) {                  // every replica of e (entry lo = main)
+      const int slot = inst_rank[p] * n_slot + (inst_phys[p] - M);
+      bulk_s2g(a.dst[u.j] + (unsigned long long)slot * B + u.dst_off,
+               pack_smem + (size_t)st * kPackTile, u.bytes);
+    }
+    bulk_commit();
+    ++n_stored;
+  }
+  bulk_wait_all();
+}
+
+int init_pack_kernels() {
+  UEP_CUDA_TRY(cudaFuncSetAttribute(pack_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    kPackStages * kPackTile));
+  return UEP_OK;
+}
+
+int launch_pack(const Ctx* c, const uep_plan_out& plan, const PackArgs& a, cudaStream_t s) {
+  pack_kernel<<<c->pack_ctas, kPackThreads, kPackStages * kPackTile, s>>>(
+      a, c->cfg.E, c->cfg.n_slot, c->M, plan.inst_off, plan.inst_rank, plan.inst_phys);
+  UEP_CUDA_TRY(cudaGetLastError());
+  return UEP_OK;
+}
+
+}  // namespace uep

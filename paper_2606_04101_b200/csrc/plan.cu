@@ -1,0 +1,391 @@
+// plan.cu — uep_plan: SolveReplication (Alg. 1 lines 1-25; §5.1).
+//
+// Latency-bound integer work (a dependent chain of arg-max steps), no HBM traffic to speak of.
+// The paper's own kernel (§5.3: one CTA, state in shared memory, several
+// probes across warps) is prior art; what is kept: one CTA, one probe per warp.  What is new:
+//   * per-probe state (slack, used slots) lives in REGISTERS, lane t%32 owns rank t; the
+//     arg-max "largest slack, lowest rank id" is ONE redux.sync.max on a packed key
+//     (slack << 8 | 255 - t);
+//   * rank order and per-rank expert order do not depend on tau (S5): sorted once;
+//   * the sequential bisection is reproduced exactly (S9) by speculating the next kPlanLevels
+//     levels of ITS OWN tree with 2^L - 1 warps and then walking the path the sequential
+//     search takes; a k-ary search would not be equivalent;
+//   * infeasible probes exit as soon as a visited rank keeps too much excess (S21);
+//   * the no-duplicate test of Alg. 1 line 12 is provably redundant (S7: an accepted pair
+//     (e,t) leaves slk_t = 0 or ends e's loop, and h(e) is overloaded hence has no slack);
+//   * the accept log is written only by one final probe at the final tau (deterministic, so it
+//     reproduces U~ of the last feasible probe, S10), then all 1024 threads emit X, the CSR
+//     cumulative quotas and the receive layout.
+#include "uep_internal.cuh"
+
+namespace uep {
+
+constexpr unsigned kFull = 0xffffffffu;
+constexpr int kMaxLog = UEP_MAX_R * UEP_MAX_NSLOT;      // 1024 accepted transfers at most
+constexpr int kPcSmem = 2048;                           // phys_count staged in smem if R*P fits
+
+struct PlanSmem {
+  int lam[UEP_MAX_E];
+  int elist[UEP_MAX_E];        // experts grouped by home rank, each group by lambda desc, id asc
+  int home[UEP_MAX_E];
+  int main_phys[UEP_MAX_E];
+  int u_main[UEP_MAX_E];
+  int n_rep[UEP_MAX_E];
+  int first[UEP_MAX_E];
+  int inst_off[UEP_MAX_E + 1];
+  int ell[UEP_MAX_R];
+  int order[UEP_MAX_R];        // ranks by l_r desc, id asc
+  int roff[UEP_MAX_R + 1];
+  int rload[UEP_MAX_R];
+  int log_e[kMaxLog], log_t[kMaxLog], log_slot[kMaxLog], log_d[kMaxLog], dscan[kMaxLog];
+  int pc[kPcSmem];
+  int warp_tmp[32];
+  int feas[32];
+  int lo, hi, n_probes, n_log;
+  long long s_valid;
+  int max_ell;
+};
+
+__device__ __forceinline__ int warp_incl_scan(int v, int lane) {
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int y = __shfl_up_sync(kFull, v, o);
+    if (lane >= o) v += y;
+  }
+  return v;
+}
+
+// Block-wide inclusive scan of one value per thread (1024 threads). tmp: 32 ints of smem.
+__device__ __forceinline__ int block_incl_scan(int v, int* tmp) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int s = warp_incl_scan(v, lane);
+  __syncthreads();
+  if (lane == 31) tmp[w] = s;
+  __syncthreads();
+  if (w == 0) {
+    int t = tmp[lane];
+    t = warp_incl_scan(t, lane);
+    tmp[lane] = t;
+  }
+  __syncthreads();
+  if (w > 0) s += tmp[w - 1];
+  return s;
+}
+
+// One greedy feasibility probe (Alg. 1 lines 6-20) by one warp.  All control flow is
+// warp-uniform.  LOG: also record the accepted transfers.
+template <int RPL, bool LOG>
+__device__ __forceinline__ bool probe(PlanSmem& sm, const int tau, const int R, const int n_slot,
+                                      const int u_min, const bool strict, const int lane,
+                                      int& n_log) {
+  unsigned key[RPL];
+  int used[RPL];
+#pragma unroll
+  for (int i = 0; i < RPL; ++i) {
+    const int t = lane + 32 * i;
+    const int slk = (t < R) ? max(tau - sm.ell[t], 0) : 0;          // line 6
+    used[i] = 0;
+    key[i] = (slk > 0 && n_slot > 0) ? (((unsigned)slk << 8) | (unsigned)(255 - t)) : 0u;
+  }
+  int nl = 0;
+  bool ok = true;
+  bool dead = false;       // no rank can absorb u_min any more: slack only shrinks, so it stays so
+  for (int oi = 0; oi < R; ++oi) {                                  // line 8
+    const int r = sm.order[oi];
+    int exc = sm.ell[r] - tau;
+    if (exc <= 0) break;                       // ranks are sorted: nobody further is overloaded
+    const int a = sm.roff[r], b = sm.roff[r + 1];
+    for (int ei = a; ei < b && exc >= u_min && !dead; ++ei) {       // line 9
+      const int e = sm.elist[ei];
+      int cap = sm.lam[e];                                          // line 10 (S6)
+      if (cap < u_min) break;                  // sorted by lambda: no later expert can pass line 16
+      while (true) {                                                // line 11
+        unsigned kl = key[0];
+#pragma unroll
+        for (int i = 1; i < RPL; ++i) kl = max(kl, key[i]);
+        const unsigned km = __reduce_max_sync(kFull, kl);           // lines 12-14
+        const int s = (int)(km >> 8);
+        if (s < u_min) { dead = true; break; }                      // line 13 (T empty) or line 16
+        const int d = min(exc, min(s, cap));                        // line 15
+        if (d < u_min) break;                                       // line 16
+        const int t = 255 - (int)(km & 255u);
+        int slot = 0;
+#pragma unroll
+        for (int i = 0; i < RPL; ++i) {
+          if (t == lane + 32 * i) {                                 // owner lane: lines 17-19
+            slot = used[i];
+            used[i] += 1;
+            const int ns = s - d;
+            key[i] = (ns > 0 && used[i] < n_slot) ? (((unsigned)ns << 8) | (unsigned)(255 - t)) : 0u;
+          }
+        }
+        if (LOG) {
+          if (lane == (t & 31)) {
+            sm.log_e[nl] = e; sm.log_t[nl] = t; sm.log_slot[nl] = slot; sm.log_d[nl] = d;
+          }
+        }
+        ++nl;
+        exc -= d;
+        cap -= d;
+        if (exc == 0 || cap == 0) break;
+      }
+    }
+    // line 20 per rank (S21 early exit): strict needs exc == 0, tolerant exc < u_min (S8)
+    if (strict ? (exc > 0) : (exc >= u_min)) { ok = false; break; }
+    if (!strict && sm.ell[r] - tau < u_min) break;   // tolerant: every later rank passes too
+  }
+  n_log = nl;
+  return ok;
+}
+
+template <int RPL>
+__global__ void __launch_bounds__(kPlanThreads, 1)
+plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict__ g_home,
+            const int32_t* __restrict__ g_main_phys, const int32_t* __restrict__ g_roff,
+            const int32_t* __restrict__ g_rexp, uep_plan_out out, int E, int R, int n_slot, int M,
+            int P, int u_min, int beta_num, int beta_den, int strict_i, int S_total) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  PlanSmem& sm = *reinterpret_cast<PlanSmem*>(smem_raw);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const bool strict = strict_i != 0;
+
+  // ---- stage inputs ---------------------------------------------------------------------
+  if (tid < E) {
+    sm.lam[tid] = expert_count[tid];
+    sm.home[tid] = g_home[tid];
+    sm.main_phys[tid] = g_main_phys[tid];
+    sm.elist[tid] = g_rexp[tid];
+  }
+  if (tid <= R) sm.roff[tid] = g_roff[tid];
+  __syncthreads();
+  // line 2: l_r
+  if (tid < R) {
+    int s = 0;
+    for (int i = sm.roff[tid]; i < sm.roff[tid + 1]; ++i) s += sm.lam[sm.elist[i]];
+    sm.ell[tid] = s;
+  }
+  __syncthreads();
+  // sum and max of l_r (R <= 256 -> first 8 warps)
+  {
+    int v = (tid < R) ? sm.ell[tid] : 0;
+    int sum = __reduce_add_sync(kFull, v);
+    int mx = __reduce_max_sync(kFull, v);
+    if (lane == 0) { sm.warp_tmp[warp] = sum; sm.feas[warp] = mx; }
+  }
+  __syncthreads();
+  if (tid == 0) {
+    long long sv = 0;
+    int mx = 0;
+    for (int w = 0; w < 32; ++w) { sv += sm.warp_tmp[w]; mx = max(mx, sm.feas[w]); }
+    sm.s_valid = sv;
+    sm.max_ell = mx;
+    // line 3 (S3): tau_lo = floor(beta * ceil(mean)), tau_hi = max l_r
+    const long long mean_ceil = (sv + R - 1) / R;
+    const long long tl = mean_ceil * beta_num / beta_den;
+    sm.lo = (int)min(tl, (long long)0x7fffffff);
+    sm.hi = mx;
+    sm.n_probes = 0;
+    sm.n_log = 0;
+  }
+  // rank order: position = number of ranks that come before (l desc, id asc). warp per rank.
+  for (int r = warp; r < R; r += 32) {
+    const int lr = sm.ell[r];
+    int cnt = 0;
+    for (int q = lane; q < R; q += 32) {
+      const int lq = sm.ell[q];
+      cnt += (lq > lr || (lq == lr && q < r)) ? 1 : 0;
+    }
+    cnt = __reduce_add_sync(kFull, cnt);
+    if (lane == 0) sm.order[cnt] = r;
+  }
+  // per-rank expert order: lambda desc, id asc. warp per expert; positions into u_main (temp).
+  for (int e = warp; e < E; e += 32) {
+    const int h = sm.home[e], le = sm.lam[e];
+    const int a = sm.roff[h], b = sm.roff[h + 1];
+    int cnt = 0;
+    for (int i = a + lane; i < b; i += 32) {
+      const int q = sm.elist[i];
+      const int lq = sm.lam[q];
+      cnt += (lq > le || (lq == le && q < e)) ? 1 : 0;
+    }
+    cnt = __reduce_add_sync(kFull, cnt);
+    if (lane == 0) sm.u_main[e] = a + cnt;
+  }
+  __syncthreads();
+  if (tid < E) sm.elist[sm.u_main[tid]] = tid;
+  __syncthreads();
+  const int tau_lo0 = sm.lo, tau_hi0 = sm.hi;
+
+  // ---- bisection, kPlanLevels levels per round (S9) ---------------------------------------
+  while (true) {
+    const int lo = sm.lo, hi = sm.hi;
+    if (lo >= hi) break;                                            // line 4
+    if (warp >= 1) {
+      const int node = warp;                                        // heap index 1..31
+      const int depth = 31 - __clz(node);
+      int l = lo, h = hi;
+      bool valid = true;
+      for (int L = depth - 1; L >= 0; --L) {
+        if (l >= h) { valid = false; break; }
+        const int mid = (l + h) >> 1;
+        if ((node >> L) & 1) l = mid + 1; else h = mid;             // 1: assumed infeasible
+      }
+      if (l >= h) valid = false;
+      if (valid) {
+        int nl;
+        const bool f = probe<RPL, false>(sm, (l + h) >> 1, R, n_slot, u_min, strict, lane, nl);
+        if (lane == 0) sm.feas[node] = f ? 1 : 0;
+      }
+    }
+    __syncthreads();
+    if (tid == 0) {
+      int node = 1, l = lo, h = hi, np = sm.n_probes;
+      while (node < (1 << kPlanLevels) && l < h) {
+        const int mid = (l + h) >> 1;                               // line 5
+        ++np;
+        if (sm.feas[node]) { h = mid; node = 2 * node; }            // lines 21-22
+        else { l = mid + 1; node = 2 * node + 1; }                  // line 24
+      }
+      sm.lo = l; sm.hi = h; sm.n_probes = np;
+    }
+    __syncthreads();
+  }
+  const int tau = sm.hi;
+
+  // ---- materialise: one logged probe at the final tau (S10) -------------------------------
+  if (warp == 0 && sm.n_probes > 0) {
+    int nl;
+    probe<RPL, true>(sm, tau, R, n_slot, u_min, strict, lane, nl);
+    if (lane == 0) sm.n_log = nl;
+  }
+  if (tid < E) { sm.u_main[tid] = sm.lam[tid]; sm.n_rep[tid] = 0; sm.first[tid] = 0x7fffffff; }
+  const int RP = R * P;
+  const bool pc_in_smem = RP <= kPcSmem;
+  int* pc = pc_in_smem ? sm.pc : out.phys_count;
+  for (int i = tid; i < RP; i += kPlanThreads) pc[i] = 0;
+  for (int i = tid; i < R * n_slot; i += kPlanThreads) out.slot_expert[i] = -1;
+  if (out.U) for (int i = tid; i < E * R; i += kPlanThreads) out.U[i] = 0;
+  __syncthreads();
+  const int n_log = sm.n_log;
+
+  // ---- emit (line 22 "materialize U~ into X" + cumulative reroute metadata, §5.2) ---------
+  if (tid < n_log) {
+    const int e = sm.log_e[tid];
+    atomicSub(&sm.u_main[e], sm.log_d[tid]);
+    atomicAdd(&sm.n_rep[e], 1);
+    atomicMin(&sm.first[e], tid);
+  }
+  __syncthreads();
+  {
+    const int v = (tid < E) ? (1 + sm.n_rep[tid]) : 0;
+    const int inc = block_incl_scan(v, sm.warp_tmp);
+    if (tid < E) sm.inst_off[tid] = inc - v;
+    if (tid == E - 1) sm.inst_off[E] = inc;
+    __syncthreads();
+    const int d = (tid < n_log) ? sm.log_d[tid] : 0;
+    const int ds = block_incl_scan(d, sm.warp_tmp);
+    if (tid < n_log) sm.dscan[tid] = ds;
+  }
+  __syncthreads();
+  if (tid <= E) out.inst_off[tid] = sm.inst_off[tid];
+  int fan = 0;
+  if (tid < E) {
+    const int pos = sm.inst_off[tid], h = sm.home[tid], um = sm.u_main[tid];
+    out.inst_rank[pos] = h;
+    out.inst_phys[pos] = sm.main_phys[tid];
+    out.inst_cum[pos] = um;
+    pc[h * P + sm.main_phys[tid]] = um;
+    if (out.U) out.U[tid * R + h] = um;
+    fan = 1 + sm.n_rep[tid];
+  }
+  if (tid < n_log) {
+    const int e = sm.log_e[tid], t = sm.log_t[tid], sl = sm.log_slot[tid], d = sm.log_d[tid];
+    const int f = sm.first[e];
+    const int pos = sm.inst_off[e] + 1 + (tid - f);                 // S11: acceptance order
+    const int before = (f > 0) ? sm.dscan[f - 1] : 0;
+    out.inst_rank[pos] = t;
+    out.inst_phys[pos] = M + sl;
+    out.inst_cum[pos] = sm.u_main[e] + sm.dscan[tid] - before;
+    out.slot_expert[t * n_slot + sl] = e;                           // X
+    pc[t * P + M + sl] = d;
+    if (out.U) out.U[e * R + t] = d;
+  }
+  for (int i = E + n_log + tid; i < E + R * n_slot; i += kPlanThreads) {   // unused CSR tail
+    out.inst_rank[i] = -1; out.inst_phys[i] = -1; out.inst_cum[i] = 0;
+  }
+  // max fan-out and number of replicated experts
+  {
+    int mf = __reduce_max_sync(kFull, fan);
+    int ng = __reduce_add_sync(kFull, (fan > 1) ? 1 : 0);
+    __syncthreads();                                                // pc complete
+    if (lane == 0) { sm.feas[warp] = mf; sm.warp_tmp[warp] = ng; }
+  }
+  // receive layout (S13): per rank exclusive prefix over its P physical slots
+  int load = 0;
+  if (tid < R) {
+    for (int q = 0; q < P; ++q) {
+      const int cnt = pc[tid * P + q];
+      out.phys_base[tid * P + q] = load;
+      if (pc_in_smem) out.phys_count[tid * P + q] = cnt;
+      load += cnt;
+    }
+    out.rank_load[tid] = load;
+  }
+  __syncthreads();
+  int max_fan = 0, n_groups = 0;
+  if (tid == 0) for (int w = 0; w < 32; ++w) { max_fan = max(max_fan, sm.feas[w]); n_groups += sm.warp_tmp[w]; }
+  __syncthreads();
+  {
+    const int inc = block_incl_scan(load, sm.warp_tmp);
+    if (tid < R) out.rank_base[tid] = inc - load;
+    if (tid == R - 1) out.rank_base[R] = inc;
+    const int mx = __reduce_max_sync(kFull, load);
+    __syncthreads();
+    if (lane == 0) sm.feas[warp] = mx;
+    __syncthreads();
+  }
+  if (tid == 0) {
+    int max_load = 0;
+    for (int w = 0; w < 32; ++w) max_load = max(max_load, sm.feas[w]);
+    out.scalars[UEP_SC_TAU] = tau;
+    out.scalars[UEP_SC_N_REPLICAS] = n_log;
+    out.scalars[UEP_SC_MAX_LOAD] = max_load;
+    out.scalars[UEP_SC_MAX_FANOUT] = max_fan;
+    out.scalars[UEP_SC_N_PROBES] = sm.n_probes;
+    out.scalars[UEP_SC_N_INVALID] = (int)((long long)S_total - sm.s_valid);
+    out.scalars[UEP_SC_TAU_LO0] = tau_lo0;
+    out.scalars[UEP_SC_TAU_HI0] = tau_hi0;
+    out.scalars[UEP_SC_N_GROUPS] = n_groups;
+    for (int i = UEP_SC_N_GROUPS + 1; i < UEP_N_SCALARS; ++i) out.scalars[i] = 0;
+  }
+}
+
+template <int RPL>
+static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out& plan,
+                         cudaStream_t s) {
+  const uep_config& g = c->cfg;
+  plan_kernel<RPL><<<1, kPlanThreads, sizeof(PlanSmem), s>>>(
+      count, c->d_home, c->d_main_phys, c->d_roff, c->d_rexp, plan, g.E, g.R, g.n_slot, c->M, c->P,
+      g.u_min, g.beta_num, g.beta_den, g.floor_mode == UEP_FLOOR_STRICT ? 1 : 0, c->S);
+  UEP_CUDA_TRY(cudaGetLastError());
+  return UEP_OK;
+}
+
+int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s) {
+  const int R = c->cfg.R;
+  if (R <= 32) return launch_plan_t<1>(c, count, plan, s);
+  if (R <= 64) return launch_plan_t<2>(c, count, plan, s);
+  if (R <= 128) return launch_plan_t<4>(c, count, plan, s);
+  return launch_plan_t<8>(c, count, plan, s);
+}
+
+int init_plan_kernels() {
+  const int bytes = (int)sizeof(PlanSmem);
+  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  return UEP_OK;
+}
+
+}  // namespace uep

@@ -1,0 +1,322 @@
+// uep_api.cu — C-ABI entry points: context, argument checks, stage chaining (include/uep.h).
+// Host logic only; every step of the path runs in the kernels of hist.cu / plan.cu /
+// remap.cu / pack.cu.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+#include <algorithm>
+#include "uep_internal.cuh"
+
+namespace uep {
+
+static thread_local char g_cuda_err[256] = "";
+
+int set_cuda_error(cudaError_t e) {
+  std::snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e),
+                cudaGetErrorString(e));
+  return UEP_ERR_CUDA;
+}
+
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+static int check_plan_ptrs(const Ctx* c, const uep_plan_out* p) {
+  if (!p) return UEP_ERR_INVALID_ARG;
+  const void* req[] = {p->slot_expert, p->inst_off,  p->inst_rank, p->inst_phys, p->inst_cum,
+                       p->phys_count,  p->phys_base, p->rank_load, p->rank_base, p->scalars};
+  for (const void* q : req)
+    if (!q || !aligned16(q)) return UEP_ERR_INVALID_ARG;
+  if (p->U && !aligned16(p->U)) return UEP_ERR_INVALID_ARG;
+  (void)c;
+  return UEP_OK;
+}
+
+static int fill_pack_args(int32_t n_tensors, const void* const* src, const size_t* bytes,
+                          void* const* dst, PackArgs& a) {
+  if (n_tensors < 0 || n_tensors > UEP_MAX_TENSORS) return UEP_ERR_INVALID_ARG;
+  a.n_tensors = n_tensors;
+  if (n_tensors && (!src || !bytes || !dst)) return UEP_ERR_INVALID_ARG;
+  for (int j = 0; j < n_tensors; ++j) {
+    if (!src[j] || !dst[j] || !aligned16(src[j]) || !aligned16(dst[j])) return UEP_ERR_INVALID_ARG;
+    if (bytes[j] == 0 || (bytes[j] & 15)) return UEP_ERR_INVALID_ARG;
+    a.src[j] = static_cast<const unsigned char*>(src[j]);
+    a.dst[j] = static_cast<unsigned char*>(dst[j]);
+    a.bytes[j] = bytes[j];
+  }
+  return UEP_OK;
+}
+
+}  // namespace uep
+
+using namespace uep;
+
+extern "C" {
+
+int uep_create(const uep_config* cfg, uep_ctx** out) {
+  if (!cfg || !out) return UEP_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (cfg->T < 0 || cfg->k < 1 || cfg->E < 1 || cfg->R < 1 || cfg->n_slot < 0 ||
+      cfg->u_min < 1 || cfg->beta_num < 1 || cfg->beta_den < 1)
+    return UEP_ERR_INVALID_ARG;
+  if (cfg->floor_mode != UEP_FLOOR_STRICT && cfg->floor_mode != UEP_FLOOR_TOLERANT)
+    return UEP_ERR_INVALID_ARG;
+  if (cfg->gate_dtype < UEP_GATE_F32 || cfg->gate_dtype > UEP_GATE_NONE) return UEP_ERR_INVALID_ARG;
+  if (cfg->E > UEP_MAX_E || cfg->R > UEP_MAX_R || cfg->n_slot > UEP_MAX_NSLOT)
+    return UEP_ERR_UNSUPPORTED;
+  const long long S = (long long)cfg->T * cfg->k;
+  if (S >= (1LL << 24)) return UEP_ERR_UNSUPPORTED;      // planner packs slack into 24 bits
+  if ((long long)cfg->beta_num * ((S + cfg->R - 1) / cfg->R) >= (1LL << 62)) return UEP_ERR_UNSUPPORTED;
+
+  int dev = 0, n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev == 0) { cudaGetLastError(); return UEP_ERR_NO_DEVICE; }
+  UEP_CUDA_TRY(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  UEP_CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major < 10) return UEP_ERR_UNSUPPORTED;       // sm_100a only
+
+  Ctx* c = new (std::nothrow) Ctx();
+  if (!c) return UEP_ERR_INVALID_ARG;
+  std::memset(c, 0, sizeof(Ctx));
+  c->cfg = *cfg;
+  c->cfg.home_rank = nullptr;                            // never retained
+  c->S = (int)S;
+  c->sm_count = prop.multiProcessorCount;
+  const int E = cfg->E, R = cfg->R;
+  c->E_pad = (E + 3) & ~3;
+
+  // static layout (Table 1): h(e), E_r, main slot index
+  std::vector<int32_t> home(E), main_phys(E), roff(R + 1, 0), rexp(E);
+  for (int e = 0; e < E; ++e) {
+    int h = cfg->home_rank ? cfg->home_rank[e] : (int)(((long long)e * R) / E);
+    if (h < 0 || h >= R) { delete c; return UEP_ERR_INVALID_ARG; }
+    home[e] = h;
+    roff[h + 1] += 1;
+  }
+  int M = 0;
+  for (int r = 0; r < R; ++r) { M = std::max(M, roff[r + 1]); roff[r + 1] += roff[r]; }
+  {
+    std::vector<int32_t> fill(R, 0);
+    for (int e = 0; e < E; ++e) {
+      main_phys[e] = fill[home[e]];
+      rexp[roff[home[e]] + fill[home[e]]] = e;
+      fill[home[e]] += 1;
+    }
+  }
+  c->M = M;
+  c->P = M + cfg->n_slot;
+
+  // launch geometry: one histogram/remap CTA per SM, chunk a multiple of 128 slots
+  {
+    long long per = (S + c->sm_count - 1) / c->sm_count;
+    per = std::max<long long>(per, kMinChunk);
+    per = (per + 127) / 128 * 128;
+    c->chunk_len = (int)per;
+    c->n_chunks = (int)std::max<long long>(1, (S + per - 1) / per);
+  }
+  c->pack_ctas = c->sm_count;
+
+  auto fail = [&](int rc) { uep_destroy(reinterpret_cast<uep_ctx*>(c)); return rc; };
+  cudaError_t e;
+#define UEP_TRY_OR_FAIL(x) do { e = (x); if (e != cudaSuccess) return fail(set_cuda_error(e)); } while (0)
+  UEP_TRY_OR_FAIL(cudaMalloc(&c->d_home, sizeof(int32_t) * E));
+  UEP_TRY_OR_FAIL(cudaMalloc(&c->d_main_phys, sizeof(int32_t) * E));
+  UEP_TRY_OR_FAIL(cudaMalloc(&c->d_roff, sizeof(int32_t) * (R + 1)));
+  UEP_TRY_OR_FAIL(cudaMalloc(&c->d_rexp, sizeof(int32_t) * E));
+  UEP_TRY_OR_FAIL(cudaMemcpy(c->d_home, home.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
+  UEP_TRY_OR_FAIL(cudaMemcpy(c->d_main_phys, main_phys.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
+  UEP_TRY_OR_FAIL(cudaMemcpy(c->d_roff, roff.data(), sizeof(int32_t) * (R + 1), cudaMemcpyHostToDevice));
+  UEP_TRY_OR_FAIL(cudaMemcpy(c->d_rexp, rexp.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
+  UEP_TRY_OR_FAIL(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+  UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+  UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+#undef UEP_TRY_OR_FAIL
+  int rc = init_plan_kernels();
+  if (rc == UEP_OK) rc = init_remap_kernels();
+  if (rc == UEP_OK) rc = init_pack_kernels();
+  if (rc != UEP_OK) return fail(rc);
+  *out = reinterpret_cast<uep_ctx*>(c);
+  return UEP_OK;
+}
+
+void uep_destroy(uep_ctx* ctx) {
+  Ctx* c = reinterpret_cast<Ctx*>(ctx);
+  if (!c) return;
+  if (c->d_home) cudaFree(c->d_home);
+  if (c->d_main_phys) cudaFree(c->d_main_phys);
+  if (c->d_roff) cudaFree(c->d_roff);
+  if (c->d_rexp) cudaFree(c->d_rexp);
+  if (c->side) cudaStreamDestroy(c->side);
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+  if (c->ev_join) cudaEventDestroy(c->ev_join);
+  delete c;
+}
+
+size_t uep_workspace_bytes(const uep_ctx* ctx) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c) return 0;
+  return (size_t)kWsHeaderBytes + sizeof(int32_t) * (size_t)c->n_chunks * c->E_pad;
+}
+
+int uep_workspace_init(const uep_ctx* ctx, void* ws, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !ws || !aligned16(ws)) return UEP_ERR_INVALID_ARG;
+  UEP_CUDA_TRY(cudaMemsetAsync(ws, 0, kWsHeaderBytes, static_cast<cudaStream_t>(stream)));
+  return UEP_OK;
+}
+
+int uep_plan_bytes(const uep_ctx* ctx, uep_plan_sizes* out) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !out) return UEP_ERR_INVALID_ARG;
+  const int E = c->cfg.E, R = c->cfg.R, ns = c->cfg.n_slot;
+  out->slot_expert = std::max(1, R * ns);
+  out->inst_off = E + 1;
+  out->inst_cap = E + R * ns;
+  out->phys = R * c->P;
+  out->rank_load = R;
+  out->rank_base = R + 1;
+  out->U = E * R;
+  out->scalars = UEP_N_SCALARS;
+  out->M = c->M;
+  out->P = c->P;
+  return UEP_OK;
+}
+
+int uep_get_launch_info(const uep_ctx* ctx, uep_launch_info* out) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !out) return UEP_ERR_INVALID_ARG;
+  out->n_chunks = c->n_chunks;
+  out->chunk_len = c->chunk_len;
+  out->hist_threads = kHistThreads;
+  out->remap_threads = kRemapThreads;
+  out->plan_threads = kPlanThreads;
+  out->pack_ctas = c->pack_ctas;
+  out->pack_tile_bytes = kPackTile;
+  out->sm_count = c->sm_count;
+  return UEP_OK;
+}
+
+int uep_histogram(const uep_ctx* ctx, const int32_t* topk_ids, int32_t* expert_count, void* ws,
+                  void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !expert_count || !ws || !aligned16(expert_count) || !aligned16(ws))
+    return UEP_ERR_INVALID_ARG;
+  if (c->S > 0 && (!topk_ids || !aligned16(topk_ids))) return UEP_ERR_INVALID_ARG;
+  return launch_histogram(c, topk_ids, expert_count, ws, static_cast<cudaStream_t>(stream));
+}
+
+int uep_plan(const uep_ctx* ctx, const int32_t* expert_count, const uep_plan_out* plan, void* ws,
+             void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  (void)ws;
+  if (!c || !expert_count || !aligned16(expert_count)) return UEP_ERR_INVALID_ARG;
+  int rc = check_plan_ptrs(c, plan);
+  if (rc != UEP_OK) return rc;
+  return launch_plan(c, expert_count, *plan, static_cast<cudaStream_t>(stream));
+}
+
+int uep_remap(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
+              const uep_plan_out* plan, int32_t* out_replica, int32_t* out_rank,
+              int32_t* out_offset, void* out_gate, void* ws, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !ws || !aligned16(ws)) return UEP_ERR_INVALID_ARG;
+  int rc = check_plan_ptrs(c, plan);
+  if (rc != UEP_OK) return rc;
+  if (c->S > 0) {
+    if (!topk_ids || !out_replica || !out_rank || !out_offset) return UEP_ERR_INVALID_ARG;
+    if (!aligned16(topk_ids) || !aligned16(out_replica) || !aligned16(out_rank) ||
+        !aligned16(out_offset))
+      return UEP_ERR_INVALID_ARG;
+  }
+  if ((gate == nullptr) != (out_gate == nullptr)) return UEP_ERR_INVALID_ARG;
+  if (gate && (c->cfg.gate_dtype == UEP_GATE_NONE || !aligned16(gate) || !aligned16(out_gate)))
+    return UEP_ERR_INVALID_ARG;
+  return launch_remap(c, topk_ids, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws,
+                      static_cast<cudaStream_t>(stream));
+}
+
+int uep_pack(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,
+             const void* const* src, const size_t* bytes_per_expert, void* const* dst,
+             void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c) return UEP_ERR_INVALID_ARG;
+  int rc = check_plan_ptrs(c, plan);
+  if (rc != UEP_OK) return rc;
+  PackArgs a;
+  rc = fill_pack_args(n_tensors, src, bytes_per_expert, dst, a);
+  if (rc != UEP_OK) return rc;
+  if (n_tensors == 0 || c->cfg.n_slot == 0) return UEP_OK;
+  return launch_pack(c, *plan, a, static_cast<cudaStream_t>(stream));
+}
+
+int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
+                int32_t* expert_count, const uep_plan_out* plan, int32_t* out_replica,
+                int32_t* out_rank, int32_t* out_offset, void* out_gate, int32_t n_tensors,
+                const void* const* src, const size_t* bytes_per_expert, void* const* dst,
+                void* ws, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c) return UEP_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  PackArgs a;
+  int rc = fill_pack_args(n_tensors, src, bytes_per_expert, dst, a);
+  if (rc != UEP_OK) return rc;
+  rc = uep_histogram(ctx, topk_ids, expert_count, ws, stream);
+  if (rc != UEP_OK) return rc;
+  rc = uep_plan(ctx, expert_count, plan, ws, stream);
+  if (rc != UEP_OK) return rc;
+  const bool do_pack = n_tensors > 0 && c->cfg.n_slot > 0;
+  if (do_pack) {   // fork: pack depends only on the plan and overlaps the remap (Eq. 1)
+    UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
+    UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+  }
+  rc = uep_remap(ctx, topk_ids, gate, plan, out_replica, out_rank, out_offset, out_gate, ws, stream);
+  if (do_pack) {
+    int rc2 = launch_pack(c, *plan, a, c->side);
+    UEP_CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
+    UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_join, 0));
+    if (rc == UEP_OK) rc = rc2;
+  }
+  return rc;
+}
+
+int uep_balance_host(const uep_ctx* ctx, const int32_t* topk_ids_host, const void* gate_host,
+                     int32_t* dev_topk_ids, void* dev_gate, int32_t* expert_count,
+                     const uep_plan_out* plan, int32_t* out_replica, int32_t* out_rank,
+                     int32_t* out_offset, void* out_gate, int32_t* out_replica_host,
+                     int32_t* out_rank_host, int32_t* out_offset_host, void* out_gate_host,
+                     int32_t* scalars_host, int32_t n_tensors, const void* const* src,
+                     const size_t* bytes_per_expert, void* const* dst, void* ws, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !topk_ids_host || !dev_topk_ids || !plan) return UEP_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const size_t S = (size_t)c->S;
+  const size_t gb = c->cfg.gate_dtype == UEP_GATE_F32 ? 4 : (c->cfg.gate_dtype == UEP_GATE_BF16 ? 2 : 0);
+  UEP_CUDA_TRY(cudaMemcpyAsync(dev_topk_ids, topk_ids_host, S * 4, cudaMemcpyHostToDevice, s));
+  const bool has_gate = gate_host && dev_gate && gb;
+  if (has_gate) UEP_CUDA_TRY(cudaMemcpyAsync(dev_gate, gate_host, S * gb, cudaMemcpyHostToDevice, s));
+  int rc = uep_balance(ctx, dev_topk_ids, has_gate ? dev_gate : nullptr, expert_count, plan,
+                       out_replica, out_rank, out_offset, has_gate ? out_gate : nullptr, n_tensors,
+                       src, bytes_per_expert, dst, ws, stream);
+  if (rc != UEP_OK) return rc;
+  if (out_replica_host) UEP_CUDA_TRY(cudaMemcpyAsync(out_replica_host, out_replica, S * 4, cudaMemcpyDeviceToHost, s));
+  if (out_rank_host) UEP_CUDA_TRY(cudaMemcpyAsync(out_rank_host, out_rank, S * 4, cudaMemcpyDeviceToHost, s));
+  if (out_offset_host) UEP_CUDA_TRY(cudaMemcpyAsync(out_offset_host, out_offset, S * 4, cudaMemcpyDeviceToHost, s));
+  if (has_gate && out_gate_host) UEP_CUDA_TRY(cudaMemcpyAsync(out_gate_host, out_gate, S * gb, cudaMemcpyDeviceToHost, s));
+  if (scalars_host) UEP_CUDA_TRY(cudaMemcpyAsync(scalars_host, plan->scalars, sizeof(int32_t) * UEP_N_SCALARS, cudaMemcpyDeviceToHost, s));
+  UEP_CUDA_TRY(cudaStreamSynchronize(s));
+  return UEP_OK;
+}
+
+const char* uep_strerror(int code) {
+  switch (code) {
+    case UEP_OK: return "ok";
+    case UEP_ERR_INVALID_ARG: return "invalid argument (NULL or misaligned pointer, bad size)";
+    case UEP_ERR_UNSUPPORTED: return "unsupported shape or device (limits in uep.h; sm_100 required)";
+    case UEP_ERR_CUDA: return "CUDA error (see uep_last_cuda_error)";
+    case UEP_ERR_NO_DEVICE: return "no CUDA device";
+    default: return "unknown error";
+  }
+}
+
+const char* uep_last_cuda_error(void) { return g_cuda_err; }
+
+}  // extern "C"

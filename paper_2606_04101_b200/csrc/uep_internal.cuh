@@ -1,0 +1,75 @@
+// uep_internal.cuh — shared declarations of the CUDA path (sm_100a only).
+// Nothing here is shared with oracle/ (the CPU oracle is an independent program).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "uep.h"
+
+#if defined(__CUDA_ARCH__) && (__CUDA_ARCH__ < 1000)
+#error "libuep is written for sm_100a (B200) only"
+#endif
+
+namespace uep {
+
+constexpr int kWsHeaderBytes = 256;      // [0] ticket of the histogram's last-CTA reduction
+constexpr int kHistThreads = 1024;
+constexpr int kRemapThreads = 1024;
+constexpr int kRemapWarps = kRemapThreads / 32;
+constexpr int kRemapItems = 16;          // slots per lane per round (register-resident)
+constexpr int kRemapRound = kRemapThreads * kRemapItems;   // 16384 slots per CTA round
+constexpr int kPlanThreads = 1024;
+constexpr int kPlanLevels = 5;           // bisection levels speculated per round (2^5-1 warps)
+constexpr int kPackTile = 16 * 1024;     // bytes per bulk-copy tile
+constexpr int kPackStages = 8;           // shared-memory ring depth
+constexpr int kMinChunk = 2048;          // smallest histogram/remap chunk (slots per CTA)
+
+struct Ctx {
+  uep_config cfg;
+  int S;                  // T*k
+  int M, P;               // main / physical slots per rank
+  int E_pad;              // E rounded up to a multiple of 4 (row pitch of the chunk table)
+  int n_chunks, chunk_len;
+  int sm_count;
+  int pack_ctas;
+  // static layout, device
+  int32_t* d_home;        // [E]   h(e)
+  int32_t* d_main_phys;   // [E]   index of e among E_{h(e)} ascending
+  int32_t* d_roff;        // [R+1] CSR of E_r
+  int32_t* d_rexp;        // [E]   experts grouped by home rank, ascending e
+  // fork/join for uep_balance
+  cudaStream_t side;
+  cudaEvent_t ev_fork, ev_join;
+};
+
+struct PackArgs {
+  const unsigned char* src[UEP_MAX_TENSORS];
+  unsigned char* dst[UEP_MAX_TENSORS];
+  unsigned long long bytes[UEP_MAX_TENSORS];
+  int n_tensors;
+};
+
+int set_cuda_error(cudaError_t e);
+
+int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s);
+int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s);
+int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& plan,
+                 int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
+                 void* ws, cudaStream_t s);
+int launch_pack(const Ctx* c, const uep_plan_out& plan, const PackArgs& a, cudaStream_t s);
+int init_plan_kernels();          // opt-in shared memory attributes
+int init_remap_kernels();
+int init_pack_kernels();
+
+inline int32_t* ws_table(void* ws) {
+  return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes);
+}
+inline unsigned* ws_ticket(void* ws) { return reinterpret_cast<unsigned*>(ws); }
+
+}  // namespace uep
+
+#define UEP_CUDA_TRY(expr)                                   \
+  do {                                                       \
+    cudaError_t _e = (expr);                                 \
+    if (_e != cudaSuccess) return ::uep::set_cuda_error(_e); \
+  } while (0)

@@ -1,0 +1,303 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Bar: bit-exact on every integer / index array and scalar,
+byte-exact pack and gates (all of the path is integer or byte work; there is no floating-point
+tolerance anywhere).  All tests need a B200 and are marked gpu."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import uep_checks as ck
+from paper_2606_04101_b200 import binding, synth
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+PLAN_ARRAYS = ("slot_expert", "inst_off", "inst_rank", "inst_phys", "inst_cum", "phys_count",
+               "phys_base", "rank_load", "rank_base", "scalars", "U")
+
+
+def gpu_chain(ids, gate, E, R, n_slot, u_min, mode=binding.FLOOR_TOLERANT, home=None,
+              states=(), use_balance=False, beta=(101, 100)):
+    """Run hist -> plan -> remap -> pack on the GPU; return host copies of everything."""
+    T, k = ids.shape
+    gd = binding.GATE_NONE if gate is None else \
+        (binding.GATE_BF16 if gate.element_size() == 2 else binding.GATE_F32)
+    ctx = binding.Context(T, k, E, R, n_slot, u_min, beta[0], beta[1], mode, gd, home)
+    ws = ctx.new_workspace()
+    plan = ctx.new_plan(dense_U=True)
+    d_ids = ids.to(DEV)
+    d_gate = None if gate is None else gate.to(DEV)
+    count = torch.full((E,), -7, dtype=torch.int32, device=DEV)
+    rep, rnk, off, og = ctx.new_outputs(d_gate)
+    for t in (rep, rnk, off):
+        t.fill_(-9)
+    srcs = [s.to(DEV) for s in states]
+    sentinels = []
+    for sr in srcs:                       # random bytes: empty slots must survive untouched
+        sn = torch.empty((R, max(n_slot, 1)) + tuple(sr.shape[1:]), dtype=sr.dtype, device=DEV)
+        sn.view(torch.uint8).copy_(torch.randint(0, 256, sn.view(torch.uint8).shape,
+                                                 dtype=torch.uint8, device=DEV))
+        sentinels.append(sn)
+    dsts = [sn.clone() for sn in sentinels]
+    if use_balance:
+        ctx.uep_balance(d_ids, d_gate, count, plan, rep, rnk, off, og, srcs, dsts, ws)
+    else:
+        ctx.uep_histogram(d_ids, count, ws)
+        ctx.uep_plan(count, plan, ws)
+        ctx.uep_remap(d_ids, d_gate, plan, rep, rnk, off, og, ws)
+        if srcs:
+            ctx.uep_pack(plan, srcs, dsts)
+    torch.cuda.synchronize()
+    res = dict(count=count.cpu().numpy(), plan=plan.host(), rep=rep.cpu().numpy(),
+               rnk=rnk.cpu().numpy(), off=off.cpu().numpy(),
+               og=None if og is None else og.cpu(), dsts=[d.cpu() for d in dsts],
+               sentinels=[s.cpu() for s in sentinels], ctx=ctx)
+    return res
+
+
+def oracle_chain(ids, gate, E, R, n_slot, u_min, mode=oracle.FLOOR_TOLERANT, home=None,
+                 beta=(101, 100)):
+    ids_np = ids.numpy()
+    lam, bad = oracle.histogram(ids_np, E)
+    p = oracle.plan(lam, R, n_slot, u_min, beta[0], beta[1], mode, home, S_total=ids_np.size)
+    g_np = None
+    if gate is not None:
+        g_np = gate.view(torch.int16).numpy().view(np.uint16) if gate.element_size() == 2 \
+            else gate.view(torch.int32).numpy().view(np.uint32)
+    rep, rnk, off, og = oracle.remap(ids_np, g_np, p)
+    return lam, p, rep, rnk, off, og
+
+
+def assert_parity(g, o, ids, gate, states=(), n_valid=None):
+    lam, p, rep, rnk, off, og = o
+    assert np.array_equal(g["count"], lam)
+    hp = g["plan"]
+    for n in PLAN_ARRAYS:
+        a, b = getattr(hp, n), getattr(p, n)
+        assert np.array_equal(np.asarray(a).reshape(-1), np.asarray(b).reshape(-1)), n
+    assert np.array_equal(g["rep"], rep) and np.array_equal(g["rnk"], rnk) \
+        and np.array_equal(g["off"], off)
+    if gate is not None:
+        nv = int(p.rank_base[-1])
+        gg = g["og"]
+        gbits = gg.view(torch.int16).numpy().view(np.uint16) if gg.element_size() == 2 \
+            else gg.view(torch.int32).numpy().view(np.uint32)
+        assert np.array_equal(gbits[:nv], og[:nv])
+    for st, d, sn in zip(states, g["dsts"], g["sentinels"]):
+        src_b = st.contiguous().view(torch.uint8).numpy().reshape(st.shape[0], -1)
+        ref = sn.contiguous().view(torch.uint8).numpy().reshape(p.R, max(p.n_slot, 1), -1).copy()
+        if p.n_slot:
+            oracle.pack(p.slot_expert, np.ascontiguousarray(src_b), ref)
+        got = d.contiguous().view(torch.uint8).numpy().reshape(ref.shape)
+        assert np.array_equal(got, ref)
+
+
+def with_layout(hp, home=None):
+    """Attach the static layout (h(e), main slot index) so uep_checks can run on a GPU plan."""
+    hp.home, hp.main_phys, M = oracle.layout(hp.E, hp.R, home)
+    assert M == hp.M
+    return hp
+
+
+def test_tiny_config_full_chain_both_modes():
+    c = synth.CONFIGS["tiny"]
+    ids = synth.zipf_topk_ids(c["T"], c["k"], c["E"], c["zipf_s"], 2024)
+    gate = synth.gates_uniform_renorm(c["T"], c["k"], 11)
+    state = synth.expert_state(c["E"], 256 * 512, 5)
+    for mode in (binding.FLOOR_STRICT, binding.FLOOR_TOLERANT):
+        for use_balance in (False, True):
+            g = gpu_chain(ids, gate, c["E"], c["R"], c["n_slot"], c["u_min"], mode,
+                          states=[state], use_balance=use_balance)
+            o = oracle_chain(ids, gate, c["E"], c["R"], c["n_slot"], c["u_min"], mode)
+            assert_parity(g, o, ids, gate, [state])
+            assert o[1].n_replicas > 0
+
+
+GRID = [  # (T, k, E, R, n_slot, s)  — sizes spanning several chunks/rounds and ragged tails
+    (4099, 2, 16, 4, 1, 1.2), (8191, 8, 128, 32, 2, 0.6), (65536, 8, 128, 32, 2, 1.4),
+    (50001, 8, 256, 64, 2, 1.0), (16384, 4, 512, 256, 4, 2.0), (4097, 1, 64, 8, 1, 0.0),
+    (8192, 8, 160, 40, 4, 1.0), (2048, 4, 64, 256, 1, 1.0), (30011, 8, 512, 8, 3, 1.6),
+    (1, 1, 1, 1, 0, 0.0), (3, 2, 5, 3, 2, 0.5), (131, 1, 7, 2, 1, 1.0), (700000, 4, 500, 250, 3, 1.1),
+]
+
+
+@pytest.mark.parametrize("T,k,E,R,n_slot,s", GRID)
+@pytest.mark.parametrize("mode", [binding.FLOOR_STRICT, binding.FLOOR_TOLERANT])
+def test_grid_parity(T, k, E, R, n_slot, s, mode):
+    ids = synth.zipf_topk_ids(T, k, E, s, seed=T + E + R)
+    gate = synth.gates_uniform_renorm(T, k, 3)
+    u_min = synth.stress_u_min(T * k, R)
+    state = synth.expert_state(E, 1000 * 8 + 8, 1)     # ragged: 16016 B per expert, < one tile
+    g = gpu_chain(ids, gate, E, R, n_slot, u_min, mode, states=[state])
+    o = oracle_chain(ids, gate, E, R, n_slot, u_min, mode)
+    assert_parity(g, o, ids, gate, [state])
+
+
+STRESS = [  # (S, k, E, R, n_slot, dist)
+    (1024, 1, 64, 8, 1, "uniform"), (1024, 4, 256, 64, 2, "zipf2"), (4096, 8, 512, 256, 4, "one"),
+    (262144, 8, 64, 256, 3, "zipf2"), (262144, 4, 256, 8, 1, "one"), (1 << 20, 8, 512, 64, 2, "uniform"),
+    (1 << 22, 8, 256, 64, 4, "zipf2"), (1 << 22, 8, 512, 256, 4, "one"), (1 << 22, 1, 64, 8, 1, "uniform"),
+    (1 << 22, 4, 512, 256, 1, "zipf2"),
+]
+
+
+@pytest.mark.parametrize("S,k,E,R,n_slot,dist", STRESS)
+def test_stress_sweep_parity(S, k, E, R, n_slot, dist):
+    T = S // k
+    if dist == "one":
+        ids = synth.one_expert_ids(T, k, E // 3)
+    else:
+        ids = synth.zipf_topk_ids(T, k, E, 2.0 if dist == "zipf2" else 0.0, seed=S + E)
+    gate = synth.gates_uniform_renorm(T, k, 9)
+    u_min = synth.stress_u_min(S, R)
+    state = synth.expert_state(E, 2048 * 16, 2)         # 64 KiB per expert: 4 tiles
+    g = gpu_chain(ids, gate, E, R, n_slot, u_min, states=[state])
+    o = oracle_chain(ids, gate, E, R, n_slot, u_min)
+    assert_parity(g, o, ids, gate, [state])
+    ck.check_plan(o[0], with_layout(g["plan"]), u_min)
+
+
+def test_invalid_ids_gate_bits_and_bf16():
+    rng = np.random.default_rng(3)
+    T, k, E, R = 20000, 4, 16, 4
+    ids = torch.from_numpy(rng.integers(-3, 20, size=(T, k)).astype(np.int32))
+    bits = (np.arange(T * k, dtype=np.uint32) * np.uint32(2654435761)).astype(np.uint32)
+    bits[:8] = [0x7FC00001, 0xFFC12345, 0x80000000, 0x00000001, 0x807FFFFF, 0x7F800000,
+                0xFF800000, 0x7FA00000]
+    gate = torch.from_numpy(bits.view(np.float32).reshape(T, k).copy())
+    g = gpu_chain(ids, gate, E, R, 1, 32)
+    o = oracle_chain(ids, gate, E, R, 1, 32)
+    assert_parity(g, o, ids, gate)
+    assert int(g["plan"].scalars[binding.SC_N_INVALID]) == int(((ids < 0) | (ids >= E)).sum())
+    gate16 = synth.gates_softmax_bf16(T, k, 4)
+    g = gpu_chain(ids, gate16, E, R, 1, 32)
+    o = oracle_chain(ids, gate16, E, R, 1, 32)
+    assert_parity(g, o, ids, gate16)
+    g = gpu_chain(ids, None, E, R, 1, 32)                # no gates at all
+    o = oracle_chain(ids, None, E, R, 1, 32)
+    assert_parity(g, o, ids, None)
+
+
+def test_explicit_home_map_and_identity_cases():
+    rng = np.random.default_rng(8)
+    T, k, E, R = 30000, 4, 64, 8
+    ids = synth.zipf_topk_ids(T, k, E, 1.0, 77)
+    home = rng.integers(0, R, E).astype(np.int32)
+    g = gpu_chain(ids, None, E, R, 3, 256, home=home)
+    o = oracle_chain(ids, None, E, R, 3, 256, home=home)
+    assert_parity(g, o, ids, None)
+    # balanced input -> identity (S4); n_slot = 0; R = 1
+    ids_b = (torch.arange(T * k, dtype=torch.int32) % E).view(T, k)
+    for (RR, ns) in ((8, 2), (8, 0), (1, 2)):
+        for ii in (ids_b, ids):
+            g = gpu_chain(ii, None, E, RR, ns, 16)
+            o = oracle_chain(ii, None, E, RR, ns, 16)
+            assert_parity(g, o, ii, None)
+
+
+def test_multi_tensor_pack_training_state():
+    """config-3 style moved state: bf16 W + fp32 grad/m/v, several tiles and a ragged last tile."""
+    T, k, E, R, ns = 32768, 8, 64, 16, 2
+    ids = synth.zipf_topk_ids(T, k, E, 1.3, 5)
+    n = 40000 + 8                                        # 80016 B bf16 / 160032 B fp32 per expert
+    states = [synth.expert_state(E, n, 1), synth.expert_state(E, n, 2, torch.float32),
+              synth.expert_state(E, n, 3, torch.float32), synth.expert_state(E, n, 4, torch.float32)]
+    g = gpu_chain(ids, None, E, R, ns, 512, states=states, use_balance=True)
+    o = oracle_chain(ids, None, E, R, ns, 512)
+    assert o[1].n_replicas > 4
+    assert_parity(g, o, ids, None, states)
+
+
+@pytest.mark.parametrize("name,s", [("glm_air", 0.6), ("glm_air", 1.4), ("dsv3_prefill", 1.0)])
+def test_full_size_configs_bit_exact(name, s):
+    """BASELINE configs 1 and 2 at full size, in the launch configuration bench.py times
+    (uep_balance): every integer output against the oracle, element by element."""
+    c = synth.CONFIGS[name]
+    ids = synth.zipf_topk_ids(c["T"], c["k"], c["E"], s, 4242, device=DEV).cpu()
+    gate = synth.gates_softmax_bf16(c["T"], c["k"], 6) if c["gate"] == "bf16" \
+        else synth.gates_uniform_renorm(c["T"], c["k"], 6)
+    state = synth.expert_state(c["E"], 1 << 20, 3)       # 2 MiB per expert stands in for 88 MB
+    g = gpu_chain(ids, gate, c["E"], c["R"], c["n_slot"], c["u_min"], states=[state],
+                  use_balance=True)
+    o = oracle_chain(ids, gate, c["E"], c["R"], c["n_slot"], c["u_min"])
+    assert_parity(g, o, ids, gate, [state])
+    ck.check_plan(o[0], with_layout(g["plan"]), c["u_min"])
+    ck.check_remap(ids.numpy(), g["plan"], g["rep"], g["rnk"], g["off"])
+
+
+def test_graph_capture_replay_and_determinism():
+    c = synth.CONFIGS["glm_air"]
+    T, k, E, R, ns = 16384, c["k"], c["E"], c["R"], c["n_slot"]
+    ctx = binding.Context(T, k, E, R, ns, 256)
+    ws = ctx.new_workspace()
+    plan = ctx.new_plan(dense_U=True)
+    d_ids = torch.zeros((T, k), dtype=torch.int32, device=DEV)
+    d_gate = torch.zeros((T, k), dtype=torch.float32, device=DEV)
+    count = torch.zeros(E, dtype=torch.int32, device=DEV)
+    rep, rnk, off, og = ctx.new_outputs(d_gate)
+    state = synth.expert_state(E, 20000, 1, device=DEV)
+    dst = torch.zeros((R, ns, 20000), dtype=state.dtype, device=DEV)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(stream):
+        ctx.uep_balance(d_ids, d_gate, count, plan, rep, rnk, off, og, [state], [dst], ws)  # warm
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            ctx.uep_balance(d_ids, d_gate, count, plan, rep, rnk, off, og, [state], [dst], ws)
+    torch.cuda.synchronize()
+    prev = None
+    for it, seed in enumerate((1, 2, 2)):
+        ids = synth.zipf_topk_ids(T, k, E, 0.8 + 0.4 * seed, seed)
+        gate = synth.gates_uniform_renorm(T, k, seed)
+        d_ids.copy_(ids)
+        d_gate.copy_(gate)
+        dst.zero_()
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        g = dict(count=count.cpu().numpy(), plan=plan.host(), rep=rep.cpu().numpy(),
+                 rnk=rnk.cpu().numpy(), off=off.cpu().numpy(), og=og.cpu(), dsts=[dst.cpu()],
+                 sentinels=[torch.zeros_like(dst).cpu()])
+        o = oracle_chain(ids, gate, E, R, ns, 256)
+        assert_parity(g, o, ids, gate, [state.cpu()])
+        if it == 2:                                       # same input twice: bit-identical
+            for a, b in zip(prev, (g["rep"], g["rnk"], g["off"], g["og"].numpy())):
+                assert np.array_equal(a, b)
+        prev = (g["rep"], g["rnk"], g["off"], g["og"].numpy())
+
+
+def test_error_codes_and_empty_input():
+    with pytest.raises(binding.UepError):
+        binding.Context(16, 2, 513, 4, 1, 8)             # E > UEP_MAX_E
+    with pytest.raises(binding.UepError):
+        binding.Context(16, 2, 16, 4, 5, 8)              # n_slot > 4
+    with pytest.raises(binding.UepError):
+        binding.Context(16, 2, 16, 4, 1, 0)              # u_min < 1
+    with pytest.raises(binding.UepError):
+        binding.Context(1 << 22, 8, 16, 4, 1, 8)         # S >= 2^24
+    ctx = binding.Context(1024, 2, 16, 4, 1, 8)
+    ws = ctx.new_workspace()
+    plan = ctx.new_plan()
+    count = torch.zeros(16, dtype=torch.int32, device=DEV)
+    ids = torch.zeros((1024, 2), dtype=torch.int32, device=DEV)
+    with pytest.raises(binding.UepError):                # misaligned ids pointer
+        ctx.uep_histogram(ids.view(-1)[1:], count, ws)
+    src = torch.zeros((16, 24), dtype=torch.uint8, device=DEV)     # 24 B per expert: not % 16
+    dst = torch.zeros((4, 1, 24), dtype=torch.uint8, device=DEV)
+    with pytest.raises(binding.UepError):
+        ctx.uep_pack(plan, [src], [dst])
+    # T = 0: everything runs, identity plan
+    ctx0 = binding.Context(0, 2, 16, 4, 1, 8)
+    ws0 = ctx0.new_workspace()
+    p0 = ctx0.new_plan()
+    e_ids = torch.zeros((0, 2), dtype=torch.int32, device=DEV)
+    r0, k0, o0, _ = ctx0.new_outputs(None)
+    ctx0.uep_balance(e_ids, None, count, p0, r0, k0, o0, None, [], [], ws0)
+    torch.cuda.synchronize()
+    assert int(count.sum()) == 0 and int(p0.scalars[binding.SC_N_REPLICAS]) == 0
+    op = oracle.plan(np.zeros(16, np.int32), 4, 1, 8)
+    hp = p0.host()
+    for n in PLAN_ARRAYS[:-1]:
+        assert np.array_equal(np.asarray(getattr(hp, n)).reshape(-1),
+                              np.asarray(getattr(op, n)).reshape(-1)), n
