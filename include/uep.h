@@ -80,7 +80,7 @@ typedef struct uep_config {
 typedef struct uep_plan_sizes {
   int32_t slot_expert;           /* R*n_slot (>=1 allocated)                                      */
   int32_t inst_off;              /* E+1                                                           */
-  int32_t inst_cap;              /* E + R*n_slot : inst_rank / inst_phys / inst_cum               */
+  int32_t inst_cap;              /* E + R*n_slot : inst_rank / inst_phys / inst_cum / inst_base   */
   int32_t phys;                  /* R*P : phys_count / phys_base                                  */
   int32_t rank_load;             /* R                                                             */
   int32_t rank_base;             /* R+1                                                           */
@@ -97,6 +97,8 @@ typedef struct uep_plan_sizes {
  *                           host rank, local physical slot on that rank (main e -> its index
  *                           among E_{h(e)} ascending; redundant slot s -> M+s), and the
  *                           INCLUSIVE cumulative quota (last = lambda_e)
+ *   inst_base[]             offset of the instance's first token inside its host rank's receive
+ *                           buffer = phys_base[inst_rank][inst_phys] (S13), same indexing
  *   phys_count/base[R][P]   tokens received per local physical slot and their exclusive prefix
  *   rank_load[R]            sum_e u_{e,t};  rank_base[R+1] its exclusive prefix (last = #valid)
  *   scalars[UEP_N_SCALARS]  see UEP_SC_*
@@ -107,6 +109,7 @@ typedef struct uep_plan_out {
   int32_t* inst_rank;
   int32_t* inst_phys;
   int32_t* inst_cum;
+  int32_t* inst_base;
   int32_t* phys_count;
   int32_t* phys_base;
   int32_t* rank_load;
@@ -123,7 +126,7 @@ void uep_destroy(uep_ctx* ctx);
 
 /* Bytes of DEVICE workspace one in-flight call needs.  It carries the per-chunk expert counts
  * from uep_histogram to uep_remap (their exclusive prefix over chunks gives each slot's global
- * stable rank).  uep_workspace_init must be called once (async on `stream`) before first use. */
+ * stable rank; uep_remap forms that prefix itself).  uep_workspace_init must be called once (async on `stream`) before first use. */
 size_t uep_workspace_bytes(const uep_ctx* ctx);
 int uep_workspace_init(const uep_ctx* ctx, void* ws, void* stream);
 int uep_plan_bytes(const uep_ctx* ctx, uep_plan_sizes* out);      /* out: HOST */
@@ -131,7 +134,7 @@ int uep_plan_bytes(const uep_ctx* ctx, uep_plan_sizes* out);      /* out: HOST *
 /* lambda_e = #{slots s : topk_ids[s] == e} (Alg. 1 line 2).
  *   topk_ids      DEVICE int32 [T,k] row-major (slot s = i*k + kk)
  *   expert_count  DEVICE int32 [E], overwritten
- *   ws            DEVICE workspace; afterwards holds the chunk prefix table for uep_remap    */
+ *   ws            DEVICE workspace; afterwards holds the chunk count table for uep_remap    */
 int uep_histogram(const uep_ctx* ctx, const int32_t* topk_ids, int32_t* expert_count, void* ws,
                   void* stream);
 

@@ -43,7 +43,7 @@ class _PlanSizes(ctypes.Structure):
                  "scalars", "M", "P")]
 
 
-_PLAN_FIELDS = ("slot_expert", "inst_off", "inst_rank", "inst_phys", "inst_cum", "phys_count",
+_PLAN_FIELDS = ("slot_expert", "inst_off", "inst_rank", "inst_phys", "inst_cum", "inst_base", "phys_count",
                 "phys_base", "rank_load", "rank_base", "scalars", "U")
 
 
@@ -110,6 +110,7 @@ class Plan:
     inst_rank: torch.Tensor
     inst_phys: torch.Tensor
     inst_cum: torch.Tensor
+    inst_base: torch.Tensor
     phys_count: torch.Tensor
     phys_base: torch.Tensor
     rank_load: torch.Tensor
@@ -182,7 +183,7 @@ class Context:
         sz = self.sizes
         z = lambda n: torch.zeros(max(int(n), 1), dtype=torch.int32, device=self.device)
         p = Plan(self.E, self.R, self.n_slot, sz.M, sz.P, z(sz.slot_expert), z(sz.inst_off),
-                 z(sz.inst_cap), z(sz.inst_cap), z(sz.inst_cap), z(sz.phys), z(sz.phys),
+                 z(sz.inst_cap), z(sz.inst_cap), z(sz.inst_cap), z(sz.inst_cap), z(sz.phys), z(sz.phys),
                  z(sz.rank_load), z(sz.rank_base), z(sz.scalars), z(sz.U) if dense_U else None)
         p.c = _PlanOut(*[_ptr(getattr(p, n)).value or 0 for n in _PLAN_FIELDS])
         return p

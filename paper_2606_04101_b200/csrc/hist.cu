@@ -1,14 +1,19 @@
 // hist.cu — uep_histogram: lambda_e = #{s : topk_ids[s] == e}  (Alg. 1 line 2).
 //
-// HBM-bound: 4 B/slot read once.  One CTA per chunk (one chunk per SM), int4-vectorised
-// coalesced loads issued up front, a per-CTA shared-memory histogram (E <= 512), one row of
-// the chunk table written per CTA.  The last CTA to finish (ticket) turns the table into its
-// exclusive prefix over chunks — what uep_remap needs for global stable ranks — and emits the
-// column totals as expert_count.  No float, no order-dependent atomics: results are
-// bit-identical run to run.
+// HBM-bound: 4 B/slot read once.  One CTA per chunk (one chunk per SM).  Every thread issues
+// all of its int4 loads of a round before it touches shared memory (kHistVecs x 16 B in flight
+// per thread, 64 KB per SM), then counts into a WARP-PRIVATE shared-memory row (pitch E_pad+1
+// so the same expert in different rows falls into different banks): no contention between
+// warps on a hot expert, only the intra-warp multiplicity.  The CTA's row of the chunk table
+// (raw counts; uep_remap builds its own prefix over chunks from it) is written once.  The last
+// CTA to finish (ticket) sums the table's columns with one round of independent int4 L2 loads
+// and emits expert_count.  Integer adds only: bit-identical run to run.
 #include "uep_internal.cuh"
 
 namespace uep {
+
+constexpr int kHistWarps = kHistThreads / 32;
+constexpr int kHistVecs = 4;                                  // int4 loads per thread per round
 
 __device__ __forceinline__ int4 ld_stream_v4(const int4* p) {
   int4 r;
@@ -17,49 +22,69 @@ __device__ __forceinline__ int4 ld_stream_v4(const int4* p) {
   return r;
 }
 
-__device__ __forceinline__ void count_one(int* hist, int e, int E) {
-  if ((unsigned)e < (unsigned)E) atomicAdd(&hist[e], 1);
+__device__ __forceinline__ void count_one(int* row, int e, int E) {
+  if ((unsigned)e < (unsigned)E) atomicAdd(&row[e], 1);
 }
 
-constexpr int kHistUnroll = 4;
+// dynamic shared memory (ints): priv[kHistWarps][E_pad+1] | part[kColPartInts] | tot[E_pad]
+__host__ __device__ inline size_t hist_smem_ints(int E_pad) {
+  return (size_t)kHistWarps * (E_pad + 1) + kColPartInts + E_pad;
+}
 
 __global__ void __launch_bounds__(kHistThreads, 1)
 hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len,
             int n_chunks, int32_t* __restrict__ table, unsigned* __restrict__ ticket,
             int32_t* __restrict__ expert_count) {
-  __shared__ int hist[UEP_MAX_E];
-  __shared__ int part[kHistThreads];
+  extern __shared__ __align__(16) int hsm[];
+  const int pitch = E_pad + 1;
+  int* priv = hsm;
+  int* part = hsm + ((kHistWarps * pitch + 3) & ~3);
+  int* tot = part + kColPartInts;
   __shared__ unsigned s_last;
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, warp = tid >> 5;
   const int c = blockIdx.x;
-  for (int e = tid; e < E_pad; e += kHistThreads) hist[e] = 0;
-  __syncthreads();
 
   const long long begin = (long long)c * chunk_len;
   const int len = (int)min((long long)chunk_len, (long long)S - begin);   // > 0 by construction
   const int n_vec = len >> 2;
   const int4* v = reinterpret_cast<const int4*>(ids + begin);             // chunk_len % 128 == 0
-  int i = tid;
-  for (; i + (kHistUnroll - 1) * kHistThreads < n_vec; i += kHistUnroll * kHistThreads) {
-    int4 x[kHistUnroll];
+
+  // first round's loads go out before the shared-memory rows are zeroed
+  int4 x[kHistVecs];
 #pragma unroll
-    for (int u = 0; u < kHistUnroll; ++u) x[u] = ld_stream_v4(v + i + u * kHistThreads);
-#pragma unroll
-    for (int u = 0; u < kHistUnroll; ++u) {
-      count_one(hist, x[u].x, E); count_one(hist, x[u].y, E);
-      count_one(hist, x[u].z, E); count_one(hist, x[u].w, E);
-    }
+  for (int u = 0; u < kHistVecs; ++u) {
+    const int i = u * kHistThreads + tid;
+    x[u] = (i < n_vec) ? ld_stream_v4(v + i) : make_int4(-1, -1, -1, -1);
   }
-  for (; i < n_vec; i += kHistThreads) {
-    int4 x = ld_stream_v4(v + i);
-    count_one(hist, x.x, E); count_one(hist, x.y, E);
-    count_one(hist, x.z, E); count_one(hist, x.w, E);
-  }
-  if (tid < (len & 3)) count_one(hist, ids[begin + (n_vec << 2) + tid], E);   // ragged tail
+  for (int i = tid; i < kHistWarps * pitch; i += kHistThreads) priv[i] = 0;
   __syncthreads();
 
-  int32_t* row = table + (size_t)c * E_pad;
-  for (int e = tid; e < E_pad; e += kHistThreads) row[e] = hist[e];
+  int* row = priv + warp * pitch;
+  for (int vbase = 0; vbase < n_vec; vbase += kHistThreads * kHistVecs) {
+#pragma unroll
+    for (int u = 0; u < kHistVecs; ++u) {
+      count_one(row, x[u].x, E); count_one(row, x[u].y, E);
+      count_one(row, x[u].z, E); count_one(row, x[u].w, E);
+    }
+    const int nb = vbase + kHistThreads * kHistVecs;
+    if (nb < n_vec) {
+#pragma unroll
+      for (int u = 0; u < kHistVecs; ++u) {
+        const int i = nb + u * kHistThreads + tid;
+        x[u] = (i < n_vec) ? ld_stream_v4(v + i) : make_int4(-1, -1, -1, -1);
+      }
+    }
+  }
+  if (tid < (len & 3)) count_one(row, ids[begin + (n_vec << 2) + tid], E);   // ragged tail
+  __syncthreads();
+
+  int32_t* grow = table + (size_t)c * E_pad;
+  for (int e = tid; e < E_pad; e += kHistThreads) {
+    int s = 0;
+#pragma unroll 8
+    for (int w = 0; w < kHistWarps; ++w) s += priv[w * pitch + e];
+    grow[e] = s;
+  }
   __threadfence();
   __syncthreads();
   if (tid == 0) s_last = (atomicAdd(ticket, 1u) == (unsigned)(n_chunks - 1));
@@ -67,32 +92,9 @@ hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
   if (!s_last) return;
   __threadfence();
 
-  // Last CTA: exclusive prefix over chunks, per expert column; totals -> expert_count.
-  // G thread groups split the rows; each (column, group) thread walks its row segment.
-  const int G = max(1, min(kHistThreads / E_pad, n_chunks));
-  const int seg = (n_chunks + G - 1) / G;
-  const int col = tid % E_pad, g = tid / E_pad;
-  const bool act = (tid < E_pad * G);
-  const int r0 = g * seg, r1 = min(n_chunks, r0 + seg);
-  int sum = 0;
-  if (act) {
-#pragma unroll 8
-    for (int r = r0; r < r1; ++r) sum += __ldcg(table + (size_t)r * E_pad + col);
-    part[tid] = sum;
-  }
-  __syncthreads();
-  if (act) {
-    int run = 0;
-    for (int gg = 0; gg < g; ++gg) run += part[gg * E_pad + col];
-#pragma unroll 8
-    for (int r = r0; r < r1; ++r) {
-      int32_t* p = table + (size_t)r * E_pad + col;
-      const int x = __ldcg(p);
-      *p = run;
-      run += x;
-    }
-    if (g == G - 1 && col < E) expert_count[col] = run;
-  }
+  // Last CTA: column totals -> expert_count.
+  column_sums(table, n_chunks, E_pad, part, tot);
+  for (int e = tid; e < E; e += kHistThreads) expert_count[e] = tot[e];
   if (tid == 0) *ticket = 0u;        // self-reset: the next launch (graph replay) starts clean
 }
 
@@ -104,12 +106,20 @@ __global__ void hist_empty_kernel(int E, int E_pad, int32_t* table, int32_t* exp
   }
 }
 
+int init_hist_kernels() {
+  UEP_CUDA_TRY(cudaFuncSetAttribute(hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)(sizeof(int) * (hist_smem_ints(UEP_MAX_E) + 4))));
+  return UEP_OK;
+}
+
 int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s) {
   if (c->S == 0) {
     hist_empty_kernel<<<1, 256, 0, s>>>(c->cfg.E, c->E_pad, ws_table(ws), count);
   } else {
-    hist_kernel<<<c->n_chunks, kHistThreads, 0, s>>>(ids, c->S, c->cfg.E, c->E_pad, c->chunk_len,
-                                                     c->n_chunks, ws_table(ws), ws_ticket(ws), count);
+    const size_t smem = sizeof(int) * (hist_smem_ints(c->E_pad) + 4);
+    hist_kernel<<<c->n_chunks, kHistThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
+                                                        c->chunk_len, c->n_chunks, ws_table(ws),
+                                                        ws_ticket(ws), count);
   }
   UEP_CUDA_TRY(cudaGetLastError());
   return UEP_OK;

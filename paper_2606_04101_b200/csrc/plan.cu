@@ -311,7 +311,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (out.U) out.U[e * R + t] = d;
   }
   for (int i = E + n_log + tid; i < E + R * n_slot; i += kPlanThreads) {   // unused CSR tail
-    out.inst_rank[i] = -1; out.inst_phys[i] = -1; out.inst_cum[i] = 0;
+    out.inst_rank[i] = -1; out.inst_phys[i] = -1; out.inst_cum[i] = 0; out.inst_base[i] = 0;
   }
   // max fan-out and number of replicated experts
   {
@@ -326,12 +326,21 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     for (int q = 0; q < P; ++q) {
       const int cnt = pc[tid * P + q];
       out.phys_base[tid * P + q] = load;
-      if (pc_in_smem) out.phys_count[tid * P + q] = cnt;
+      if (pc_in_smem) { out.phys_count[tid * P + q] = cnt; pc[tid * P + q] = load; }
       load += cnt;
     }
     out.rank_load[tid] = load;
   }
   __syncthreads();
+  // inst_base: offset of each instance's first token in its rank's receive buffer (S13)
+  {
+    const int* pb = pc_in_smem ? pc : out.phys_base;      // bases (global ones are CTA-visible now)
+    if (tid < E) out.inst_base[sm.inst_off[tid]] = pb[sm.home[tid] * P + sm.main_phys[tid]];
+    if (tid < n_log) {
+      const int e = sm.log_e[tid];
+      out.inst_base[sm.inst_off[e] + 1 + (tid - sm.first[e])] = pb[sm.log_t[tid] * P + M + sm.log_slot[tid]];
+    }
+  }
   int max_fan = 0, n_groups = 0;
   if (tid == 0) for (int w = 0; w < 32; ++w) { max_fan = max(max_fan, sm.feas[w]); n_groups += sm.warp_tmp[w]; }
   __syncthreads();

@@ -22,7 +22,7 @@ static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t
 
 static int check_plan_ptrs(const Ctx* c, const uep_plan_out* p) {
   if (!p) return UEP_ERR_INVALID_ARG;
-  const void* req[] = {p->slot_expert, p->inst_off,  p->inst_rank, p->inst_phys, p->inst_cum,
+  const void* req[] = {p->slot_expert, p->inst_off,  p->inst_rank, p->inst_phys, p->inst_cum, p->inst_base,
                        p->phys_count,  p->phys_base, p->rank_load, p->rank_base, p->scalars};
   for (const void* q : req)
     if (!q || !aligned16(q)) return UEP_ERR_INVALID_ARG;
@@ -131,6 +131,7 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
 #undef UEP_TRY_OR_FAIL
   int rc = init_plan_kernels();
+  if (rc == UEP_OK) rc = init_hist_kernels();
   if (rc == UEP_OK) rc = init_remap_kernels();
   if (rc == UEP_OK) rc = init_pack_kernels();
   if (rc != UEP_OK) return fail(rc);

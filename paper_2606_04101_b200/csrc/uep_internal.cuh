@@ -61,6 +61,40 @@ int init_plan_kernels();          // opt-in shared memory attributes
 int init_remap_kernels();
 int init_pack_kernels();
 
+int init_hist_kernels();
+
+// ---- column sums of the chunk table (device) ---------------------------------------------------
+// out[e] = sum_{r < n_rows} table[r][e] for e < E_pad.  Whole CTA (1024 threads) must call it.
+// int4 loads, every thread's loads independent (one L2 round trip), partials in `part`
+// (kColPartInts ints of shared memory), result in `out` (shared).  Ends with a __syncthreads().
+constexpr int kColPartInts = 4096;
+#ifdef __CUDACC__
+__device__ __forceinline__ void column_sums(const int32_t* __restrict__ table, int n_rows, int E_pad,
+                                            int* part, int* out) {
+  const int tid = threadIdx.x;
+  const int CG = E_pad >> 2;                                // int4 column groups per row
+  const int NRG = min(32, (int)blockDim.x / CG);            // row groups; NRG*E_pad <= kColPartInts
+  const int cg = tid % CG, rg = tid / CG;
+  if (rg < NRG) {
+    int4 acc = make_int4(0, 0, 0, 0);
+    const int4* col = reinterpret_cast<const int4*>(table) + cg;
+#pragma unroll 5
+    for (int r = rg; r < n_rows; r += NRG) {
+      const int4 v = __ldcg(col + (size_t)r * CG);
+      acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+    }
+    reinterpret_cast<int4*>(part)[rg * CG + cg] = acc;
+  }
+  __syncthreads();
+  for (int e = tid; e < E_pad; e += blockDim.x) {
+    int s = 0;
+    for (int g = 0; g < NRG; ++g) s += part[g * E_pad + e];
+    out[e] = s;
+  }
+  __syncthreads();
+}
+#endif
+
 inline int32_t* ws_table(void* ws) {
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes);
 }

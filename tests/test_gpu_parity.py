@@ -76,6 +76,12 @@ def assert_parity(g, o, ids, gate, states=(), n_valid=None):
     for n in PLAN_ARRAYS:
         a, b = getattr(hp, n), getattr(p, n)
         assert np.array_equal(np.asarray(a).reshape(-1), np.asarray(b).reshape(-1)), n
+    # inst_base is a derived view of the oracle's receive layout: phys_base[inst_rank][inst_phys]
+    n_inst = int(p.inst_off[-1])
+    exp_base = np.asarray(p.phys_base).reshape(p.R, -1)[np.asarray(p.inst_rank)[:n_inst],
+                                                        np.asarray(p.inst_phys)[:n_inst]]
+    assert np.array_equal(np.asarray(hp.inst_base)[:n_inst], exp_base), "inst_base"
+    assert not np.asarray(hp.inst_base)[n_inst:].any()
     assert np.array_equal(g["rep"], rep) and np.array_equal(g["rnk"], rnk) \
         and np.array_equal(g["off"], off)
     if gate is not None:
