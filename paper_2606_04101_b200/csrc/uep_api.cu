@@ -109,7 +109,7 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   {
     long long per = (S + c->sm_count - 1) / c->sm_count;
     per = std::max<long long>(per, kMinChunk);
-    per = (per + 127) / 128 * 128;
+    per = (per + 1023) / 1024 * 1024;    // whole 1024-slot steps: remap rounds are unpredicated
     c->chunk_len = (int)per;
     c->n_chunks = (int)std::max<long long>(1, (S + per - 1) / per);
   }
