@@ -5,62 +5,143 @@
 // (rank, offset) inside that rank's receive buffer; gate copied bit-exact (moved as raw
 // 16/32-bit integers, S17).
 //
-// HBM-bound by its bytes (4 B id + g B gate read, 12 B + g B written per slot), but on a
-// 50 MB problem the limiter is the INSTRUCTION count of the stable ranking (integer pipes
-// issue one warp instruction per two cycles), so the kernel is built to rank a slot in as
-// few instructions as possible:
-//   * one CTA per chunk, every warp owns a contiguous span and loads its ids and gates up
-//     front (coalesced 128 B per warp-load, unpredicated when the round is full);
-//   * ranking inside a warp uses a warp-private shared-memory row of {peer mask, count} cells:
-//     lanes OR their lane bit into the cell of their expert, read {mask, count} back with one
-//     64-bit load, and the lowest peer stores {0, count + popc(mask)}.  Rank = count +
-//     popc(mask & lower lanes): stable by construction, no order-dependent atomic result is
-//     ever used (the OR is commutative);
-//   * one cross-warp scan per expert column turns the counts into CTA-wide bases; the CTA's own
-//     base comes from summing the chunk-table rows below it (independent int4 L2 loads, in
-//     flight together with the id loads);
-//   * lookup: per CTA and expert one 16-B record describes the instance holding the CTA's first
-//     slot of that expert; a slot only walks further when it crosses a quota edge;
-//   * gates are staged in shared memory in (expert, rank) order and written as contiguous runs
-//     (a scatter of 4-B stores costs one L2 request per lane).
+// Two kernels, split at the only data dependence on the plan:
+//   rank_kernel   (plan-INDEPENDENT) stable rank of every slot among the slots of the same
+//                 expert inside its chunk, packed with the expert id into one int32 per slot in
+//                 the workspace.  uep_balance runs it on a side stream concurrently with
+//                 uep_histogram and uep_plan, so it is off the critical path gate -> dispatch.
+//   lookup_kernel (plan-DEPENDENT) global rank = chunk base (column sums of the chunk-table rows
+//                 below, independent int4 L2 loads) + rank in chunk; cumulative-quota lookup;
+//                 writes (replica, rank, offset) and the gates in dispatch order.
+//
+// rank_kernel: one CTA per chunk (<= 16384 slots, register-resident), every warp owns a
+// contiguous span and loads its ids up front (coalesced).  Ranking inside a warp uses a
+// warp-private shared-memory row of {peer mask, count} cells: lanes OR their lane bit into the
+// cell of their expert, read {mask, count} back with one 64-bit load, and the lowest peer stores
+// {0, count + popc(mask)}.  Rank = count + popc(mask & lower lanes): stable by construction, no
+// order-dependent atomic result is ever used (the OR is commutative).  One cross-warp scan per
+// expert column turns the counts into chunk-wide bases.
+//
+// lookup_kernel: per CTA and expert one 16-B record describes the instance holding the CTA's
+// first slot of that expert; a slot only walks further when it crosses a quota edge.  Gates are
+// staged in shared memory in (expert, rank) order together with their destination index and
+// written out as contiguous runs (a scatter of 4-B stores costs one L2 request per lane).
 #include "uep_internal.cuh"
 
 namespace uep {
 
 constexpr unsigned kFullMask = 0xffffffffu;
 constexpr size_t kMaxSmem = 227 * 1024;
+constexpr int kEMask = (1 << kPackedEBits) - 1;
 
-// dynamic shared memory layout (ints):
-//   wrow[kRemapWarps][E_pad] (int2) | rec[E_pad] (int4) | base[E_pad] | base0[E_pad] | elb[E_pad]
-//   | s_off[E_pad+4] | rbase[(R+7)&~3] | i_cum | i_dbase | i_gbase | i_rank (inst_cap each) | wtot[32]
-//   | scratch: part[kColPartInts] during staging, then (STAGE) the gate staging buffer
-__host__ __device__ inline size_t remap_fixed_ints(int E_pad, int R, int inst_cap) {
-  return 2 * (size_t)kRemapWarps * E_pad + 4 * (size_t)E_pad + 3 * (size_t)E_pad + (E_pad + 4) +
-         ((R + 7) & ~3) + 4 * (size_t)((inst_cap + 3) & ~3) + 32;
+// ------------------------------------------------------------------------------------------------
+// rank_kernel.  dynamic shared memory: wrow[kRemapWarps][E_pad] (int2 {mask, count})
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kRemapThreads, 1)
+rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len,
+            int32_t* __restrict__ packed) {
+  extern __shared__ __align__(16) int smem[];
+  int2* wrow = reinterpret_cast<int2*>(smem);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const unsigned lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
+  const long long cbegin = (long long)blockIdx.x * chunk_len;
+  const int clen = (int)min((long long)chunk_len, (long long)S - cbegin);      // <= kMaxChunk
+  const int items = (clen + kRemapThreads - 1) / kRemapThreads;                // steps per warp
+  const bool full = (clen == items * kRemapThreads);
+  const int wbeg = warp * items * 32;
+  const int room = full ? 0x7fffffff : clen - wbeg - lane;   // step i in range iff i*32 < room
+  ids += cbegin + wbeg + lane;
+  packed += cbegin + wbeg + lane;
+
+  int ev[kRemapItems];
+#pragma unroll
+  for (int i = 0; i < kRemapItems; ++i)
+    ev[i] = (i < items && i * 32 < room) ? __ldg(ids + i * 32) : -1;
+  {
+    int4* z = reinterpret_cast<int4*>(wrow);
+    for (int i = tid; i < kRemapWarps * E_pad / 2; i += kRemapThreads) z[i] = make_int4(0, 0, 0, 0);
+  }
+  __syncthreads();
+
+  // stable rank inside the warp span: steps in order, lanes in order
+  int2* wr = wrow + warp * E_pad;
+#pragma unroll
+  for (int i = 0; i < kRemapItems; ++i) {
+    if (i < items) {
+      const int e = ev[i];
+      const bool valid = (unsigned)e < (unsigned)E;
+      int2* cell = wr + (valid ? e : 0);
+      if (valid) atomicOr(reinterpret_cast<unsigned*>(&cell->x), lane_bit);
+      __syncwarp();
+      const int2 mc = *cell;                                        // {peer mask, count so far}
+      __syncwarp();
+      const unsigned m = (unsigned)mc.x;
+      if (valid && (m & lt_mask) == 0u) *cell = make_int2(0, mc.y + __popc(m));   // lowest peer
+      __syncwarp();                                                 // cell cleared before the next step
+      ev[i] = valid ? (e | ((mc.y + __popc(m & lt_mask)) << kPackedEBits)) : -1;
+    }
+  }
+  __syncthreads();
+
+  // cross-warp exclusive scan per expert column; the count field becomes the base of (warp, e)
+  for (int e = tid; e < E; e += kRemapThreads) {
+    int run = 0;
+#pragma unroll 8
+    for (int w = 0; w < kRemapWarps; ++w) {
+      const int x = wrow[w * E_pad + e].y;
+      wrow[w * E_pad + e].y = run;
+      run += x;
+    }
+  }
+  __syncthreads();
+
+#pragma unroll
+  for (int i = 0; i < kRemapItems; ++i) {
+    if (i < items && i * 32 < room) {
+      const int pk = ev[i];
+      packed[i * 32] = (pk >= 0) ? pk + (wr[pk & kEMask].y << kPackedEBits) : -1;
+    }
+  }
 }
-__host__ __device__ inline size_t remap_smem_bytes(int E_pad, int R, int inst_cap, bool stage,
-                                                   int gate_bytes) {
+
+int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s) {
+  if (c->S == 0) return UEP_OK;
+  const size_t smem = sizeof(int2) * (size_t)kRemapWarps * c->E_pad;
+  rank_kernel<<<c->n_chunks, kRemapThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad, c->chunk_len,
+                                                       ws_packed(c, ws));
+  UEP_CUDA_TRY(cudaGetLastError());
+  return UEP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// lookup_kernel.  dynamic shared memory layout (ints):
+//   rec[E_pad] (int4) | base0[E_pad] | elb[E_pad] | s_off[E_pad+4] | rbase[(R+7)&~3]
+//   | i_cum | i_dbase | i_gbase | i_rank (icap each) | wtot[36]
+//   | scratch: part[kColPartInts] while staging, then (STAGE) sg[kMaxChunk] gates + sd[kMaxChunk] ints
+// ------------------------------------------------------------------------------------------------
+__host__ __device__ inline size_t lookup_smem_bytes(int E_pad, int R, int inst_cap, bool stage,
+                                                    int gate_bytes) {
+  const size_t fixed = 4 * (size_t)E_pad + 2 * (size_t)E_pad + (E_pad + 4) + ((R + 7) & ~3) +
+                       4 * (size_t)((inst_cap + 3) & ~3) + 36;
   size_t scratch = sizeof(int) * (size_t)kColPartInts;
-  const size_t sg = (size_t)kRemapRound * gate_bytes;
-  if (stage && sg > scratch) scratch = sg;
-  return sizeof(int) * remap_fixed_ints(E_pad, R, inst_cap) + scratch;
+  const size_t st = (size_t)kMaxChunk * (gate_bytes + sizeof(int));
+  if (stage && st > scratch) scratch = st;
+  return sizeof(int) * fixed + scratch;
 }
 
 template <typename GateT, bool STAGE>
 __global__ void __launch_bounds__(kRemapThreads, 1)
-remap_kernel(const int32_t* __restrict__ ids, const GateT* __restrict__ gate, int S, int E,
-             int E_pad, int R, int inst_cap, int chunk_len, const int32_t* __restrict__ table,
-             const int32_t* __restrict__ g_inst_off, const int32_t* __restrict__ g_inst_rank,
-             const int32_t* __restrict__ g_inst_cum, const int32_t* __restrict__ g_inst_base,
-             const int32_t* __restrict__ g_rank_base, int32_t* __restrict__ out_replica,
-             int32_t* __restrict__ out_rank, int32_t* __restrict__ out_offset,
-             GateT* __restrict__ out_gate) {
+lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate, int S, int E,
+              int E_pad, int R, int inst_cap, int chunk_len, const int32_t* __restrict__ table,
+              const int32_t* __restrict__ g_inst_off, const int32_t* __restrict__ g_inst_rank,
+              const int32_t* __restrict__ g_inst_cum, const int32_t* __restrict__ g_inst_base,
+              const int32_t* __restrict__ g_rank_base, int32_t* __restrict__ out_replica,
+              int32_t* __restrict__ out_rank, int32_t* __restrict__ out_offset,
+              GateT* __restrict__ out_gate) {
   extern __shared__ __align__(16) int smem[];
-  int2* wrow = reinterpret_cast<int2*>(smem);                       // [warps][E_pad] {mask, count}
-  int4* rec = reinterpret_cast<int4*>(wrow + kRemapWarps * E_pad);  // [E_pad] fast-path record
-  int* base = reinterpret_cast<int*>(rec + E_pad);                  // [E_pad] running rank base of the CTA
-  int* base0 = base + E_pad;                     // [E_pad] base at the start of the round
-  int* elb = base0 + E_pad;                      // [E_pad] staging position of rank j is elb[e] + j
+  int4* rec = reinterpret_cast<int4*>(smem);     // [E_pad] fast-path record per expert
+  int* base0 = reinterpret_cast<int*>(rec + E_pad);   // [E_pad] global rank of the chunk's first slot of e
+  int* elb = base0 + E_pad;                      // [E_pad] staging position of chunk rank jl is elb[e] + jl
   int* s_off = elb + E_pad;                      // [E+1]
   int* rbase = s_off + (E_pad + 4);              // [R+1]
   const int icap = (inst_cap + 3) & ~3;
@@ -68,51 +149,34 @@ remap_kernel(const int32_t* __restrict__ ids, const GateT* __restrict__ gate, in
   int* i_dbase = i_cum + icap;                   // inst_base - cum_prev
   int* i_gbase = i_dbase + icap;                 // rank_base[rank] + i_dbase
   int* i_rank = i_gbase + icap;
-  int* wtot = i_rank + icap;                     // [32]
-  int* part = wtot + 32;                         // column-sum partials (staging only)
-  GateT* sg = reinterpret_cast<GateT*>(part);    // gate staging buffer (after staging)
+  int* wtot = i_rank + icap;                     // [32] warp totals, [32] = chunk total
+  int* part = wtot + 36;                         // column-sum partials (staging only)
+  GateT* sg = reinterpret_cast<GateT*>(part);    // staged gates, (expert, rank) order
+  int* sd = reinterpret_cast<int*>(sg + kMaxChunk);   // their out_gate index
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const unsigned lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
   const int c = blockIdx.x;
   const long long cbegin = (long long)c * chunk_len;
   const int clen = (int)min((long long)chunk_len, (long long)S - cbegin);
+  const int items = (clen + kRemapThreads - 1) / kRemapThreads;
+  const bool full = (clen == items * kRemapThreads);
+  const int wbeg = warp * items * 32;
+  const int room = full ? 0x7fffffff : clen - wbeg - lane;
   const bool has_gate = gate != nullptr;
-  ids += cbegin; out_replica += cbegin; out_rank += cbegin; out_offset += cbegin;
-  if (has_gate) gate += cbegin;
+  const long long tbeg = cbegin + wbeg + lane;
+  packed += tbeg; out_replica += tbeg; out_rank += tbeg; out_offset += tbeg;
+  if (has_gate) gate += tbeg;
 
-  int ev[kRemapItems];
+  int pv[kRemapItems];
   GateT gv[kRemapItems];
-  // loads of one round: warp w owns slots [w*span, (w+1)*span) of the round, step i covers
-  // 32 consecutive slots (one coalesced 128-B line of ids)
-  auto load_round = [&](int wbeg, int rend, int items, bool full) {
-    const int32_t* ip = ids + wbeg + lane;
-    const GateT* gp = gate + wbeg + lane;
-    if (full) {
 #pragma unroll
-      for (int i = 0; i < kRemapItems; ++i) {
-        if (i < items) {
-          ev[i] = __ldg(ip + i * 32);
-          if (has_gate) gv[i] = __ldg(gp + i * 32);
-        }
-      }
-    } else {
-      const int room = rend - wbeg - lane;                        // slot i*32 is in range iff i*32 < room
-#pragma unroll
-      for (int i = 0; i < kRemapItems; ++i) {
-        const bool in = (i < items) && (i * 32 < room);
-        ev[i] = in ? __ldg(ip + i * 32) : -1;
-        if (has_gate) gv[i] = in ? __ldg(gp + i * 32) : GateT(0);
-      }
-    }
-  };
-  {
-    const int rlen = min(kRemapRound, clen);
-    const int items = (rlen + kRemapThreads - 1) / kRemapThreads;
-    load_round(warp * items * 32, rlen, items, rlen == items * kRemapThreads);
+  for (int i = 0; i < kRemapItems; ++i) {
+    const bool in = (i < items) && (i * 32 < room);
+    pv[i] = in ? __ldg(packed + i * 32) : -1;
+    if (has_gate) gv[i] = in ? __ldg(gate + i * 32) : GateT(0);
   }
 
-  // ---- this CTA's base ranks: column sums of the table rows below its own (loads in flight) ----
+  // ---- chunk base ranks: column sums of the table rows below this chunk (loads in flight) ------
   const int CG = E_pad >> 2;
   const int NRG = min(32, kRemapThreads / CG);
   {
@@ -128,6 +192,7 @@ remap_kernel(const int32_t* __restrict__ ids, const GateT* __restrict__ gate, in
       reinterpret_cast<int4*>(part)[rg * CG + cg] = acc;
     }
   }
+  const int n_own = (tid < E) ? __ldcg(table + (size_t)c * E_pad + tid) : 0;   // slots of e in this chunk
   // ---- stage the plan (coalesced, L2-resident) ---------------------------------------------------
   for (int e = tid; e <= E; e += kRemapThreads) s_off[e] = g_inst_off[e];
   for (int r = tid; r <= R; r += kRemapThreads) rbase[r] = g_rank_base[r];
@@ -139,16 +204,25 @@ remap_kernel(const int32_t* __restrict__ ids, const GateT* __restrict__ gate, in
     if (p + 1 < inst_cap) i_dbase[p + 1] = cum;  // cum_prev of the next entry
     if (p == 0) i_dbase[0] = 0;
   }
-  {
-    int4* z = reinterpret_cast<int4*>(wrow);
-    for (int i = tid; i < kRemapWarps * E_pad / 2; i += kRemapThreads) z[i] = make_int4(0, 0, 0, 0);
+  int el_inc = n_own;                            // inclusive scan of n_own over experts
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int y = __shfl_up_sync(kFullMask, el_inc, o);
+    if (lane >= o) el_inc += y;
   }
+  if (lane == 31) wtot[warp] = el_inc;
   __syncthreads();
   for (int e = tid; e < E_pad; e += kRemapThreads) {
     int sum = 0;
     for (int g = 0; g < NRG; ++g) sum += part[g * E_pad + e];
-    base[e] = sum;
+    base0[e] = sum;
     if (e < E) i_dbase[s_off[e]] = 0;            // first instance of an expert: cum_prev = 0
+  }
+  {
+    int pre = 0;
+    for (int w = 0; w < warp; ++w) pre += wtot[w];
+    if (tid < E) elb[tid] = pre + el_inc - n_own;
+    if (tid == kRemapThreads - 1) wtot[32] = pre + el_inc;          // valid slots in this chunk
   }
   __syncthreads();
   const int n_inst = s_off[E];
@@ -158,165 +232,105 @@ remap_kernel(const int32_t* __restrict__ ids, const GateT* __restrict__ gate, in
     i_gbase[p] = rbase[i_rank[p]] + d;
   }
   __syncthreads();
-  // rec[e] = {cum, dbase, gbase, rep<<16|rank} of the instance holding rank base[e]
-  auto make_rec = [&](int e, int pstart) {
-    const int lo = s_off[e], last = s_off[e + 1] - 1, j = base[e];
-    int p = pstart < lo ? lo : pstart;
-    while (p < last && i_cum[p] <= j) ++p;
-    rec[e] = make_int4(i_cum[p], i_dbase[p], i_gbase[p], ((p - lo) << 16) | i_rank[p]);
-  };
-  for (int e = tid; e < E; e += kRemapThreads) make_rec(e, 0);
+  // rec[e], in chunk-rank space: {cum - base0, dbase + base0, gbase + base0, rep<<16|rank} of the
+  // instance holding the chunk's first slot of e
+  for (int e = tid; e < E; e += kRemapThreads) {
+    const int lo = s_off[e], last = s_off[e + 1] - 1, b0 = base0[e];
+    int p = lo;
+    while (p < last && i_cum[p] <= b0) ++p;
+    rec[e] = make_int4(i_cum[p] - b0, i_dbase[p] + b0, i_gbase[p] + b0, ((p - lo) << 16) | i_rank[p]);
+  }
+  __syncthreads();
 
-  // ---- rounds of up to kRemapRound slots -----------------------------------------------------
-  for (int rbeg = 0; rbeg < clen; rbeg += kRemapRound) {
-    const int rlen = min(kRemapRound, clen - rbeg);
-    const int items = (rlen + kRemapThreads - 1) / kRemapThreads;   // steps per warp, <= kRemapItems
-    const int wbeg = rbeg + warp * items * 32;                      // offset inside the chunk
-    const bool full = (rlen == items * kRemapThreads);
-    if (rbeg > 0) {
-      __syncthreads();                                              // previous round done with wrow, rec, sg
-      load_round(wbeg, rbeg + rlen, items, full);
-      int4* z = reinterpret_cast<int4*>(wrow);
-      for (int i = tid; i < kRemapWarps * E_pad / 2; i += kRemapThreads) z[i] = make_int4(0, 0, 0, 0);
-      for (int e = tid; e < E; e += kRemapThreads) make_rec(e, s_off[e] + (rec[e].w >> 16));
-    }
-    __syncthreads();                                                // rows zeroed, plan staged, rec ready
-
-    // stable rank inside the warp span: steps in order, lanes in order
-    int2* wr = wrow + warp * E_pad;
 #pragma unroll
-    for (int i = 0; i < kRemapItems; ++i) {
-      if (i < items) {
-        const int e = ev[i];
-        const bool valid = (unsigned)e < (unsigned)E;
-        int2* cell = wr + (valid ? e : 0);
-        if (valid) atomicOr(reinterpret_cast<unsigned*>(&cell->x), lane_bit);
-        __syncwarp();
-        const int2 mc = *cell;                                      // {peer mask, count so far}
-        __syncwarp();
-        const unsigned m = (unsigned)mc.x;
-        if (valid && (m & lt_mask) == 0u) *cell = make_int2(0, mc.y + __popc(m));   // lowest peer
-        __syncwarp();                                               // cell cleared before the next step
-        ev[i] = valid ? (e | ((mc.y + __popc(m & lt_mask)) << 10)) : -1;   // e | rank in warp span
-      }
-    }
-    __syncthreads();
-
-    // cross-warp exclusive scan per expert column; the count field becomes the base of (warp, e)
-    {
-      int n = 0, old = 0;
-      if (tid < E) {
-        int run = base[tid];
-        old = run;
-#pragma unroll 8
-        for (int w = 0; w < kRemapWarps; ++w) {
-          const int x = wrow[w * E_pad + tid].y;
-          wrow[w * E_pad + tid].y = run;
-          run += x;
-        }
-        base[tid] = run;
-        base0[tid] = old;
-        n = run - old;
-      }
-      if (STAGE && has_gate) {                                      // staging offsets: scan of n over e
-        int inc = n;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const int y = __shfl_up_sync(kFullMask, inc, o);
-          if (lane >= o) inc += y;
-        }
-        if (lane == 31) wtot[warp] = inc;
-        __syncthreads();
-        int pre = 0;
-        for (int w = 0; w < warp; ++w) pre += wtot[w];
-        if (tid < E) elb[tid] = pre + inc - n - old;
-      }
-    }
-    __syncthreads();
-
-    int32_t* o_rep = out_replica + wbeg + lane;
-    int32_t* o_rnk = out_rank + wbeg + lane;
-    int32_t* o_off = out_offset + wbeg + lane;
-    const int room = full ? 0x7fffffff : rbeg + rlen - wbeg - lane;
-#pragma unroll
-    for (int i = 0; i < kRemapItems; ++i) {
-      if (i < items && i * 32 < room) {
-        const int pk = ev[i];
-        int rep = -1, rk = -1, of = -1;
-        if (pk >= 0) {
-          const int e = pk & 1023;
-          const int j = wr[e].y + (pk >> 10);            // global stable rank among slots of e
-          const int4 rc = rec[e];
-          int db = rc.y, gb = rc.z, rr = rc.w;
-          if (j >= rc.x) {                               // past the first instance of this CTA's window
-            int p = s_off[e] + (rr >> 16) + 1;
-            const int last = s_off[e + 1] - 1;           // cum[last] = lambda_e > j when ws matches plan
-            while (p < last && i_cum[p] <= j) ++p;
-            db = i_dbase[p]; gb = i_gbase[p]; rr = ((p - s_off[e]) << 16) | i_rank[p];
-          }
-          rep = rr >> 16;
-          rk = rr & 0xffff;
-          of = db + j;
-          if (has_gate) {
-            if (STAGE) sg[elb[e] + j] = gv[i];
-            else out_gate[gb + j] = gv[i];
-          }
-        }
-        o_rep[i * 32] = rep;
-        o_rnk[i * 32] = rk;
-        o_off[i * 32] = of;
-      }
-    }
-
-    if (STAGE && has_gate) {                             // write the staged gates as contiguous runs
-      __syncthreads();
-      for (int e = warp; e < E; e += kRemapWarps) {
-        const int j1 = base[e], off = elb[e];
-        int p = s_off[e] + (rec[e].w >> 16);
-        const int last = s_off[e + 1] - 1;
-        for (int j = base0[e] + lane; j < j1; j += 32) {
+  for (int i = 0; i < kRemapItems; ++i) {
+    if (i < items && i * 32 < room) {
+      const int pk = pv[i];
+      int rep = -1, rk = -1, of = -1;
+      if (pk >= 0) {
+        const int e = pk & kEMask, jl = pk >> kPackedEBits;
+        const int4 rc = rec[e];
+        int db = rc.y, gb = rc.z, rr = rc.w;
+        if (jl >= rc.x) {                                // past the first instance of this chunk's window
+          const int b0 = base0[e], j = jl + b0;
+          int p = s_off[e] + (rr >> 16) + 1;
+          const int last = s_off[e + 1] - 1;             // cum[last] = lambda_e > j when ws matches plan
           while (p < last && i_cum[p] <= j) ++p;
-          out_gate[i_gbase[p] + j] = sg[off + j];
+          db = i_dbase[p] + b0; gb = i_gbase[p] + b0; rr = ((p - s_off[e]) << 16) | i_rank[p];
+        }
+        rep = rr >> 16;
+        rk = rr & 0xffff;
+        of = db + jl;
+        if (has_gate) {
+          if (STAGE) {
+            const int lp = elb[e] + jl;
+            sg[lp] = gv[i];
+            sd[lp] = gb + jl;
+          } else {
+            out_gate[gb + jl] = gv[i];
+          }
         }
       }
+      out_replica[i * 32] = rep;
+      out_rank[i * 32] = rk;
+      out_offset[i * 32] = of;
+    }
+  }
+
+  if (STAGE && has_gate) {                               // staged gates leave as contiguous runs
+    __syncthreads();
+    const int n_valid = wtot[32];
+#pragma unroll
+    for (int i = 0; i < kRemapItems; ++i) {
+      const int lp = i * kRemapThreads + tid;
+      if (lp < n_valid) out_gate[sd[lp]] = sg[lp];
     }
   }
 }
 
 template <typename GateT>
-static int launch_remap_t(const Ctx* c, const int32_t* ids, const GateT* gate,
-                          const uep_plan_out& p, int32_t* out_replica, int32_t* out_rank,
-                          int32_t* out_offset, GateT* out_gate, void* ws, cudaStream_t s) {
+static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& p,
+                           int32_t* out_replica, int32_t* out_rank, int32_t* out_offset,
+                           GateT* out_gate, void* ws, cudaStream_t s) {
   const uep_config& g = c->cfg;
   const int inst_cap = g.E + g.R * g.n_slot;
-  const bool stage = gate && remap_smem_bytes(c->E_pad, g.R, inst_cap, true, sizeof(GateT)) <= kMaxSmem;
-  const size_t smem = remap_smem_bytes(c->E_pad, g.R, inst_cap, stage, sizeof(GateT));
-  auto k = stage ? remap_kernel<GateT, true> : remap_kernel<GateT, false>;
+  const bool stage = gate != nullptr;
+  const size_t smem = lookup_smem_bytes(c->E_pad, g.R, inst_cap, stage, sizeof(GateT));
+  auto k = stage ? lookup_kernel<GateT, true> : lookup_kernel<GateT, false>;
   k<<<c->n_chunks, kRemapThreads, smem, s>>>(
-      ids, gate, c->S, g.E, c->E_pad, g.R, inst_cap, c->chunk_len, ws_table(ws), p.inst_off,
-      p.inst_rank, p.inst_cum, p.inst_base, p.rank_base, out_replica, out_rank, out_offset, out_gate);
+      ws_packed(c, ws), gate, c->S, g.E, c->E_pad, g.R, inst_cap, c->chunk_len, ws_table(ws),
+      p.inst_off, p.inst_rank, p.inst_cum, p.inst_base, p.rank_base, out_replica, out_rank,
+      out_offset, out_gate);
   UEP_CUDA_TRY(cudaGetLastError());
   return UEP_OK;
 }
 
 int init_remap_kernels() {
   const int bytes = (int)kMaxSmem;
-  UEP_CUDA_TRY(cudaFuncSetAttribute(remap_kernel<uint32_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(remap_kernel<uint32_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(remap_kernel<uint16_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(remap_kernel<uint16_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(rank_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint16_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint16_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   return UEP_OK;
+}
+
+int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& p, int32_t* out_replica,
+                  int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s) {
+  if (c->S == 0) return UEP_OK;
+  if (c->cfg.gate_dtype == UEP_GATE_BF16 && gate)
+    return launch_lookup_t<uint16_t>(c, static_cast<const uint16_t*>(gate), p, out_replica, out_rank,
+                                     out_offset, static_cast<uint16_t*>(out_gate), ws, s);
+  return launch_lookup_t<uint32_t>(c, static_cast<const uint32_t*>(gate), p, out_replica, out_rank,
+                                   out_offset, static_cast<uint32_t*>(out_gate), ws, s);
 }
 
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& p,
                  int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
                  void* ws, cudaStream_t s) {
-  if (c->S == 0) return UEP_OK;
-  if (c->cfg.gate_dtype == UEP_GATE_BF16 && gate)
-    return launch_remap_t<uint16_t>(c, ids, static_cast<const uint16_t*>(gate), p, out_replica,
-                                    out_rank, out_offset, static_cast<uint16_t*>(out_gate), ws, s);
-  return launch_remap_t<uint32_t>(c, ids, static_cast<const uint32_t*>(gate), p, out_replica,
-                                  out_rank, out_offset, static_cast<uint32_t*>(out_gate), ws, s);
+  int rc = launch_rank(c, ids, ws, s);
+  if (rc != UEP_OK) return rc;
+  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s);
 }
 
 }  // namespace uep

@@ -105,11 +105,14 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   c->M = M;
   c->P = M + cfg->n_slot;
 
-  // launch geometry: one histogram/remap CTA per SM, chunk a multiple of 128 slots
+  // launch geometry: one histogram/rank/lookup CTA per chunk; one chunk per SM while a chunk fits
+  // the register-resident round of the rank kernel (kMaxChunk slots), more chunks beyond that.
+  // Chunks are whole 1024-slot steps so that every chunk but the last runs unpredicated.
   {
     long long per = (S + c->sm_count - 1) / c->sm_count;
     per = std::max<long long>(per, kMinChunk);
-    per = (per + 1023) / 1024 * 1024;    // whole 1024-slot steps: remap rounds are unpredicated
+    per = (per + 1023) / 1024 * 1024;
+    per = std::min<long long>(per, kMaxChunk);
     c->chunk_len = (int)per;
     c->n_chunks = (int)std::max<long long>(1, (S + per - 1) / per);
   }
@@ -129,6 +132,7 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   UEP_TRY_OR_FAIL(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
   UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
   UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+  UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_rank, cudaEventDisableTiming));
 #undef UEP_TRY_OR_FAIL
   int rc = init_plan_kernels();
   if (rc == UEP_OK) rc = init_hist_kernels();
@@ -149,13 +153,14 @@ void uep_destroy(uep_ctx* ctx) {
   if (c->side) cudaStreamDestroy(c->side);
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);
+  if (c->ev_rank) cudaEventDestroy(c->ev_rank);
   delete c;
 }
 
 size_t uep_workspace_bytes(const uep_ctx* ctx) {
   const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
   if (!c) return 0;
-  return (size_t)kWsHeaderBytes + sizeof(int32_t) * (size_t)c->n_chunks * c->E_pad;
+  return (size_t)kWsHeaderBytes + ws_table_bytes(c) + sizeof(int32_t) * (((size_t)c->S + 63) & ~(size_t)63);
 }
 
 int uep_workspace_init(const uep_ctx* ctx, void* ws, void* stream) {
@@ -260,23 +265,40 @@ int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
   PackArgs a;
   int rc = fill_pack_args(n_tensors, src, bytes_per_expert, dst, a);
   if (rc != UEP_OK) return rc;
-  rc = uep_histogram(ctx, topk_ids, expert_count, ws, stream);
+  // argument checks of the remap stage up front: the rank kernel is launched first
+  if (!ws || !aligned16(ws)) return UEP_ERR_INVALID_ARG;
+  rc = check_plan_ptrs(c, plan);
   if (rc != UEP_OK) return rc;
-  rc = uep_plan(ctx, expert_count, plan, ws, stream);
-  if (rc != UEP_OK) return rc;
+  if (c->S > 0) {
+    if (!topk_ids || !out_replica || !out_rank || !out_offset) return UEP_ERR_INVALID_ARG;
+    if (!aligned16(topk_ids) || !aligned16(out_replica) || !aligned16(out_rank) ||
+        !aligned16(out_offset))
+      return UEP_ERR_INVALID_ARG;
+  }
+  if ((gate == nullptr) != (out_gate == nullptr)) return UEP_ERR_INVALID_ARG;
+  if (gate && (c->cfg.gate_dtype == UEP_GATE_NONE || !aligned16(gate) || !aligned16(out_gate)))
+    return UEP_ERR_INVALID_ARG;
+  // fork: the plan-independent half of the remap (stable ranks inside each chunk) runs on the side
+  // stream concurrently with histogram + plan
+  UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
+  UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+  rc = launch_rank(c, topk_ids, ws, c->side);
+  UEP_CUDA_TRY(cudaEventRecord(c->ev_rank, c->side));
+  int rc2 = uep_histogram(ctx, topk_ids, expert_count, ws, stream);
+  if (rc2 == UEP_OK) rc2 = uep_plan(ctx, expert_count, plan, ws, stream);
   const bool do_pack = n_tensors > 0 && c->cfg.n_slot > 0;
-  if (do_pack) {   // fork: pack depends only on the plan and overlaps the remap (Eq. 1)
+  if (do_pack && rc2 == UEP_OK) {   // pack depends only on the plan and overlaps the lookup (Eq. 1)
     UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
     UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+    int rc3 = launch_pack(c, *plan, a, c->side);
+    if (rc == UEP_OK) rc = rc3;
   }
-  rc = uep_remap(ctx, topk_ids, gate, plan, out_replica, out_rank, out_offset, out_gate, ws, stream);
-  if (do_pack) {
-    int rc2 = launch_pack(c, *plan, a, c->side);
-    UEP_CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
-    UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_join, 0));
-    if (rc == UEP_OK) rc = rc2;
-  }
-  return rc;
+  UEP_CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
+  UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_rank, 0));          // join the rank kernel
+  if (rc == UEP_OK && rc2 == UEP_OK)
+    rc2 = launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s);
+  UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_join, 0));          // join the side stream (pack)
+  return rc != UEP_OK ? rc : rc2;
 }
 
 int uep_balance_host(const uep_ctx* ctx, const int32_t* topk_ids_host, const void* gate_host,

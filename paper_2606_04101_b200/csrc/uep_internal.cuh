@@ -23,6 +23,8 @@ constexpr int kPlanLevels = 5;           // bisection levels speculated per roun
 constexpr int kPackTile = 16 * 1024;     // bytes per bulk-copy tile
 constexpr int kPackStages = 8;           // shared-memory ring depth
 constexpr int kMinChunk = 2048;          // smallest histogram/remap chunk (slots per CTA)
+constexpr int kMaxChunk = kRemapRound;   // largest: one register-resident round per CTA
+constexpr int kPackedEBits = 9;          // packed slot word: expert id | (rank inside chunk << 9); -1 invalid
 
 struct Ctx {
   uep_config cfg;
@@ -39,7 +41,7 @@ struct Ctx {
   int32_t* d_rexp;        // [E]   experts grouped by home rank, ascending e
   // fork/join for uep_balance
   cudaStream_t side;
-  cudaEvent_t ev_fork, ev_join;
+  cudaEvent_t ev_fork, ev_join, ev_rank;
 };
 
 struct PackArgs {
@@ -53,6 +55,11 @@ int set_cuda_error(cudaError_t e);
 
 int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s);
 int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s);
+// uep_remap = launch_rank (plan-independent: stable rank of every slot inside its chunk, packed
+// with the expert id into the workspace) + launch_lookup (plan-dependent: cumulative-quota lookup).
+int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s);
+int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& plan, int32_t* out_replica,
+                  int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s);
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& plan,
                  int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
                  void* ws, cudaStream_t s);
@@ -99,6 +106,12 @@ inline int32_t* ws_table(void* ws) {
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes);
 }
 inline unsigned* ws_ticket(void* ws) { return reinterpret_cast<unsigned*>(ws); }
+inline size_t ws_table_bytes(const Ctx* c) {
+  return (sizeof(int32_t) * (size_t)c->n_chunks * c->E_pad + 255) & ~(size_t)255;
+}
+inline int32_t* ws_packed(const Ctx* c, void* ws) {      // [S] packed (expert, rank in chunk)
+  return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c));
+}
 
 }  // namespace uep
 
