@@ -189,6 +189,13 @@ class Rig:
         self.ctx.uep_remap(self.ids[i], self.gates[i], self.plans[i], o[0], o[1], o[2], o[3],
                            self.ws[i])
 
+    def rank(self, i):
+        self.ctx.uep_remap_rank(self.ids[i], self.ws[i])
+
+    def lookup(self, i):
+        o = self.outs[i]
+        self.ctx.uep_remap_lookup(self.gates[i], self.plans[i], o[0], o[1], o[2], o[3], self.ws[i])
+
     def pack(self, i):
         self.ctx.uep_pack(self.plans[i], self.src, self.dst)
 
@@ -291,7 +298,11 @@ def run_uep(args):
 
     # ---- stage timing: graph-captured chains over all instances (L2-cold by rotation) --------
     reps = 5
-    chain = capture([lambda i=i: (rig.hist(i), rig.plan(i), rig.remap(i)) for i in range(n_inst)], stream)
+    # the chain is uep_balance without state tensors: histogram -> plan -> lookup on the stream,
+    # the rank half of the remap forked beside histogram + plan (as the library schedules it)
+    chain = capture([lambda i=i: rig.balance(i, with_pack=False) for i in range(n_inst)], stream)
+    g_rank = capture([lambda i=i: rig.rank(i) for i in range(n_inst)], stream)
+    g_lookup = capture([lambda i=i: rig.lookup(i) for i in range(n_inst)], stream)
     g_hist = capture([lambda i=i: rig.hist(i) for i in range(n_inst)], stream)
     g_plan = capture([lambda i=i: rig.plan(i) for i in range(n_inst)], stream)
     g_remap = capture([lambda i=i: rig.remap(i) for i in range(n_inst)], stream)
@@ -299,6 +310,8 @@ def run_uep(args):
     hist_ms, _ = time_graph(g_hist, stream, reps)
     plan_ms, _ = time_graph(g_plan, stream, reps)
     remap_ms, _ = time_graph(g_remap, stream, reps)
+    rank_ms, _ = time_graph(g_rank, stream, reps)
+    lookup_ms, _ = time_graph(g_lookup, stream, reps)
     n_pack = min(n_inst, 8)
     g_pack = capture([lambda i=i: rig.pack(i) for i in range(n_pack)], stream)
     pack_ms, _ = time_graph(g_pack, stream, 3, warm=1)
@@ -331,7 +344,12 @@ def run_uep(args):
 
     pack_us = us(pack_ms, n_pack)
     r_pack = roof("pack_kernel", sum(bytes_pack) / n_pack, pack_us)
-    rooflines = [r_pack, roof("remap_kernel", bytes_remap, us(remap_ms, n_inst)),
+    # remap = rank_kernel + lookup_kernel: 24 B/slot algorithmic (fp32 gates) over both; each half
+    # also against its own traffic (rank: 4 B id in + 4 B packed out; lookup: 4 B packed + g in,
+    # 12 B + g out)
+    rooflines = [r_pack, roof("rank_kernel+lookup_kernel (uep_remap)", bytes_remap, us(remap_ms, n_inst)),
+                 roof("lookup_kernel", bytes_remap, us(lookup_ms, n_inst)),
+                 roof("rank_kernel", 8 * S, us(rank_ms, n_inst)),
                  roof("hist_kernel", bytes_hist, us(hist_ms, n_inst))]
     result = {
         "metric": METRIC, "value": round(plan_latency_us, 3), "unit": UNIT, "n_gpus": world,
@@ -346,7 +364,9 @@ def run_uep(args):
                    "parallelism": "instances sharded over ranks, no collective",
                    "state_scale": args.state_scale},
         "stages_us": {"histogram": round(us(hist_ms, n_inst), 2), "plan": round(us(plan_ms, n_inst), 2),
-                      "remap": round(us(remap_ms, n_inst), 2), "pack": round(pack_us, 2),
+                      "remap": round(us(remap_ms, n_inst), 2),
+                      "remap_rank": round(us(rank_ms, n_inst), 2),
+                      "remap_lookup": round(us(lookup_ms, n_inst), 2), "pack": round(pack_us, 2),
                       "hist_plan_remap_chain": round(plan_latency_us, 2),
                       "hist_plan_remap_chain_min": round(chain_min * 1e3 / n_inst, 2),
                       "whole_step": round(step_ms * 1e3 / K, 2)},
@@ -357,7 +377,7 @@ def run_uep(args):
                     "n_probes_mean": round(statistics.mean(int(s[binding.SC_N_PROBES]) for s in sc), 1)},
         "roofline": {k: r_pack[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")},
         "rooflines": rooflines,
-        "gpu_launches": 4 * K,
+        "gpu_launches": 5 * K,
         "clocks": clocks,
         "launch_info": rig.ctx.launch_info,
     }

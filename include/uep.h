@@ -155,6 +155,18 @@ int uep_remap(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
               const uep_plan_out* plan, int32_t* out_replica, int32_t* out_rank,
               int32_t* out_offset, void* out_gate, void* ws, void* stream);
 
+/* The two halves of uep_remap, for callers that overlap them with other work (uep_balance does):
+ *   uep_remap_rank    plan-INDEPENDENT: stable rank of every slot among the slots of its expert
+ *                     inside its chunk, written to the workspace.  Needs only topk_ids; may run
+ *                     concurrently with uep_histogram / uep_plan on another stream.
+ *   uep_remap_lookup  plan-DEPENDENT: needs ws after BOTH uep_histogram and uep_remap_rank on the
+ *                     same topk_ids, and the plan.  Same outputs and argument rules as uep_remap.
+ * uep_remap(...) == uep_remap_rank(...) then uep_remap_lookup(...) on one stream. */
+int uep_remap_rank(const uep_ctx* ctx, const int32_t* topk_ids, void* ws, void* stream);
+int uep_remap_lookup(const uep_ctx* ctx, const void* gate, const uep_plan_out* plan,
+                     int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
+                     void* ws, void* stream);
+
 /* Pack the state of every replicated expert into its destination slot:
  *   dst[j][(t*n_slot+s)*B_j .. +B_j) = src[j][e*B_j .. +B_j)  for x_{t,s} = e != empty.
  * Empty slots are not touched.  src/dst/bytes_per_expert: HOST arrays [n_tensors] of DEVICE
@@ -163,9 +175,11 @@ int uep_pack(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,
              const void* const* src, const size_t* bytes_per_expert, void* const* dst,
              void* stream);
 
-/* histogram -> plan -> remap and pack, chained on `stream` (pack runs on an internal side
- * stream forked/joined with events, so that it overlaps the remap as in Eq. 1,
- * max(T_reroute, T_w_distr)).  Capturable.  n_tensors may be 0. */
+/* histogram -> plan -> remap and pack, chained on `stream`.  Internally forked/joined with
+ * events on a side stream: uep_remap_rank runs beside histogram + plan (it does not depend on
+ * them), and pack runs beside uep_remap_lookup, overlapping the reroute with the weight
+ * distribution as in Eq. 1, max(T_reroute, T_w_distr).  Capturable.
+ * n_tensors may be 0. */
 int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
                 int32_t* expert_count, const uep_plan_out* plan, int32_t* out_replica,
                 int32_t* out_rank, int32_t* out_offset, void* out_gate, int32_t n_tensors,

@@ -16,6 +16,7 @@
 //   * the accept log is written only by one final probe at the final tau (deterministic, so it
 //     reproduces U~ of the last feasible probe, S10), then all 1024 threads emit X, the CSR
 //     cumulative quotas and the receive layout.
+#include <algorithm>
 #include "uep_internal.cuh"
 
 namespace uep {
@@ -37,11 +38,16 @@ struct PlanSmem {
   int order[UEP_MAX_R];        // ranks by l_r desc, id asc
   int roff[UEP_MAX_R + 1];
   int rload[UEP_MAX_R];
-  int log_e[kMaxLog], log_t[kMaxLog], log_slot[kMaxLog], log_d[kMaxLog], dscan[kMaxLog];
+  int s_ell[UEP_MAX_R];        // l_r in visit order
+  int v_off[UEP_MAX_R + 1];    // CSR of the flat visit list: experts of the oi-th visited rank
+  int v_lam[UEP_MAX_E];        // lambda_e in visit order
+  int v_e[UEP_MAX_E];          // expert ids in visit order
+  int dscan[kMaxLog];
+  int log_n[32];               // accepted transfers of the probe each warp logged
   int pc[kPcSmem];
   int warp_tmp[32];
   int feas[32];
-  int lo, hi, n_probes, n_log;
+  int lo, hi, n_probes, n_log, log_buf;
   long long s_valid;
   int max_ell;
 };
@@ -73,11 +79,15 @@ __device__ __forceinline__ int block_incl_scan(int v, int* tmp) {
 }
 
 // One greedy feasibility probe (Alg. 1 lines 6-20) by one warp.  All control flow is
-// warp-uniform.  LOG: also record the accepted transfers.
+// warp-uniform.  A single warp issues one dependent instruction every ~4 cycles, so the probe is
+// written for the fewest instructions on that chain: ranks and experts stream from the flat
+// visit list (s_ell / v_off / v_lam, sorted once per solve), the owner of the arg-max is the lane
+// whose key equals the reduced key (keys are unique: they carry the rank id), and its new key is
+// the old one minus delta << 8.  LOG: also record the accepted transfers {e, t, slot, delta}.
 template <int RPL, bool LOG>
-__device__ __forceinline__ bool probe(PlanSmem& sm, const int tau, const int R, const int n_slot,
-                                      const int u_min, const bool strict, const int lane,
-                                      int& n_log) {
+__device__ __forceinline__ bool probe(const PlanSmem& sm, const int tau, const int R,
+                                      const int n_slot, const int u_min, const bool strict,
+                                      const int lane, int4* __restrict__ log, int& n_log) {
   unsigned key[RPL];
   int used[RPL];
 #pragma unroll
@@ -87,55 +97,52 @@ __device__ __forceinline__ bool probe(PlanSmem& sm, const int tau, const int R, 
     used[i] = 0;
     key[i] = (slk > 0 && n_slot > 0) ? (((unsigned)slk << 8) | (unsigned)(255 - t)) : 0u;
   }
+  const int brk = strict ? 1 : u_min;        // a rank is drained when exc < brk (S8)
   int nl = 0;
-  bool ok = true;
-  bool dead = false;       // no rank can absorb u_min any more: slack only shrinks, so it stays so
   for (int oi = 0; oi < R; ++oi) {                                  // line 8
-    const int r = sm.order[oi];
-    int exc = sm.ell[r] - tau;
-    if (exc <= 0) break;                       // ranks are sorted: nobody further is overloaded
-    const int a = sm.roff[r], b = sm.roff[r + 1];
-    for (int ei = a; ei < b && exc >= u_min && !dead; ++ei) {       // line 9
-      const int e = sm.elist[ei];
-      int cap = sm.lam[e];                                          // line 10 (S6)
+    int exc = sm.s_ell[oi] - tau;
+    if (exc < brk) break;                      // ranks are sorted: every later rank is drained too
+    const int a = sm.v_off[oi], b = sm.v_off[oi + 1];
+    bool dead = false;     // no rank can absorb u_min any more: slack only shrinks, so it stays so
+    for (int ei = a; ei < b && exc >= u_min; ++ei) {                // line 9
+      int cap = sm.v_lam[ei];                                       // line 10 (S6)
       if (cap < u_min) break;                  // sorted by lambda: no later expert can pass line 16
-      while (true) {                                                // line 11
+      do {                                                          // line 11
         unsigned kl = key[0];
 #pragma unroll
         for (int i = 1; i < RPL; ++i) kl = max(kl, key[i]);
         const unsigned km = __reduce_max_sync(kFull, kl);           // lines 12-14
         const int s = (int)(km >> 8);
-        if (s < u_min) { dead = true; break; }                      // line 13 (T empty) or line 16
         const int d = min(exc, min(s, cap));                        // line 15
-        if (d < u_min) break;                                       // line 16
-        const int t = 255 - (int)(km & 255u);
+        if (d < u_min) { dead = s < u_min; break; }                 // line 16 (or line 13: T empty)
         int slot = 0;
 #pragma unroll
         for (int i = 0; i < RPL; ++i) {
-          if (t == lane + 32 * i) {                                 // owner lane: lines 17-19
+          if (key[i] == km) {                                       // owner lane: lines 17-19
             slot = used[i];
             used[i] += 1;
-            const int ns = s - d;
-            key[i] = (ns > 0 && used[i] < n_slot) ? (((unsigned)ns << 8) | (unsigned)(255 - t)) : 0u;
+            key[i] = (s > d && used[i] < n_slot) ? km - ((unsigned)d << 8) : 0u;
           }
         }
         if (LOG) {
-          if (lane == (t & 31)) {
-            sm.log_e[nl] = e; sm.log_t[nl] = t; sm.log_slot[nl] = slot; sm.log_d[nl] = d;
-          }
+          const int t = 255 - (int)(km & 255u);
+          if (lane == (t & 31)) log[nl] = make_int4(sm.v_e[ei], t, slot, d);
         }
         ++nl;
         exc -= d;
         cap -= d;
-        if (exc == 0 || cap == 0) break;
-      }
+      } while (exc > 0 && cap > 0);
+      if (dead) break;
     }
     // line 20 per rank (S21 early exit): strict needs exc == 0, tolerant exc < u_min (S8)
-    if (strict ? (exc > 0) : (exc >= u_min)) { ok = false; break; }
-    if (!strict && sm.ell[r] - tau < u_min) break;   // tolerant: every later rank passes too
+    if (exc >= brk) { n_log = nl; return false; }
+    if (dead) {            // nothing can be moved any more: feasible iff no later rank needs to
+      n_log = nl;
+      return (oi + 1 >= R) || (sm.s_ell[oi + 1] - tau < brk);
+    }
   }
   n_log = nl;
-  return ok;
+  return true;
 }
 
 template <int RPL>
@@ -143,11 +150,18 @@ __global__ void __launch_bounds__(kPlanThreads, 1)
 plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict__ g_home,
             const int32_t* __restrict__ g_main_phys, const int32_t* __restrict__ g_roff,
             const int32_t* __restrict__ g_rexp, uep_plan_out out, int E, int R, int n_slot, int M,
-            int P, int u_min, int beta_num, int beta_den, int strict_i, int S_total) {
+            int P, int u_min, int beta_num, int beta_den, int strict_i, int S_total, int n_bufs,
+            int log_cap) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   PlanSmem& sm = *reinterpret_cast<PlanSmem*>(smem_raw);
+  // accept logs: n_bufs buffers of log_cap entries {e, t, slot, delta}; with 32 buffers every
+  // warp of the LAST speculation round logs its probe, so the plan needs no extra probe
+  int4* logs = reinterpret_cast<int4*>(smem_raw + ((sizeof(PlanSmem) + 15) & ~(size_t)15));
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool strict = strict_i != 0;
+#ifdef UEP_PLAN_TIMING
+  long long t_start = clock64(), t_setup = 0, t_bisect = 0, t_final = 0;
+#endif
 
   // ---- stage inputs ---------------------------------------------------------------------
   if (tid < E) {
@@ -214,7 +228,29 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   __syncthreads();
   if (tid < E) sm.elist[sm.u_main[tid]] = tid;
   __syncthreads();
+  // flat visit list: ranks in visit order, each with its experts in visit order (S5)
+  {
+    const int r = (tid < R) ? sm.order[tid] : 0;
+    const int cnt = (tid < R) ? (sm.roff[r + 1] - sm.roff[r]) : 0;
+    const int inc = block_incl_scan(cnt, sm.warp_tmp);
+    if (tid < R) {
+      sm.s_ell[tid] = sm.ell[r];
+      sm.v_off[tid] = inc - cnt;
+      if (tid == R - 1) sm.v_off[R] = inc;
+      const int src = sm.roff[r];
+      for (int q = 0; q < cnt; ++q) {
+        const int e = sm.elist[src + q];
+        sm.v_e[inc - cnt + q] = e;
+        sm.v_lam[inc - cnt + q] = sm.lam[e];
+      }
+    }
+    if (tid == 0) sm.log_buf = -1;
+  }
+  __syncthreads();
   const int tau_lo0 = sm.lo, tau_hi0 = sm.hi;
+#ifdef UEP_PLAN_TIMING
+  t_setup = clock64();
+#endif
 
   // ---- bisection, kPlanLevels levels per round (S9) ---------------------------------------
   while (true) {
@@ -232,32 +268,49 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       }
       if (l >= h) valid = false;
       if (valid) {
-        int nl;
-        const bool f = probe<RPL, false>(sm, (l + h) >> 1, R, n_slot, u_min, strict, lane, nl);
-        if (lane == 0) sm.feas[node] = f ? 1 : 0;
+        int nl = 0;
+        bool f;
+        if (n_bufs > 1 && hi - lo < (1 << kPlanLevels)) {           // last round: log every probe
+          f = probe<RPL, true>(sm, (l + h) >> 1, R, n_slot, u_min, strict, lane,
+                               logs + (size_t)warp * log_cap, nl);
+        } else {
+          f = probe<RPL, false>(sm, (l + h) >> 1, R, n_slot, u_min, strict, lane, nullptr, nl);
+        }
+        if (lane == 0) { sm.feas[node] = f ? 1 : 0; sm.log_n[node] = nl; }
       }
     }
     __syncthreads();
     if (tid == 0) {
-      int node = 1, l = lo, h = hi, np = sm.n_probes;
+      int node = 1, l = lo, h = hi, np = sm.n_probes, last_feas = -1;
       while (node < (1 << kPlanLevels) && l < h) {
         const int mid = (l + h) >> 1;                               // line 5
         ++np;
-        if (sm.feas[node]) { h = mid; node = 2 * node; }            // lines 21-22
+        if (sm.feas[node]) { h = mid; last_feas = node; node = 2 * node; }   // lines 21-22
         else { l = mid + 1; node = 2 * node + 1; }                  // line 24
       }
       sm.lo = l; sm.hi = h; sm.n_probes = np;
+      // the probe at the final tau (= last feasible one) was logged iff this was a logging round
+      if (n_bufs > 1 && hi - lo < (1 << kPlanLevels) && last_feas > 0) {
+        sm.log_buf = last_feas; sm.n_log = sm.log_n[last_feas];
+      }
     }
     __syncthreads();
   }
   const int tau = sm.hi;
+#ifdef UEP_PLAN_TIMING
+  t_bisect = clock64();
+#endif
 
   // ---- materialise: one logged probe at the final tau (S10) -------------------------------
-  if (warp == 0 && sm.n_probes > 0) {
+  // (only when the last round did not log it: the final tau was found in an earlier round, or
+  // the log buffers of 31 concurrent probes do not fit in shared memory)
+  const int log_buf = sm.log_buf;
+  if (warp == 0 && sm.n_probes > 0 && log_buf < 0) {
     int nl;
-    probe<RPL, true>(sm, tau, R, n_slot, u_min, strict, lane, nl);
+    probe<RPL, true>(sm, tau, R, n_slot, u_min, strict, lane, logs, nl);
     if (lane == 0) sm.n_log = nl;
   }
+  const int4* lg = logs + (size_t)(log_buf < 0 ? 0 : log_buf) * log_cap;
   if (tid < E) { sm.u_main[tid] = sm.lam[tid]; sm.n_rep[tid] = 0; sm.first[tid] = 0x7fffffff; }
   const int RP = R * P;
   const bool pc_in_smem = RP <= kPcSmem;
@@ -267,11 +320,14 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   if (out.U) for (int i = tid; i < E * R; i += kPlanThreads) out.U[i] = 0;
   __syncthreads();
   const int n_log = sm.n_log;
+#ifdef UEP_PLAN_TIMING
+  t_final = clock64();
+#endif
 
   // ---- emit (line 22 "materialize U~ into X" + cumulative reroute metadata, §5.2) ---------
   if (tid < n_log) {
-    const int e = sm.log_e[tid];
-    atomicSub(&sm.u_main[e], sm.log_d[tid]);
+    const int e = lg[tid].x;
+    atomicSub(&sm.u_main[e], lg[tid].w);
     atomicAdd(&sm.n_rep[e], 1);
     atomicMin(&sm.first[e], tid);
   }
@@ -282,7 +338,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (tid < E) sm.inst_off[tid] = inc - v;
     if (tid == E - 1) sm.inst_off[E] = inc;
     __syncthreads();
-    const int d = (tid < n_log) ? sm.log_d[tid] : 0;
+    const int d = (tid < n_log) ? lg[tid].w : 0;
     const int ds = block_incl_scan(d, sm.warp_tmp);
     if (tid < n_log) sm.dscan[tid] = ds;
   }
@@ -299,7 +355,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     fan = 1 + sm.n_rep[tid];
   }
   if (tid < n_log) {
-    const int e = sm.log_e[tid], t = sm.log_t[tid], sl = sm.log_slot[tid], d = sm.log_d[tid];
+    const int e = lg[tid].x, t = lg[tid].y, sl = lg[tid].z, d = lg[tid].w;
     const int f = sm.first[e];
     const int pos = sm.inst_off[e] + 1 + (tid - f);                 // S11: acceptance order
     const int before = (f > 0) ? sm.dscan[f - 1] : 0;
@@ -337,8 +393,8 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     const int* pb = pc_in_smem ? pc : out.phys_base;      // bases (global ones are CTA-visible now)
     if (tid < E) out.inst_base[sm.inst_off[tid]] = pb[sm.home[tid] * P + sm.main_phys[tid]];
     if (tid < n_log) {
-      const int e = sm.log_e[tid];
-      out.inst_base[sm.inst_off[e] + 1 + (tid - sm.first[e])] = pb[sm.log_t[tid] * P + M + sm.log_slot[tid]];
+      const int e = lg[tid].x;
+      out.inst_base[sm.inst_off[e] + 1 + (tid - sm.first[e])] = pb[lg[tid].y * P + M + lg[tid].z];
     }
   }
   int max_fan = 0, n_groups = 0;
@@ -366,16 +422,28 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     out.scalars[UEP_SC_TAU_HI0] = tau_hi0;
     out.scalars[UEP_SC_N_GROUPS] = n_groups;
     for (int i = UEP_SC_N_GROUPS + 1; i < UEP_N_SCALARS; ++i) out.scalars[i] = 0;
+#ifdef UEP_PLAN_TIMING   // developer probe: cycles of setup / bisection / final probe / emit
+    out.scalars[12] = (int)(t_setup - t_start);
+    out.scalars[13] = (int)(t_bisect - t_setup);
+    out.scalars[14] = (int)(t_final - t_bisect);
+    out.scalars[15] = (int)(clock64() - t_final);
+#endif
   }
 }
+
+constexpr size_t kLogBudget = 128 * 1024;     // shared memory for the accept logs of one round
 
 template <int RPL>
 static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out& plan,
                          cudaStream_t s) {
   const uep_config& g = c->cfg;
-  plan_kernel<RPL><<<1, kPlanThreads, sizeof(PlanSmem), s>>>(
+  const int log_cap = std::max(1, g.R * g.n_slot);
+  const int n_bufs = (32 * (size_t)log_cap * sizeof(int4) <= kLogBudget) ? 32 : 1;
+  const size_t smem = ((sizeof(PlanSmem) + 15) & ~(size_t)15) + (size_t)n_bufs * log_cap * sizeof(int4);
+  plan_kernel<RPL><<<1, kPlanThreads, smem, s>>>(
       count, c->d_home, c->d_main_phys, c->d_roff, c->d_rexp, plan, g.E, g.R, g.n_slot, c->M, c->P,
-      g.u_min, g.beta_num, g.beta_den, g.floor_mode == UEP_FLOOR_STRICT ? 1 : 0, c->S);
+      g.u_min, g.beta_num, g.beta_den, g.floor_mode == UEP_FLOOR_STRICT ? 1 : 0, c->S, n_bufs,
+      log_cap);
   UEP_CUDA_TRY(cudaGetLastError());
   return UEP_OK;
 }
@@ -389,7 +457,7 @@ int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cu
 }
 
 int init_plan_kernels() {
-  const int bytes = (int)sizeof(PlanSmem);
+  const int bytes = (int)(sizeof(PlanSmem) + 16 + kLogBudget);
   UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));

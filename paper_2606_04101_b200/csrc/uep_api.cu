@@ -240,6 +240,41 @@ int uep_remap(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
                       static_cast<cudaStream_t>(stream));
 }
 
+static int check_remap_outputs(const Ctx* c, const void* gate, const uep_plan_out* plan,
+                               const int32_t* out_replica, const int32_t* out_rank,
+                               const int32_t* out_offset, const void* out_gate, const void* ws) {
+  if (!ws || !aligned16(ws)) return UEP_ERR_INVALID_ARG;
+  int rc = check_plan_ptrs(c, plan);
+  if (rc != UEP_OK) return rc;
+  if (c->S > 0) {
+    if (!out_replica || !out_rank || !out_offset) return UEP_ERR_INVALID_ARG;
+    if (!aligned16(out_replica) || !aligned16(out_rank) || !aligned16(out_offset))
+      return UEP_ERR_INVALID_ARG;
+  }
+  if ((gate == nullptr) != (out_gate == nullptr)) return UEP_ERR_INVALID_ARG;
+  if (gate && (c->cfg.gate_dtype == UEP_GATE_NONE || !aligned16(gate) || !aligned16(out_gate)))
+    return UEP_ERR_INVALID_ARG;
+  return UEP_OK;
+}
+
+int uep_remap_rank(const uep_ctx* ctx, const int32_t* topk_ids, void* ws, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !ws || !aligned16(ws)) return UEP_ERR_INVALID_ARG;
+  if (c->S > 0 && (!topk_ids || !aligned16(topk_ids))) return UEP_ERR_INVALID_ARG;
+  return launch_rank(c, topk_ids, ws, static_cast<cudaStream_t>(stream));
+}
+
+int uep_remap_lookup(const uep_ctx* ctx, const void* gate, const uep_plan_out* plan,
+                     int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
+                     void* ws, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c) return UEP_ERR_INVALID_ARG;
+  int rc = check_remap_outputs(c, gate, plan, out_replica, out_rank, out_offset, out_gate, ws);
+  if (rc != UEP_OK) return rc;
+  return launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws,
+                       static_cast<cudaStream_t>(stream));
+}
+
 int uep_pack(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,
              const void* const* src, const size_t* bytes_per_expert, void* const* dst,
              void* stream) {
