@@ -17,12 +17,22 @@
 //     reproduces U~ of the last feasible probe, S10), then all 1024 threads emit X, the CSR
 //     cumulative quotas and the receive layout.
 #include <algorithm>
+#include <cstdlib>
+#include <cooperative_groups.h>
 #include "uep_internal.cuh"
 
 namespace uep {
 
+namespace cg = cooperative_groups;
+
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kMaxLog = UEP_MAX_R * UEP_MAX_NSLOT;      // 1024 accepted transfers at most
+// CTAs (SMs) sharing one solve, so that the 63 probes of a round spread over many schedulers:
+// 8 CTAs = two probes per scheduler.  Measured on B200 (DSV3 shape): 4 / 8 / 16 CTAs give
+// 22.9 / 20.6 / 20.4 us of bisection, i.e. from 8 up the probes are bound by the latency of their
+// own dependent chain, not by issue slots, so the portable size 8 is the default
+// (UEP_PLAN_CLUSTER overrides; 16 needs the non-portable opt-in, set in init_plan_kernels).
+constexpr int kPlanMaxNodes = 64;     // 2^6: six bisection levels speculated per round with 8 CTAs
 constexpr int kPcSmem = 2048;                           // phys_count staged in smem if R*P fits
 
 struct PlanSmem {
@@ -43,7 +53,8 @@ struct PlanSmem {
   int v_lam[UEP_MAX_E];        // lambda_e in visit order
   int v_e[UEP_MAX_E];          // expert ids in visit order
   int dscan[kMaxLog];
-  int log_n[32];               // accepted transfers of the probe each warp logged
+  int log_n[2][kPlanMaxNodes]; // accepted transfers of the probe at each tree node (per round parity)
+  int node_feas[2][kPlanMaxNodes];   // probe verdict per tree node, written by its owner to every CTA
   int pc[kPcSmem];
   int warp_tmp[32];
   int feas[32];
@@ -151,11 +162,14 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
             const int32_t* __restrict__ g_main_phys, const int32_t* __restrict__ g_roff,
             const int32_t* __restrict__ g_rexp, uep_plan_out out, int E, int R, int n_slot, int M,
             int P, int u_min, int beta_num, int beta_den, int strict_i, int S_total, int n_bufs,
-            int log_cap) {
+            int log_cap, int levels) {
+  cg::cluster_group cluster = cg::this_cluster();
+  const int csize = (int)cluster.num_blocks(), crank = (int)cluster.block_rank();
   extern __shared__ __align__(16) unsigned char smem_raw[];
   PlanSmem& sm = *reinterpret_cast<PlanSmem*>(smem_raw);
-  // accept logs: n_bufs buffers of log_cap entries {e, t, slot, delta}; with 32 buffers every
-  // warp of the LAST speculation round logs its probe, so the plan needs no extra probe
+  // accept logs: n_bufs buffers of log_cap entries {e, t, slot, delta}; buffer 0 serves the
+  // fallback probe, buffer 1+w the probe of warp w in the LAST speculation round (every probe of
+  // that round is logged, so the plan normally needs no extra probe)
   int4* logs = reinterpret_cast<int4*>(smem_raw + ((sizeof(PlanSmem) + 15) & ~(size_t)15));
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool strict = strict_i != 0;
@@ -201,31 +215,40 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     sm.n_probes = 0;
     sm.n_log = 0;
   }
-  // rank order: position = number of ranks that come before (l desc, id asc). warp per rank.
-  for (int r = warp; r < R; r += 32) {
-    const int lr = sm.ell[r];
-    int cnt = 0;
-    for (int q = lane; q < R; q += 32) {
-      const int lq = sm.ell[q];
-      cnt += (lq > lr || (lq == lr && q < r)) ? 1 : 0;
+#ifdef UEP_PLAN_TIMING
+  const long long t_s1 = clock64();
+#endif
+  // rank order: position = number of ranks that come before (l desc, id asc); a warp per rank,
+  // by the upper half of the CTA, while the lower half orders the experts
+  if (warp >= 16) {
+    for (int r = warp - 16; r < R; r += 16) {
+      const int lr = sm.ell[r];
+      int cnt = 0;
+      for (int q = lane; q < R; q += 32) {
+        const int lq = sm.ell[q];
+        cnt += (lq > lr || (lq == lr && q < r)) ? 1 : 0;
+      }
+      cnt = __reduce_add_sync(kFull, cnt);
+      if (lane == 0) sm.order[cnt] = r;
     }
-    cnt = __reduce_add_sync(kFull, cnt);
-    if (lane == 0) sm.order[cnt] = r;
-  }
-  // per-rank expert order: lambda desc, id asc. warp per expert; positions into u_main (temp).
-  for (int e = warp; e < E; e += 32) {
-    const int h = sm.home[e], le = sm.lam[e];
+  } else if (tid < E) {
+    // per-rank expert order: lambda desc, id asc; a thread per expert counts the experts of its
+    // home rank that come before it; positions into u_main (temp)
+    const int e = tid, h = sm.home[e], le = sm.lam[e];
     const int a = sm.roff[h], b = sm.roff[h + 1];
     int cnt = 0;
-    for (int i = a + lane; i < b; i += 32) {
+#pragma unroll 4
+    for (int i = a; i < b; ++i) {
       const int q = sm.elist[i];
       const int lq = sm.lam[q];
       cnt += (lq > le || (lq == le && q < e)) ? 1 : 0;
     }
-    cnt = __reduce_add_sync(kFull, cnt);
-    if (lane == 0) sm.u_main[e] = a + cnt;
+    sm.u_main[e] = a + cnt;
   }
   __syncthreads();
+#ifdef UEP_PLAN_TIMING
+  const long long t_s2 = clock64();
+#endif
   if (tid < E) sm.elist[sm.u_main[tid]] = tid;
   __syncthreads();
   // flat visit list: ranks in visit order, each with its experts in visit order (S5)
@@ -252,12 +275,21 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   t_setup = clock64();
 #endif
 
-  // ---- bisection, kPlanLevels levels per round (S9) ---------------------------------------
+  // ---- bisection, `levels` levels per round (S9) ---------------------------------------------
+  // Tree node n (heap index, 1 .. 2^levels - 1) is probed by warp n / csize of CTA n % csize:
+  // with 8 CTAs and 6 levels that is <= 2 probes per scheduler, so every probe runs at the
+  // latency of its own dependent chain instead of queueing for issue slots on one SM.  The
+  // verdicts are written into EVERY CTA's shared memory (DSMEM), one cluster barrier per round,
+  // and every CTA walks the path redundantly (identical state everywhere, no broadcast back).
+  const int n_nodes = 1 << levels;
+  int round = 0;
   while (true) {
     const int lo = sm.lo, hi = sm.hi;
     if (lo >= hi) break;                                            // line 4
-    if (warp >= 1) {
-      const int node = warp;                                        // heap index 1..31
+    const int buf = round & 1;
+    const bool log_round = n_bufs > 1 && hi - lo < n_nodes;         // last round: log every probe
+    const int node = warp * csize + crank;
+    if (node >= 1 && node < n_nodes) {
       const int depth = 31 - __clz(node);
       int l = lo, h = hi;
       bool valid = true;
@@ -270,47 +302,53 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       if (valid) {
         int nl = 0;
         bool f;
-        if (n_bufs > 1 && hi - lo < (1 << kPlanLevels)) {           // last round: log every probe
+        if (log_round) {
           f = probe<RPL, true>(sm, (l + h) >> 1, R, n_slot, u_min, strict, lane,
-                               logs + (size_t)warp * log_cap, nl);
+                               logs + (size_t)(1 + warp) * log_cap, nl);
         } else {
           f = probe<RPL, false>(sm, (l + h) >> 1, R, n_slot, u_min, strict, lane, nullptr, nl);
         }
-        if (lane == 0) { sm.feas[node] = f ? 1 : 0; sm.log_n[node] = nl; }
+        if (lane < csize) {
+          *cluster.map_shared_rank(&sm.node_feas[buf][node], lane) = f ? 1 : 0;
+          *cluster.map_shared_rank(&sm.log_n[buf][node], lane) = nl;
+        }
       }
     }
-    __syncthreads();
+    if (csize > 1) cluster.sync(); else __syncthreads();
     if (tid == 0) {
-      int node = 1, l = lo, h = hi, np = sm.n_probes, last_feas = -1;
-      while (node < (1 << kPlanLevels) && l < h) {
+      int nd = 1, l = lo, h = hi, np = sm.n_probes, last_feas = -1;
+      while (nd < n_nodes && l < h) {
         const int mid = (l + h) >> 1;                               // line 5
         ++np;
-        if (sm.feas[node]) { h = mid; last_feas = node; node = 2 * node; }   // lines 21-22
-        else { l = mid + 1; node = 2 * node + 1; }                  // line 24
+        if (sm.node_feas[buf][nd]) { h = mid; last_feas = nd; nd = 2 * nd; }   // lines 21-22
+        else { l = mid + 1; nd = 2 * nd + 1; }                      // line 24
       }
       sm.lo = l; sm.hi = h; sm.n_probes = np;
       // the probe at the final tau (= last feasible one) was logged iff this was a logging round
-      if (n_bufs > 1 && hi - lo < (1 << kPlanLevels) && last_feas > 0) {
-        sm.log_buf = last_feas; sm.n_log = sm.log_n[last_feas];
-      }
+      if (log_round && last_feas > 0) { sm.log_buf = last_feas; sm.n_log = sm.log_n[buf][last_feas]; }
     }
     __syncthreads();
+    ++round;
   }
   const int tau = sm.hi;
 #ifdef UEP_PLAN_TIMING
   t_bisect = clock64();
 #endif
 
-  // ---- materialise: one logged probe at the final tau (S10) -------------------------------
-  // (only when the last round did not log it: the final tau was found in an earlier round, or
-  // the log buffers of 31 concurrent probes do not fit in shared memory)
-  const int log_buf = sm.log_buf;
-  if (warp == 0 && sm.n_probes > 0 && log_buf < 0) {
+  // ---- materialise (S10).  The CTA holding the log of the final tau's probe emits the plan; the
+  // others are done (nothing touches their shared memory after the last cluster barrier).  If the
+  // last round did not log it (the final tau was found in an earlier round, or the log buffers do
+  // not fit), CTA 0 runs one logged probe at the final tau.
+  const int log_node = sm.log_buf;
+  const int owner = log_node < 0 ? 0 : log_node % csize;
+  if (crank != owner) return;
+  const int log_buf = log_node < 0 ? 0 : 1 + log_node / csize;
+  if (warp == 0 && sm.n_probes > 0 && log_node < 0) {
     int nl;
     probe<RPL, true>(sm, tau, R, n_slot, u_min, strict, lane, logs, nl);
     if (lane == 0) sm.n_log = nl;
   }
-  const int4* lg = logs + (size_t)(log_buf < 0 ? 0 : log_buf) * log_cap;
+  const int4* lg = logs + (size_t)log_buf * log_cap;
   if (tid < E) { sm.u_main[tid] = sm.lam[tid]; sm.n_rep[tid] = 0; sm.first[tid] = 0x7fffffff; }
   const int RP = R * P;
   const bool pc_in_smem = RP <= kPcSmem;
@@ -423,6 +461,8 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     out.scalars[UEP_SC_N_GROUPS] = n_groups;
     for (int i = UEP_SC_N_GROUPS + 1; i < UEP_N_SCALARS; ++i) out.scalars[i] = 0;
 #ifdef UEP_PLAN_TIMING   // developer probe: cycles of setup / bisection / final probe / emit
+    out.scalars[10] = (int)(t_s1 - t_start);
+    out.scalars[11] = (int)(t_s2 - t_s1);
     out.scalars[12] = (int)(t_setup - t_start);
     out.scalars[13] = (int)(t_bisect - t_setup);
     out.scalars[14] = (int)(t_final - t_bisect);
@@ -437,14 +477,30 @@ template <int RPL>
 static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out& plan,
                          cudaStream_t s) {
   const uep_config& g = c->cfg;
+  const int levels = 6;                                        // 63 nodes over kPlanCluster CTAs
+  const int cluster = c->plan_cluster;
+  const int warps = ((1 << levels) + cluster - 1) / cluster;   // probing warps per CTA
   const int log_cap = std::max(1, g.R * g.n_slot);
-  const int n_bufs = (32 * (size_t)log_cap * sizeof(int4) <= kLogBudget) ? 32 : 1;
+  const int n_bufs = ((size_t)(1 + warps) * log_cap * sizeof(int4) <= kLogBudget) ? 1 + warps : 1;
   const size_t smem = ((sizeof(PlanSmem) + 15) & ~(size_t)15) + (size_t)n_bufs * log_cap * sizeof(int4);
-  plan_kernel<RPL><<<1, kPlanThreads, smem, s>>>(
-      count, c->d_home, c->d_main_phys, c->d_roff, c->d_rexp, plan, g.E, g.R, g.n_slot, c->M, c->P,
-      g.u_min, g.beta_num, g.beta_den, g.floor_mode == UEP_FLOOR_STRICT ? 1 : 0, c->S, n_bufs,
-      log_cap);
-  UEP_CUDA_TRY(cudaGetLastError());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(cluster);
+  cfg.blockDim = dim3(kPlanThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = cluster;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, plan_kernel<RPL>, count, (const int32_t*)c->d_home,
+                                  (const int32_t*)c->d_main_phys, (const int32_t*)c->d_roff,
+                                  (const int32_t*)c->d_rexp, plan, g.E, g.R, g.n_slot, c->M, c->P,
+                                  g.u_min, g.beta_num, g.beta_den,
+                                  g.floor_mode == UEP_FLOOR_STRICT ? 1 : 0, c->S, n_bufs, log_cap,
+                                  levels));
   return UEP_OK;
 }
 
@@ -456,13 +512,40 @@ int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cu
   return launch_plan_t<8>(c, count, plan, s);
 }
 
-int init_plan_kernels() {
+template <int RPL>
+static int init_plan_one(int& max16) {
   const int bytes = (int)(sizeof(PlanSmem) + 16 + kLogBudget);
-  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(16);
+  cfg.blockDim = dim3(kPlanThreads);
+  cfg.dynamicSmemBytes = bytes;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 16;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  int n = 0;
+  if (cudaOccupancyMaxActiveClusters(&n, plan_kernel<RPL>, &cfg) != cudaSuccess) { cudaGetLastError(); n = 0; }
+  max16 = std::min(max16, n);
   return UEP_OK;
+}
+
+int init_plan_kernels(Ctx* c) {
+  int max16 = 1 << 30;
+  int rc = init_plan_one<1>(max16);
+  if (rc == UEP_OK) rc = init_plan_one<2>(max16);
+  if (rc == UEP_OK) rc = init_plan_one<4>(max16);
+  if (rc == UEP_OK) rc = init_plan_one<8>(max16);
+  c->plan_cluster = 8;
+  if (const char* e = getenv("UEP_PLAN_CLUSTER")) {        // developer override: 1, 2, 4, 8 or 16
+    const int v = atoi(e);
+    if (v == 1 || v == 2 || v == 4 || v == 8 || (v == 16 && max16 >= 1)) c->plan_cluster = v;
+  }
+  return rc;
 }
 
 }  // namespace uep

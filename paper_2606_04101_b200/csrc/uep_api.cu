@@ -134,7 +134,7 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
   UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_rank, cudaEventDisableTiming));
 #undef UEP_TRY_OR_FAIL
-  int rc = init_plan_kernels();
+  int rc = init_plan_kernels(c);
   if (rc == UEP_OK) rc = init_hist_kernels();
   if (rc == UEP_OK) rc = init_remap_kernels();
   if (rc == UEP_OK) rc = init_pack_kernels();

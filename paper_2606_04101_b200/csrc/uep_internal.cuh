@@ -19,7 +19,7 @@ constexpr int kRemapWarps = kRemapThreads / 32;
 constexpr int kRemapItems = 16;          // slots per lane per round (register-resident)
 constexpr int kRemapRound = kRemapThreads * kRemapItems;   // 16384 slots per CTA round
 constexpr int kPlanThreads = 1024;
-constexpr int kPlanLevels = 5;           // bisection levels speculated per round (2^5-1 warps)
+constexpr int kPlanLevels = 6;           // bisection levels speculated per round (63 probes over a cluster of 8 CTAs)
 constexpr int kPackTile = 16 * 1024;     // bytes per bulk-copy tile
 constexpr int kPackStages = 8;           // shared-memory ring depth
 constexpr int kMinChunk = 2048;          // smallest histogram/remap chunk (slots per CTA)
@@ -34,6 +34,7 @@ struct Ctx {
   int n_chunks, chunk_len;
   int sm_count;
   int pack_ctas;
+  int plan_cluster;       // CTAs per plan solve (thread-block cluster size)
   // static layout, device
   int32_t* d_home;        // [E]   h(e)
   int32_t* d_main_phys;   // [E]   index of e among E_{h(e)} ascending
@@ -64,7 +65,8 @@ int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_p
                  int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
                  void* ws, cudaStream_t s);
 int launch_pack(const Ctx* c, const uep_plan_out& plan, const PackArgs& a, cudaStream_t s);
-int init_plan_kernels();          // opt-in shared memory attributes
+struct Ctx;
+int init_plan_kernels(Ctx* c);    // opt-in shared memory attributes, cluster size
 int init_remap_kernels();
 int init_pack_kernels();
 
