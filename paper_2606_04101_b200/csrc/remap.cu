@@ -31,15 +31,15 @@
 namespace uep {
 
 constexpr unsigned kFullMask = 0xffffffffu;
-constexpr size_t kMaxSmem = 227 * 1024;
 constexpr int kEMask = (1 << kPackedEBits) - 1;
 
 // ------------------------------------------------------------------------------------------------
 // rank_kernel.  dynamic shared memory: wrow[kRemapWarps][E_pad] (int2 {mask, count})
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kRemapThreads, 1)
-rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len,
-            int32_t* __restrict__ packed) {
+__global__ void __launch_bounds__(kRemapThreads, 2)
+rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len, int n_chunks,
+            int32_t* __restrict__ packed, int32_t* __restrict__ prefix,
+            unsigned* __restrict__ ticket) {
   extern __shared__ __align__(16) int smem[];
   int2* wrow = reinterpret_cast<int2*>(smem);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -83,17 +83,25 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
   }
   __syncthreads();
 
-  // cross-warp exclusive scan per expert column; the count field becomes the base of (warp, e)
-  for (int e = tid; e < E; e += kRemapThreads) {
+  // cross-warp exclusive scan per expert column; the count field becomes the base of (warp, e);
+  // the column total is this chunk's row of the count table (row c+1: row 0 stays zero, so that
+  // the in-place inclusive scan over rows below leaves the EXCLUSIVE prefix in row c)
+  for (int e = tid; e < E_pad; e += kRemapThreads) {
     int run = 0;
+    if (e < E) {
 #pragma unroll 8
-    for (int w = 0; w < kRemapWarps; ++w) {
-      const int x = wrow[w * E_pad + e].y;
-      wrow[w * E_pad + e].y = run;
-      run += x;
+      for (int w = 0; w < kRemapWarps; ++w) {
+        const int x = wrow[w * E_pad + e].y;
+        wrow[w * E_pad + e].y = run;
+        run += x;
+      }
     }
+    prefix[(size_t)(blockIdx.x + 1) * E_pad + e] = run;
   }
+  __threadfence();
   __syncthreads();
+  __shared__ unsigned s_last;
+  if (tid == 0) s_last = (atomicAdd(ticket, 1u) == (unsigned)(n_chunks - 1));
 
 #pragma unroll
   for (int i = 0; i < kRemapItems; ++i) {
@@ -102,13 +110,55 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
       packed[i * 32] = (pk >= 0) ? pk + (wr[pk & kEMask].y << kPackedEBits) : -1;
     }
   }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+
+  // Last CTA: rows 1..n_chunks hold per-chunk counts; inclusive scan over rows, in place, turns
+  // row c into the exclusive prefix of chunk c and row n_chunks into the totals.  Each thread
+  // owns 4 columns (int4) of a contiguous block of rows; two passes over L2 (block sums, then
+  // scan + write), off the critical path of uep_balance.
+  {
+    int* part = reinterpret_cast<int*>(smem);              // wrow is dead: [NRG][E_pad] block sums
+    const int CG = E_pad >> 2;
+    const int NRG = min(16, kRemapThreads / CG);
+    const int cg = tid % CG, rg = tid / CG;
+    const int K = (n_chunks + NRG - 1) / NRG;
+    const int r0 = 1 + rg * K, r1 = min(n_chunks + 1, r0 + K);
+    int4* col = reinterpret_cast<int4*>(prefix) + cg;
+    int4 acc = make_int4(0, 0, 0, 0);
+    if (rg < NRG) {
+#pragma unroll 8
+      for (int r = r0; r < r1; ++r) {
+        const int4 v = __ldcg(col + (size_t)r * CG);
+        acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+      }
+      reinterpret_cast<int4*>(part)[rg * CG + cg] = acc;
+    }
+    __syncthreads();
+    if (rg < NRG) {
+      int4 run = make_int4(0, 0, 0, 0);
+      for (int g = 0; g < rg; ++g) {
+        const int4 v = reinterpret_cast<int4*>(part)[g * CG + cg];
+        run.x += v.x; run.y += v.y; run.z += v.z; run.w += v.w;
+      }
+#pragma unroll 8
+      for (int r = r0; r < r1; ++r) {
+        const int4 v = __ldcg(col + (size_t)r * CG);
+        run.x += v.x; run.y += v.y; run.z += v.z; run.w += v.w;
+        col[(size_t)r * CG] = run;
+      }
+    }
+    if (tid == 0) *ticket = 0u;        // self-reset for the next launch (graph replay)
+  }
 }
 
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s) {
   if (c->S == 0) return UEP_OK;
   const size_t smem = sizeof(int2) * (size_t)kRemapWarps * c->E_pad;
-  rank_kernel<<<c->n_chunks, kRemapThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad, c->chunk_len,
-                                                       ws_packed(c, ws));
+  rank_kernel<<<c->r_chunks, kRemapThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
+                                                      c->r_chunk_len, c->r_chunks, ws_packed(c, ws),
+                                                      ws_prefix(c, ws), ws_ticket(ws) + 1);
   UEP_CUDA_TRY(cudaGetLastError());
   return UEP_OK;
 }
@@ -117,22 +167,20 @@ int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s) {
 // lookup_kernel.  dynamic shared memory layout (ints):
 //   rec[E_pad] (int4) | base0[E_pad] | elb[E_pad] | s_off[E_pad+4] | rbase[(R+7)&~3]
 //   | i_cum | i_dbase | i_gbase | i_rank (icap each) | wtot[36]
-//   | scratch: part[kColPartInts] while staging, then (STAGE) sg[kMaxChunk] gates + sd[kMaxChunk] ints
+//   | (STAGE) sg[kMaxChunk] gates + sd[kMaxChunk] ints
 // ------------------------------------------------------------------------------------------------
 __host__ __device__ inline size_t lookup_smem_bytes(int E_pad, int R, int inst_cap, bool stage,
                                                     int gate_bytes) {
   const size_t fixed = 4 * (size_t)E_pad + 2 * (size_t)E_pad + (E_pad + 4) + ((R + 7) & ~3) +
                        4 * (size_t)((inst_cap + 3) & ~3) + 36;
-  size_t scratch = sizeof(int) * (size_t)kColPartInts;
-  const size_t st = (size_t)kMaxChunk * (gate_bytes + sizeof(int));
-  if (stage && st > scratch) scratch = st;
+  const size_t scratch = stage ? (size_t)kMaxChunk * (gate_bytes + sizeof(int)) : 0;
   return sizeof(int) * fixed + scratch;
 }
 
 template <typename GateT, bool STAGE>
-__global__ void __launch_bounds__(kRemapThreads, 1)
+__global__ void __launch_bounds__(kRemapThreads, 2)
 lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate, int S, int E,
-              int E_pad, int R, int inst_cap, int chunk_len, const int32_t* __restrict__ table,
+              int E_pad, int R, int inst_cap, int chunk_len, const int32_t* __restrict__ prefix,
               const int32_t* __restrict__ g_inst_off, const int32_t* __restrict__ g_inst_rank,
               const int32_t* __restrict__ g_inst_cum, const int32_t* __restrict__ g_inst_base,
               const int32_t* __restrict__ g_rank_base, int32_t* __restrict__ out_replica,
@@ -150,8 +198,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   int* i_gbase = i_dbase + icap;                 // rank_base[rank] + i_dbase
   int* i_rank = i_gbase + icap;
   int* wtot = i_rank + icap;                     // [32] warp totals, [32] = chunk total
-  int* part = wtot + 36;                         // column-sum partials (staging only)
-  GateT* sg = reinterpret_cast<GateT*>(part);    // staged gates, (expert, rank) order
+  GateT* sg = reinterpret_cast<GateT*>(wtot + 36);    // staged gates, (expert, rank) order
   int* sd = reinterpret_cast<int*>(sg + kMaxChunk);   // their out_gate index
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -176,23 +223,9 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
     if (has_gate) gv[i] = in ? __ldg(gate + i * 32) : GateT(0);
   }
 
-  // ---- chunk base ranks: column sums of the table rows below this chunk (loads in flight) ------
-  const int CG = E_pad >> 2;
-  const int NRG = min(32, kRemapThreads / CG);
-  {
-    const int cg = tid % CG, rg = tid / CG;
-    if (rg < NRG) {
-      int4 acc = make_int4(0, 0, 0, 0);
-      const int4* col = reinterpret_cast<const int4*>(table) + cg;
-#pragma unroll 10
-      for (int r = rg; r < c; r += NRG) {
-        const int4 v = __ldcg(col + (size_t)r * CG);
-        acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
-      }
-      reinterpret_cast<int4*>(part)[rg * CG + cg] = acc;
-    }
-  }
-  const int n_own = (tid < E) ? __ldcg(table + (size_t)c * E_pad + tid) : 0;   // slots of e in this chunk
+  // ---- chunk base ranks: row c of the exclusive prefix over chunks that rank_kernel left ----------
+  const int b0_own = (tid < E) ? __ldcg(prefix + (size_t)c * E_pad + tid) : 0;
+  const int n_own = (tid < E) ? __ldcg(prefix + (size_t)(c + 1) * E_pad + tid) - b0_own : 0;
   // ---- stage the plan (coalesced, L2-resident) ---------------------------------------------------
   for (int e = tid; e <= E; e += kRemapThreads) s_off[e] = g_inst_off[e];
   for (int r = tid; r <= R; r += kRemapThreads) rbase[r] = g_rank_base[r];
@@ -212,11 +245,9 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   }
   if (lane == 31) wtot[warp] = el_inc;
   __syncthreads();
-  for (int e = tid; e < E_pad; e += kRemapThreads) {
-    int sum = 0;
-    for (int g = 0; g < NRG; ++g) sum += part[g * E_pad + e];
-    base0[e] = sum;
-    if (e < E) i_dbase[s_off[e]] = 0;            // first instance of an expert: cum_prev = 0
+  if (tid < E) {
+    base0[tid] = b0_own;
+    i_dbase[s_off[tid]] = 0;                     // first instance of an expert: cum_prev = 0
   }
   {
     int pre = 0;
@@ -297,8 +328,8 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
   const bool stage = gate != nullptr;
   const size_t smem = lookup_smem_bytes(c->E_pad, g.R, inst_cap, stage, sizeof(GateT));
   auto k = stage ? lookup_kernel<GateT, true> : lookup_kernel<GateT, false>;
-  k<<<c->n_chunks, kRemapThreads, smem, s>>>(
-      ws_packed(c, ws), gate, c->S, g.E, c->E_pad, g.R, inst_cap, c->chunk_len, ws_table(ws),
+  k<<<c->r_chunks, kRemapThreads, smem, s>>>(
+      ws_packed(c, ws), gate, c->S, g.E, c->E_pad, g.R, inst_cap, c->r_chunk_len, ws_prefix(c, ws),
       p.inst_off, p.inst_rank, p.inst_cum, p.inst_base, p.rank_base, out_replica, out_rank,
       out_offset, out_gate);
   UEP_CUDA_TRY(cudaGetLastError());
@@ -306,8 +337,9 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
 }
 
 int init_remap_kernels() {
-  const int bytes = (int)kMaxSmem;
-  UEP_CUDA_TRY(cudaFuncSetAttribute(rank_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  const int rank_bytes = (int)(sizeof(int2) * (size_t)kRemapWarps * UEP_MAX_E);
+  const int bytes = (int)lookup_smem_bytes(UEP_MAX_E, UEP_MAX_R, UEP_MAX_E + UEP_MAX_R * UEP_MAX_NSLOT, true, 4);
+  UEP_CUDA_TRY(cudaFuncSetAttribute(rank_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rank_bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint16_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));

@@ -105,16 +105,22 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   c->M = M;
   c->P = M + cfg->n_slot;
 
-  // launch geometry: one histogram/rank/lookup CTA per chunk; one chunk per SM while a chunk fits
-  // the register-resident round of the rank kernel (kMaxChunk slots), more chunks beyond that.
-  // Chunks are whole 1024-slot steps so that every chunk but the last runs unpredicated.
+  // launch geometry.  Histogram: one CTA per chunk, one chunk per SM (whole 128-slot lines).
+  // Remap (rank + lookup kernels): chunks of whole 512-slot steps, <= kMaxChunk slots (one
+  // register-resident round), about two chunks per SM so that co-resident CTAs overlap their
+  // load / rank / store phases.
   {
     long long per = (S + c->sm_count - 1) / c->sm_count;
     per = std::max<long long>(per, kMinChunk);
-    per = (per + 1023) / 1024 * 1024;
-    per = std::min<long long>(per, kMaxChunk);
+    per = (per + 127) / 128 * 128;
     c->chunk_len = (int)per;
     c->n_chunks = (int)std::max<long long>(1, (S + per - 1) / per);
+    long long rper = (S + 2 * c->sm_count - 1) / (2 * c->sm_count);
+    rper = std::max<long long>(rper, kMinChunk);
+    rper = (rper + kRemapThreads - 1) / kRemapThreads * kRemapThreads;
+    rper = std::min<long long>(rper, kMaxChunk);
+    c->r_chunk_len = (int)rper;
+    c->r_chunks = (int)std::max<long long>(1, (S + rper - 1) / rper);
   }
   c->pack_ctas = c->sm_count;
 
@@ -160,13 +166,15 @@ void uep_destroy(uep_ctx* ctx) {
 size_t uep_workspace_bytes(const uep_ctx* ctx) {
   const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
   if (!c) return 0;
-  return (size_t)kWsHeaderBytes + ws_table_bytes(c) + sizeof(int32_t) * (((size_t)c->S + 63) & ~(size_t)63);
+  return (size_t)kWsHeaderBytes + ws_table_bytes(c) + ws_prefix_bytes(c) + sizeof(int32_t) * (((size_t)c->S + 63) & ~(size_t)63);
 }
 
 int uep_workspace_init(const uep_ctx* ctx, void* ws, void* stream) {
   const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
   if (!c || !ws || !aligned16(ws)) return UEP_ERR_INVALID_ARG;
+  // tickets, and row 0 of the remap prefix table (it stays zero: the scan starts at row 1)
   UEP_CUDA_TRY(cudaMemsetAsync(ws, 0, kWsHeaderBytes, static_cast<cudaStream_t>(stream)));
+  UEP_CUDA_TRY(cudaMemsetAsync(ws_prefix(c, ws), 0, ws_prefix_bytes(c), static_cast<cudaStream_t>(stream)));
   return UEP_OK;
 }
 

@@ -12,12 +12,12 @@
 
 namespace uep {
 
-constexpr int kWsHeaderBytes = 256;      // [0] ticket of the histogram's last-CTA reduction
+constexpr int kWsHeaderBytes = 256;      // [0] ticket of the histogram's last-CTA reduction, [1] of rank_kernel's
 constexpr int kHistThreads = 1024;
-constexpr int kRemapThreads = 1024;
+constexpr int kRemapThreads = 512;
 constexpr int kRemapWarps = kRemapThreads / 32;
 constexpr int kRemapItems = 16;          // slots per lane per round (register-resident)
-constexpr int kRemapRound = kRemapThreads * kRemapItems;   // 16384 slots per CTA round
+constexpr int kRemapRound = kRemapThreads * kRemapItems;   // 8192 slots per CTA
 constexpr int kPlanThreads = 1024;
 constexpr int kPlanLevels = 6;           // bisection levels speculated per round (63 probes over a cluster of 8 CTAs)
 constexpr int kPackTile = 16 * 1024;     // bytes per bulk-copy tile
@@ -31,7 +31,8 @@ struct Ctx {
   int S;                  // T*k
   int M, P;               // main / physical slots per rank
   int E_pad;              // E rounded up to a multiple of 4 (row pitch of the chunk table)
-  int n_chunks, chunk_len;
+  int n_chunks, chunk_len;        // histogram geometry: one CTA per chunk, one chunk per SM
+  int r_chunks, r_chunk_len;      // remap geometry (rank + lookup kernels): <= kMaxChunk slots per CTA
   int sm_count;
   int pack_ctas;
   int plan_cluster;       // CTAs per plan solve (thread-block cluster size)
@@ -111,8 +112,15 @@ inline unsigned* ws_ticket(void* ws) { return reinterpret_cast<unsigned*>(ws); }
 inline size_t ws_table_bytes(const Ctx* c) {
   return (sizeof(int32_t) * (size_t)c->n_chunks * c->E_pad + 255) & ~(size_t)255;
 }
-inline int32_t* ws_packed(const Ctx* c, void* ws) {      // [S] packed (expert, rank in chunk)
+inline size_t ws_prefix_bytes(const Ctx* c) {            // [r_chunks + 1][E_pad]
+  return (sizeof(int32_t) * ((size_t)c->r_chunks + 1) * c->E_pad + 255) & ~(size_t)255;
+}
+inline int32_t* ws_prefix(const Ctx* c, void* ws) {      // exclusive prefix over remap chunks (+ totals row)
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c));
+}
+inline int32_t* ws_packed(const Ctx* c, void* ws) {      // [S] packed (expert, rank in chunk)
+  return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c) +
+                                    ws_prefix_bytes(c));
 }
 
 }  // namespace uep
