@@ -263,48 +263,63 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
     i_gbase[p] = rbase[i_rank[p]] + d;
   }
   __syncthreads();
-  // rec[e], in chunk-rank space: {cum - base0, dbase + base0, gbase + base0, rep<<16|rank} of the
-  // instance holding the chunk's first slot of e
+  // rec[e], in chunk-rank space: {cum - base0, dbase + base0, gbase + base0,
+  // staging base << 19 | replica << 8 | rank} of the instance holding the chunk's first slot of e
   for (int e = tid; e < E; e += kRemapThreads) {
     const int lo = s_off[e], last = s_off[e + 1] - 1, b0 = base0[e];
     int p = lo;
     while (p < last && i_cum[p] <= b0) ++p;
-    rec[e] = make_int4(i_cum[p] - b0, i_dbase[p] + b0, i_gbase[p] + b0, ((p - lo) << 16) | i_rank[p]);
+    rec[e] = make_int4(i_cum[p] - b0, i_dbase[p] + b0, i_gbase[p] + b0,
+                       (int)(((unsigned)elb[e] << 19) | (unsigned)((p - lo) << 8) | (unsigned)i_rank[p]));
   }
   __syncthreads();
 
+  // two slots at a time: their records are loaded before any of them stores to shared memory
+  // (the compiler cannot prove that the staging stores do not alias the records)
 #pragma unroll
-  for (int i = 0; i < kRemapItems; ++i) {
-    if (i < items && i * 32 < room) {
-      const int pk = pv[i];
-      int rep = -1, rk = -1, of = -1;
-      if (pk >= 0) {
-        const int e = pk & kEMask, jl = pk >> kPackedEBits;
-        const int4 rc = rec[e];
-        int db = rc.y, gb = rc.z, rr = rc.w;
-        if (jl >= rc.x) {                                // past the first instance of this chunk's window
-          const int b0 = base0[e], j = jl + b0;
-          int p = s_off[e] + (rr >> 16) + 1;
-          const int last = s_off[e + 1] - 1;             // cum[last] = lambda_e > j when ws matches plan
-          while (p < last && i_cum[p] <= j) ++p;
-          db = i_dbase[p] + b0; gb = i_gbase[p] + b0; rr = ((p - s_off[e]) << 16) | i_rank[p];
-        }
-        rep = rr >> 16;
-        rk = rr & 0xffff;
-        of = db + jl;
-        if (has_gate) {
-          if (STAGE) {
-            const int lp = elb[e] + jl;
-            sg[lp] = gv[i];
-            sd[lp] = gb + jl;
-          } else {
-            out_gate[gb + jl] = gv[i];
+  for (int i0 = 0; i0 < kRemapItems; i0 += 2) {
+    if (i0 < items) {
+      int4 rc[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int pk = pv[i0 + u];
+        rc[u] = rec[pk >= 0 ? (pk & kEMask) : 0];
+      }
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int i = i0 + u;
+        if (i < items && i * 32 < room) {
+          const int pk = pv[i];
+          int rep = -1, rk = -1, of = -1;
+          if (pk >= 0) {
+            const int e = pk & kEMask, jl = pk >> kPackedEBits;
+            int db = rc[u].y, gb = rc[u].z;
+            const unsigned rw = (unsigned)rc[u].w;
+            rep = (int)((rw >> 8) & 0x7ffu);
+            rk = (int)(rw & 0xffu);
+            if (jl >= rc[u].x) {                         // past the first instance of this chunk's window
+              const int b0 = base0[e], j = jl + b0;
+              int p = s_off[e] + rep + 1;
+              const int last = s_off[e + 1] - 1;         // cum[last] = lambda_e > j when ws matches plan
+              while (p < last && i_cum[p] <= j) ++p;
+              db = i_dbase[p] + b0; gb = i_gbase[p] + b0; rep = p - s_off[e]; rk = i_rank[p];
+            }
+            of = db + jl;
+            if (has_gate) {
+              if (STAGE) {
+                const int lp = (int)(rw >> 19) + jl;
+                sg[lp] = gv[i];
+                sd[lp] = gb + jl;
+              } else {
+                out_gate[gb + jl] = gv[i];
+              }
+            }
           }
+          out_replica[i * 32] = rep;
+          out_rank[i * 32] = rk;
+          out_offset[i * 32] = of;
         }
       }
-      out_replica[i * 32] = rep;
-      out_rank[i * 32] = rk;
-      out_offset[i * 32] = of;
     }
   }
 
