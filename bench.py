@@ -377,7 +377,7 @@ def run_uep(args):
                     "n_probes_mean": round(statistics.mean(int(s[binding.SC_N_PROBES]) for s in sc), 1)},
         "roofline": {k: r_pack[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")},
         "rooflines": rooflines,
-        "gpu_launches": 5 * K,
+        "gpu_launches": 6 * K,
         "clocks": clocks,
         "launch_info": rig.ctx.launch_info,
     }

@@ -20,7 +20,8 @@
 // cell of their expert, read {mask, count} back with one 64-bit load, and the lowest peer stores
 // {0, count + popc(mask)}.  Rank = count + popc(mask & lower lanes): stable by construction, no
 // order-dependent atomic result is ever used (the OR is commutative).  One cross-warp scan per
-// expert column turns the counts into chunk-wide bases.
+// expert column turns the counts into chunk-wide bases and gives the chunk's row of a count
+// table, which prefix_kernel (a thread per row, a CTA per four columns) scans over chunks.
 //
 // lookup_kernel: per CTA and expert one 16-B record describes the instance holding the CTA's
 // first slot of that expert; a slot only walks further when it crosses a quota edge.  Gates are
@@ -37,9 +38,8 @@ constexpr int kEMask = (1 << kPackedEBits) - 1;
 // rank_kernel.  dynamic shared memory: wrow[kRemapWarps][E_pad] (int2 {mask, count})
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kRemapThreads, 2)
-rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len, int n_chunks,
-            int32_t* __restrict__ packed, int32_t* __restrict__ prefix,
-            unsigned* __restrict__ ticket) {
+rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len,
+            int32_t* __restrict__ packed, int32_t* __restrict__ prefix) {
   extern __shared__ __align__(16) int smem[];
   int2* wrow = reinterpret_cast<int2*>(smem);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -98,10 +98,7 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
     }
     prefix[(size_t)(blockIdx.x + 1) * E_pad + e] = run;
   }
-  __threadfence();
   __syncthreads();
-  __shared__ unsigned s_last;
-  if (tid == 0) s_last = (atomicAdd(ticket, 1u) == (unsigned)(n_chunks - 1));
 
 #pragma unroll
   for (int i = 0; i < kRemapItems; ++i) {
@@ -110,46 +107,49 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
       packed[i * 32] = (pk >= 0) ? pk + (wr[pk & kEMask].y << kPackedEBits) : -1;
     }
   }
-  __syncthreads();
-  if (!s_last) return;
-  __threadfence();
+}
 
-  // Last CTA: rows 1..n_chunks hold per-chunk counts; inclusive scan over rows, in place, turns
-  // row c into the exclusive prefix of chunk c and row n_chunks into the totals.  Each thread
-  // owns 4 columns (int4) of a contiguous block of rows; two passes over L2 (block sums, then
-  // scan + write), off the critical path of uep_balance.
-  {
-    int* part = reinterpret_cast<int*>(smem);              // wrow is dead: [NRG][E_pad] block sums
-    const int CG = E_pad >> 2;
-    const int NRG = min(16, kRemapThreads / CG);
-    const int cg = tid % CG, rg = tid / CG;
-    const int K = (n_chunks + NRG - 1) / NRG;
-    const int r0 = 1 + rg * K, r1 = min(n_chunks + 1, r0 + K);
-    int4* col = reinterpret_cast<int4*>(prefix) + cg;
-    int4 acc = make_int4(0, 0, 0, 0);
-    if (rg < NRG) {
-#pragma unroll 8
-      for (int r = r0; r < r1; ++r) {
-        const int4 v = __ldcg(col + (size_t)r * CG);
-        acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+// prefix_kernel: rows 1..n_rows of the count table hold per-chunk counts (row 0 is zero);
+// inclusive scan over rows, in place, turns row c into the EXCLUSIVE prefix of chunk c and row
+// n_rows into the totals.  One CTA per int4 column group, one thread per row (blocks of 1024
+// rows with a carry): one L2 round trip per block instead of a serial walk.
+__global__ void __launch_bounds__(1024, 1)
+prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG) {
+  __shared__ int4 wsum[32];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  int4* col = reinterpret_cast<int4*>(prefix) + blockIdx.x;
+  int4 carry = make_int4(0, 0, 0, 0);
+  for (int base = 1; base <= n_rows; base += 1024) {
+    const int r = base + tid;
+    int4 v = (r <= n_rows) ? __ldcg(col + (size_t)r * CG) : make_int4(0, 0, 0, 0);
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int x = __shfl_up_sync(kFullMask, v.x, o), y = __shfl_up_sync(kFullMask, v.y, o);
+      const int z = __shfl_up_sync(kFullMask, v.z, o), w = __shfl_up_sync(kFullMask, v.w, o);
+      if (lane >= o) { v.x += x; v.y += y; v.z += z; v.w += w; }
+    }
+    if (lane == 31) wsum[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+      int4 t = wsum[lane];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int x = __shfl_up_sync(kFullMask, t.x, o), y = __shfl_up_sync(kFullMask, t.y, o);
+        const int z = __shfl_up_sync(kFullMask, t.z, o), w = __shfl_up_sync(kFullMask, t.w, o);
+        if (lane >= o) { t.x += x; t.y += y; t.z += z; t.w += w; }
       }
-      reinterpret_cast<int4*>(part)[rg * CG + cg] = acc;
+      wsum[lane] = t;
     }
     __syncthreads();
-    if (rg < NRG) {
-      int4 run = make_int4(0, 0, 0, 0);
-      for (int g = 0; g < rg; ++g) {
-        const int4 v = reinterpret_cast<int4*>(part)[g * CG + cg];
-        run.x += v.x; run.y += v.y; run.z += v.z; run.w += v.w;
-      }
-#pragma unroll 8
-      for (int r = r0; r < r1; ++r) {
-        const int4 v = __ldcg(col + (size_t)r * CG);
-        run.x += v.x; run.y += v.y; run.z += v.z; run.w += v.w;
-        col[(size_t)r * CG] = run;
-      }
+    if (warp > 0) {
+      const int4 p = wsum[warp - 1];
+      v.x += p.x; v.y += p.y; v.z += p.z; v.w += p.w;
     }
-    if (tid == 0) *ticket = 0u;        // self-reset for the next launch (graph replay)
+    v.x += carry.x; v.y += carry.y; v.z += carry.z; v.w += carry.w;
+    if (r <= n_rows) col[(size_t)r * CG] = v;
+    const int4 tot = wsum[31];
+    carry.x += tot.x; carry.y += tot.y; carry.z += tot.z; carry.w += tot.w;
+    __syncthreads();
   }
 }
 
@@ -157,8 +157,10 @@ int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s) {
   if (c->S == 0) return UEP_OK;
   const size_t smem = sizeof(int2) * (size_t)kRemapWarps * c->E_pad;
   rank_kernel<<<c->r_chunks, kRemapThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
-                                                      c->r_chunk_len, c->r_chunks, ws_packed(c, ws),
-                                                      ws_prefix(c, ws), ws_ticket(ws) + 1);
+                                                      c->r_chunk_len, ws_packed(c, ws),
+                                                      ws_prefix(c, ws));
+  UEP_CUDA_TRY(cudaGetLastError());
+  prefix_kernel<<<c->E_pad / 4, 1024, 0, s>>>(ws_prefix(c, ws), c->r_chunks, c->E_pad / 4);
   UEP_CUDA_TRY(cudaGetLastError());
   return UEP_OK;
 }

@@ -307,3 +307,52 @@ def test_error_codes_and_empty_input():
     for n in PLAN_ARRAYS[:-1]:
         assert np.array_equal(np.asarray(getattr(hp, n)).reshape(-1),
                               np.asarray(getattr(op, n)).reshape(-1)), n
+
+
+def test_remap_halves_on_two_streams_and_workspace_reuse():
+    """uep_remap_rank is plan-independent: run it on a second stream beside histogram + plan, join,
+    then uep_remap_lookup; and reuse the same context/workspace for a second, different input."""
+    T, k, E, R, ns, um = 40000, 4, 96, 24, 2, 128          # ragged: S = 160000 is not a chunk multiple
+    ctx = binding.Context(T, k, E, R, ns, um)
+    ws = ctx.new_workspace()
+    plan = ctx.new_plan(dense_U=True)
+    main, side = torch.cuda.Stream(), torch.cuda.Stream()
+    for seed in (3, 4):
+        ids = synth.zipf_topk_ids(T, k, E, 1.3, seed)
+        gate = synth.gates_uniform_renorm(T, k, seed)
+        d_ids, d_gate = ids.to(DEV), gate.to(DEV)
+        count = torch.zeros(E, dtype=torch.int32, device=DEV)
+        rep, rnk, off, og = ctx.new_outputs(d_gate)
+        torch.cuda.synchronize()
+        ctx.uep_remap_rank(d_ids, ws, side)
+        ev = torch.cuda.Event()
+        ev.record(side)
+        ctx.uep_histogram(d_ids, count, ws, main)
+        ctx.uep_plan(count, plan, ws, main)
+        main.wait_event(ev)
+        ctx.uep_remap_lookup(d_gate, plan, rep, rnk, off, og, ws, main)
+        torch.cuda.synchronize()
+        g = dict(count=count.cpu().numpy(), plan=plan.host(), rep=rep.cpu().numpy(),
+                 rnk=rnk.cpu().numpy(), off=off.cpu().numpy(), og=og.cpu(), dsts=[], sentinels=[])
+        assert_parity(g, oracle_chain(ids, gate, E, R, ns, um), ids, gate)
+
+
+@pytest.mark.parametrize("T,k,E,R,n_slot", [
+    (1, 1, 1, 1, 0),            # one slot, one expert, one rank
+    (3, 1, 5, 7, 1),            # E < R: ranks without main experts
+    (777, 3, 33, 5, 3),         # nothing is a multiple of anything
+    (8192, 8, 512, 256, 4),     # the limits of E, R and N_slot together
+    (524288, 8, 64, 8, 1),      # 4 Mi slots: many remap chunks per SM, two waves
+])
+def test_odd_shapes_parity(T, k, E, R, n_slot):
+    S = T * k
+    um = synth.stress_u_min(S, R)
+    ids = synth.zipf_topk_ids(T, min(k, E), E, 1.1, 17) if k <= E else None
+    if ids is None or ids.shape[1] != k:
+        ids = torch.randint(0, E, (T, k), dtype=torch.int32,
+                            generator=torch.Generator().manual_seed(5))
+    gate = synth.gates_uniform_renorm(T, k, 9)
+    g = gpu_chain(ids, gate, E, R, n_slot, um, use_balance=True)
+    o = oracle_chain(ids, gate, E, R, n_slot, um)
+    assert_parity(g, o, ids, gate)
+    ck.check_remap(ids.numpy(), g["plan"], g["rep"], g["rnk"], g["off"])
