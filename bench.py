@@ -335,21 +335,29 @@ def run_uep(args):
     bytes_pack = [(n_grp[i] + n_rep[i]) * B for i in range(n_pack)]
     us = lambda ms, n: ms * 1e3 / n
 
-    def roof(name, nbytes, dur_us):
+    # DRAM traffic per launch from the committed ncu --set full capture (dsv3_prefill only; that
+    # capture is not re-taken here: a number printed under a profiler is never a bench value)
+    traffic = {}
+    tpath = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r01_final_traffic.json")
+    if args.workload == "dsv3_prefill" and args.state_scale == 1.0 and os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f)
+
+    def roof(name, nbytes, dur_us, tkey=None):
         a = nbytes / (dur_us * 1e-6) / 1e9 if dur_us > 0 else 0.0
         return {"kernel": name, "bound": "hbm", "achieved": round(a, 1), "peak": peak_gbs,
                 "unit": "GB/s", "frac": round(a / peak_gbs, 4), "frac_of_nominal_8TBs": round(a / 8000.0, 4),
-                "traffic": None, "bytes_per_launch": int(nbytes), "us_per_launch": round(dur_us, 2),
-                "peak_source": peak_src}
+                "traffic": traffic.get(tkey or name), "bytes_per_launch": int(nbytes),
+                "us_per_launch": round(dur_us, 2), "peak_source": peak_src}
 
     pack_us = us(pack_ms, n_pack)
     r_pack = roof("pack_kernel", sum(bytes_pack) / n_pack, pack_us)
     # remap = rank_kernel + lookup_kernel: 24 B/slot algorithmic (fp32 gates) over both; each half
     # also against its own traffic (rank: 4 B id in + 4 B packed out; lookup: 4 B packed + g in,
     # 12 B + g out)
-    rooflines = [r_pack, roof("rank_kernel+lookup_kernel (uep_remap)", bytes_remap, us(remap_ms, n_inst)),
+    rooflines = [r_pack, roof("rank_kernel+prefix_kernel+lookup_kernel (uep_remap)", bytes_remap, us(remap_ms, n_inst), "lookup_kernel"),
                  roof("lookup_kernel", bytes_remap, us(lookup_ms, n_inst)),
-                 roof("rank_kernel", 8 * S, us(rank_ms, n_inst)),
+                 roof("rank_kernel+prefix_kernel (uep_remap_rank)", 8 * S, us(rank_ms, n_inst), "rank_kernel"),
                  roof("hist_kernel", bytes_hist, us(hist_ms, n_inst))]
     result = {
         "metric": METRIC, "value": round(plan_latency_us, 3), "unit": UNIT, "n_gpus": world,
