@@ -124,9 +124,10 @@ typedef struct uep_plan_out {
 int uep_create(const uep_config* cfg, uep_ctx** out);
 void uep_destroy(uep_ctx* ctx);
 
-/* Bytes of DEVICE workspace one in-flight call needs.  It carries the per-chunk expert counts
- * from uep_histogram to uep_remap (their exclusive prefix over chunks gives each slot's global
- * stable rank; uep_remap forms that prefix itself).  uep_workspace_init must be called once (async on `stream`) before first use. */
+/* Bytes of DEVICE workspace one in-flight call needs (scratch of the histogram's chunk table,
+ * and of the remap: per-chunk expert counts, their exclusive prefix over chunks and one packed
+ * int32 {expert, rank inside chunk} per slot, ~4 bytes per slot in total).
+ * uep_workspace_init must be called once (async on `stream`) before first use. */
 size_t uep_workspace_bytes(const uep_ctx* ctx);
 int uep_workspace_init(const uep_ctx* ctx, void* ws, void* stream);
 int uep_plan_bytes(const uep_ctx* ctx, uep_plan_sizes* out);      /* out: HOST */
@@ -150,7 +151,8 @@ int uep_plan(const uep_ctx* ctx, const int32_t* expert_count, const uep_plan_out
  *   out_replica/out_rank/out_offset  DEVICE int32 [T,k]; (-1,-1,-1) for an invalid id
  *   out_gate      DEVICE [T*k] gate dtype, written at rank_base[rank]+offset (raw bit copy);
  *                 positions past the number of valid slots are not written
- *   ws            must come from uep_histogram on the SAME topk_ids                          */
+ *   ws            scratch of this call (chunk ranks and their prefix over chunks); the plan must
+ *                 have been computed from the histogram of the SAME topk_ids                 */
 int uep_remap(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
               const uep_plan_out* plan, int32_t* out_replica, int32_t* out_rank,
               int32_t* out_offset, void* out_gate, void* ws, void* stream);
@@ -159,8 +161,8 @@ int uep_remap(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
  *   uep_remap_rank    plan-INDEPENDENT: stable rank of every slot among the slots of its expert
  *                     inside its chunk, written to the workspace.  Needs only topk_ids; may run
  *                     concurrently with uep_histogram / uep_plan on another stream.
- *   uep_remap_lookup  plan-DEPENDENT: needs ws after BOTH uep_histogram and uep_remap_rank on the
- *                     same topk_ids, and the plan.  Same outputs and argument rules as uep_remap.
+ *   uep_remap_lookup  plan-DEPENDENT: needs ws after uep_remap_rank on the same topk_ids, and
+ *                     the plan of those ids.  Same outputs and argument rules as uep_remap.
  * uep_remap(...) == uep_remap_rank(...) then uep_remap_lookup(...) on one stream. */
 int uep_remap_rank(const uep_ctx* ctx, const int32_t* topk_ids, void* ws, void* stream);
 int uep_remap_lookup(const uep_ctx* ctx, const void* gate, const uep_plan_out* plan,
@@ -202,8 +204,10 @@ const char* uep_last_cuda_error(void);   /* text of the last CUDA error seen on 
 
 /* Launch geometry chosen at create time, for the bench's roofline arithmetic. */
 typedef struct uep_launch_info {
-  int32_t n_chunks, chunk_len;   /* histogram / remap: CTAs and slots per CTA                   */
+  int32_t n_chunks, chunk_len;   /* histogram: CTAs and slots per CTA                           */
   int32_t hist_threads, remap_threads, plan_threads, pack_ctas, pack_tile_bytes, sm_count;
+  int32_t r_chunks, r_chunk_len; /* remap (rank + lookup kernels): CTAs and slots per CTA       */
+  int32_t plan_cluster;          /* CTAs (thread-block cluster size) sharing one plan solve     */
 } uep_launch_info;
 int uep_get_launch_info(const uep_ctx* ctx, uep_launch_info* out);
 

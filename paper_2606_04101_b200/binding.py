@@ -55,7 +55,8 @@ class _PlanOut(ctypes.Structure):
 class _LaunchInfo(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in
                 ("n_chunks", "chunk_len", "hist_threads", "remap_threads", "plan_threads",
-                 "pack_ctas", "pack_tile_bytes", "sm_count")]
+                 "pack_ctas", "pack_tile_bytes", "sm_count", "r_chunks", "r_chunk_len",
+                 "plan_cluster")]
 
 
 _lib = None

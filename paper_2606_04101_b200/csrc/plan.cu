@@ -2,20 +2,26 @@
 //
 // Latency-bound integer work (a dependent chain of arg-max steps), no HBM traffic to speak of.
 // The paper's own kernel (§5.3: one CTA, state in shared memory, several
-// probes across warps) is prior art; what is kept: one CTA, one probe per warp.  What is new:
+// probes across warps) is prior art; what is kept: all state on chip, one probe per warp.
+// What is new:
+//   * a thread-block CLUSTER of 8 CTAs shares one solve: 31+ concurrent probes on one SM queue
+//     for issue slots, spread over 8 SMs each runs at the latency of its own dependent chain;
+//     verdicts travel over distributed shared memory, one cluster barrier per round;
 //   * per-probe state (slack, used slots) lives in REGISTERS, lane t%32 owns rank t; the
 //     arg-max "largest slack, lowest rank id" is ONE redux.sync.max on a packed key
-//     (slack << 8 | 255 - t);
-//   * rank order and per-rank expert order do not depend on tau (S5): sorted once;
-//   * the sequential bisection is reproduced exactly (S9) by speculating the next kPlanLevels
-//     levels of ITS OWN tree with 2^L - 1 warps and then walking the path the sequential
-//     search takes; a k-ary search would not be equivalent;
+//     (slack << 8 | 255 - t); the owner is the lane whose key equals the reduced key;
+//   * rank order and per-rank expert order do not depend on tau (S5): sorted once
+//     into a flat visit list;
+//   * the sequential bisection is reproduced exactly (S9) by speculating the next 6 levels of
+//     ITS OWN tree (63 probes) and then walking the path the sequential search takes; a k-ary
+//     search would not be equivalent;
 //   * infeasible probes exit as soon as a visited rank keeps too much excess (S21);
 //   * the no-duplicate test of Alg. 1 line 12 is provably redundant (S7: an accepted pair
 //     (e,t) leaves slk_t = 0 or ends e's loop, and h(e) is overloaded hence has no slack);
-//   * the accept log is written only by one final probe at the final tau (deterministic, so it
-//     reproduces U~ of the last feasible probe, S10), then all 1024 threads emit X, the CSR
-//     cumulative quotas and the receive layout.
+//   * the probes of the LAST round log their accepted transfers, so the CTA that holds the log
+//     of the final tau's probe (= U~ of the last feasible probe, S10) emits X, the CSR
+//     cumulative quotas and the receive layout with all its 1024 threads; otherwise one logged
+//     probe at the final tau is run (deterministic, so it reproduces that probe).
 #include <algorithm>
 #include <cstdlib>
 #include <cooperative_groups.h>

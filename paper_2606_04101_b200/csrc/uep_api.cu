@@ -207,6 +207,9 @@ int uep_get_launch_info(const uep_ctx* ctx, uep_launch_info* out) {
   out->pack_ctas = c->pack_ctas;
   out->pack_tile_bytes = kPackTile;
   out->sm_count = c->sm_count;
+  out->r_chunks = c->r_chunks;
+  out->r_chunk_len = c->r_chunk_len;
+  out->plan_cluster = c->plan_cluster;
   return UEP_OK;
 }
 
