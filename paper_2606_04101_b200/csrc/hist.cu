@@ -43,6 +43,7 @@ hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
   __shared__ unsigned s_last;
   const int tid = threadIdx.x, warp = tid >> 5;
   const int c = blockIdx.x;
+  pdl_trigger();     // uep_balance launches the planner behind this kernel with its prologue overlapped
 
   const long long begin = (long long)c * chunk_len;
   const int len = (int)min((long long)chunk_len, (long long)S - begin);   // > 0 by construction

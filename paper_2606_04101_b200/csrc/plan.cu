@@ -65,6 +65,9 @@ struct PlanSmem {
   int warp_tmp[32];
   int feas[32];
   int lo, hi, n_probes, n_log, log_buf;
+#ifdef UEP_PLAN_TIMING
+  int tmax[8];
+#endif
   long long s_valid;
   int max_ell;
 };
@@ -184,13 +187,15 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
 #endif
 
   // ---- stage inputs ---------------------------------------------------------------------
-  if (tid < E) {
-    sm.lam[tid] = expert_count[tid];
+  pdl_trigger();                   // the lookup kernel may start its plan-independent prologue
+  if (tid < E) {                   // static layout first: it does not depend on the histogram
     sm.home[tid] = g_home[tid];
     sm.main_phys[tid] = g_main_phys[tid];
     sm.elist[tid] = g_rexp[tid];
   }
   if (tid <= R) sm.roff[tid] = g_roff[tid];
+  pdl_wait();                      // the histogram (preceding kernel) is complete
+  if (tid < E) sm.lam[tid] = expert_count[tid];
   __syncthreads();
   // line 2: l_r
   if (tid < R) {
@@ -274,6 +279,9 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       }
     }
     if (tid == 0) sm.log_buf = -1;
+#ifdef UEP_PLAN_TIMING
+    if (tid < 8) sm.tmax[tid] = 0;
+#endif
   }
   __syncthreads();
   const int tau_lo0 = sm.lo, tau_hi0 = sm.hi;
@@ -308,12 +316,18 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       if (valid) {
         int nl = 0;
         bool f;
+#ifdef UEP_PLAN_TIMING
+        const long long tp0 = clock64();
+#endif
         if (log_round) {
           f = probe<RPL, true>(sm, (l + h) >> 1, R, n_slot, u_min, strict, lane,
                                logs + (size_t)(1 + warp) * log_cap, nl);
         } else {
           f = probe<RPL, false>(sm, (l + h) >> 1, R, n_slot, u_min, strict, lane, nullptr, nl);
         }
+#ifdef UEP_PLAN_TIMING
+        if (lane < csize && round < 8) atomicMax(cluster.map_shared_rank(&sm.tmax[round], lane), (int)(clock64() - tp0));
+#endif
         if (lane < csize) {
           *cluster.map_shared_rank(&sm.node_feas[buf][node], lane) = f ? 1 : 0;
           *cluster.map_shared_rank(&sm.log_n[buf][node], lane) = nl;
@@ -467,8 +481,9 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     out.scalars[UEP_SC_N_GROUPS] = n_groups;
     for (int i = UEP_SC_N_GROUPS + 1; i < UEP_N_SCALARS; ++i) out.scalars[i] = 0;
 #ifdef UEP_PLAN_TIMING   // developer probe: cycles of setup / bisection / final probe / emit
-    out.scalars[10] = (int)(t_s1 - t_start);
-    out.scalars[11] = (int)(t_s2 - t_s1);
+    out.scalars[9] = sm.tmax[0];
+    out.scalars[10] = sm.tmax[1];
+    out.scalars[11] = sm.tmax[2];
     out.scalars[12] = (int)(t_setup - t_start);
     out.scalars[13] = (int)(t_bisect - t_setup);
     out.scalars[14] = (int)(t_final - t_bisect);
@@ -481,7 +496,7 @@ constexpr size_t kLogBudget = 128 * 1024;     // shared memory for the accept lo
 
 template <int RPL>
 static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out& plan,
-                         cudaStream_t s) {
+                         cudaStream_t s, bool pdl) {
   const uep_config& g = c->cfg;
   const int levels = 6;                                        // 63 nodes over kPlanCluster CTAs
   const int cluster = c->plan_cluster;
@@ -494,13 +509,15 @@ static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out&
   cfg.blockDim = dim3(kPlanThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = s;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = cluster;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = pdl ? 2 : 1;
   UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, plan_kernel<RPL>, count, (const int32_t*)c->d_home,
                                   (const int32_t*)c->d_main_phys, (const int32_t*)c->d_roff,
                                   (const int32_t*)c->d_rexp, plan, g.E, g.R, g.n_slot, c->M, c->P,
@@ -510,12 +527,13 @@ static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out&
   return UEP_OK;
 }
 
-int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s) {
+int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
+                bool pdl) {
   const int R = c->cfg.R;
-  if (R <= 32) return launch_plan_t<1>(c, count, plan, s);
-  if (R <= 64) return launch_plan_t<2>(c, count, plan, s);
-  if (R <= 128) return launch_plan_t<4>(c, count, plan, s);
-  return launch_plan_t<8>(c, count, plan, s);
+  if (R <= 32) return launch_plan_t<1>(c, count, plan, s, pdl);
+  if (R <= 64) return launch_plan_t<2>(c, count, plan, s, pdl);
+  if (R <= 128) return launch_plan_t<4>(c, count, plan, s, pdl);
+  return launch_plan_t<8>(c, count, plan, s, pdl);
 }
 
 template <int RPL>

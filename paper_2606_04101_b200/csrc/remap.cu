@@ -228,7 +228,16 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   // ---- chunk base ranks: row c of the exclusive prefix over chunks that rank_kernel left ----------
   const int b0_own = (tid < E) ? __ldcg(prefix + (size_t)c * E_pad + tid) : 0;
   const int n_own = (tid < E) ? __ldcg(prefix + (size_t)(c + 1) * E_pad + tid) - b0_own : 0;
-  // ---- stage the plan (coalesced, L2-resident) ---------------------------------------------------
+  int el_inc = n_own;                            // inclusive scan of n_own over experts
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int y = __shfl_up_sync(kFullMask, el_inc, o);
+    if (lane >= o) el_inc += y;
+  }
+  if (lane == 31) wtot[warp] = el_inc;
+  // ---- everything above is independent of the plan: under programmatic dependent launch it
+  // overlaps the planner (uep_balance); now wait for it and stage the plan (coalesced, in L2) ------
+  pdl_wait();
   for (int e = tid; e <= E; e += kRemapThreads) s_off[e] = g_inst_off[e];
   for (int r = tid; r <= R; r += kRemapThreads) rbase[r] = g_rank_base[r];
   for (int p = tid; p < inst_cap; p += kRemapThreads) {
@@ -239,13 +248,6 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
     if (p + 1 < inst_cap) i_dbase[p + 1] = cum;  // cum_prev of the next entry
     if (p == 0) i_dbase[0] = 0;
   }
-  int el_inc = n_own;                            // inclusive scan of n_own over experts
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int y = __shfl_up_sync(kFullMask, el_inc, o);
-    if (lane >= o) el_inc += y;
-  }
-  if (lane == 31) wtot[warp] = el_inc;
   __syncthreads();
   if (tid < E) {
     base0[tid] = b0_own;
@@ -339,17 +341,28 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
 template <typename GateT>
 static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& p,
                            int32_t* out_replica, int32_t* out_rank, int32_t* out_offset,
-                           GateT* out_gate, void* ws, cudaStream_t s) {
+                           GateT* out_gate, void* ws, cudaStream_t s, bool pdl) {
   const uep_config& g = c->cfg;
   const int inst_cap = g.E + g.R * g.n_slot;
   const bool stage = gate != nullptr;
   const size_t smem = lookup_smem_bytes(c->E_pad, g.R, inst_cap, stage, sizeof(GateT));
   auto k = stage ? lookup_kernel<GateT, true> : lookup_kernel<GateT, false>;
-  k<<<c->r_chunks, kRemapThreads, smem, s>>>(
-      ws_packed(c, ws), gate, c->S, g.E, c->E_pad, g.R, inst_cap, c->r_chunk_len, ws_prefix(c, ws),
-      p.inst_off, p.inst_rank, p.inst_cum, p.inst_base, p.rank_base, out_replica, out_rank,
-      out_offset, out_gate);
-  UEP_CUDA_TRY(cudaGetLastError());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(c->r_chunks);
+  cfg.blockDim = dim3(kRemapThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl ? 1 : 0;
+  UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, k, (const int32_t*)ws_packed(c, ws), gate, c->S, g.E, c->E_pad,
+                                  g.R, inst_cap, c->r_chunk_len, (const int32_t*)ws_prefix(c, ws),
+                                  (const int32_t*)p.inst_off, (const int32_t*)p.inst_rank,
+                                  (const int32_t*)p.inst_cum, (const int32_t*)p.inst_base,
+                                  (const int32_t*)p.rank_base, out_replica, out_rank, out_offset,
+                                  out_gate));
   return UEP_OK;
 }
 
@@ -365,13 +378,14 @@ int init_remap_kernels() {
 }
 
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& p, int32_t* out_replica,
-                  int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s) {
+                  int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
+                  bool pdl) {
   if (c->S == 0) return UEP_OK;
   if (c->cfg.gate_dtype == UEP_GATE_BF16 && gate)
     return launch_lookup_t<uint16_t>(c, static_cast<const uint16_t*>(gate), p, out_replica, out_rank,
-                                     out_offset, static_cast<uint16_t*>(out_gate), ws, s);
+                                     out_offset, static_cast<uint16_t*>(out_gate), ws, s, pdl);
   return launch_lookup_t<uint32_t>(c, static_cast<const uint32_t*>(gate), p, out_replica, out_rank,
-                                   out_offset, static_cast<uint32_t*>(out_gate), ws, s);
+                                   out_offset, static_cast<uint32_t*>(out_gate), ws, s, pdl);
 }
 
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& p,
@@ -379,7 +393,7 @@ int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_p
                  void* ws, cudaStream_t s) {
   int rc = launch_rank(c, ids, ws, s);
   if (rc != UEP_OK) return rc;
-  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s);
+  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s, false);
 }
 
 }  // namespace uep

@@ -336,7 +336,9 @@ int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
   UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
   rc = launch_rank(c, topk_ids, ws, c->side);
   UEP_CUDA_TRY(cudaEventRecord(c->ev_rank, c->side));
-  if (rc2 == UEP_OK) rc2 = uep_plan(ctx, expert_count, plan, ws, stream);
+  // planner and lookup are launched programmatically dependent on their predecessor: their
+  // prologues (static layout; packed ranks, gates, prefix rows) overlap it
+  if (rc2 == UEP_OK) rc2 = launch_plan(c, expert_count, *plan, s, /*pdl=*/true);
   const bool do_pack = n_tensors > 0 && c->cfg.n_slot > 0;
   if (do_pack && rc2 == UEP_OK) {   // pack depends only on the plan and overlaps the lookup (Eq. 1)
     UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
@@ -347,7 +349,7 @@ int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
   UEP_CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
   UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_rank, 0));          // join the rank kernel
   if (rc == UEP_OK && rc2 == UEP_OK)
-    rc2 = launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s);
+    rc2 = launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s, /*pdl=*/true);
   UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_join, 0));          // join the side stream (pack)
   return rc != UEP_OK ? rc : rc2;
 }

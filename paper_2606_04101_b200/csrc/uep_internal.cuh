@@ -56,12 +56,14 @@ struct PackArgs {
 int set_cuda_error(cudaError_t e);
 
 int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s);
-int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s);
+int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
+                bool pdl = false);
 // uep_remap = launch_rank (plan-independent: stable rank of every slot inside its chunk, packed
 // with the expert id into the workspace) + launch_lookup (plan-dependent: cumulative-quota lookup).
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s);
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& plan, int32_t* out_replica,
-                  int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s);
+                  int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
+                  bool pdl = false);
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& plan,
                  int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
                  void* ws, cudaStream_t s);
@@ -79,6 +81,13 @@ int init_hist_kernels();
 // (kColPartInts ints of shared memory), result in `out` (shared).  Ends with a __syncthreads().
 constexpr int kColPartInts = 4096;
 #ifdef __CUDACC__
+// Programmatic dependent launch (sm_90+).  pdl_trigger: the next kernel in the stream, if it was
+// launched with programmatic stream serialization, may start now (its prologue overlaps this
+// kernel).  pdl_wait: block until the preceding kernel has completed and its writes are visible;
+// a no-op when the kernel was launched normally.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ void column_sums(const int32_t* __restrict__ table, int n_rows, int E_pad,
                                             int* part, int* out) {
   const int tid = threadIdx.x;
