@@ -109,12 +109,12 @@ __device__ __forceinline__ bool probe(const PlanSmem& sm, const int tau, const i
                                       const int n_slot, const int u_min, const bool strict,
                                       const int lane, int4* __restrict__ log, int& n_log) {
   unsigned key[RPL];
-  int used[RPL];
+  int left[RPL];                               // free redundant slots of the lane's ranks
 #pragma unroll
   for (int i = 0; i < RPL; ++i) {
     const int t = lane + 32 * i;
     const int slk = (t < R) ? max(tau - sm.ell[t], 0) : 0;          // line 6
-    used[i] = 0;
+    left[i] = n_slot;
     key[i] = (slk > 0 && n_slot > 0) ? (((unsigned)slk << 8) | (unsigned)(255 - t)) : 0u;
   }
   const int brk = strict ? 1 : u_min;        // a rank is drained when exc < brk (S8)
@@ -135,13 +135,16 @@ __device__ __forceinline__ bool probe(const PlanSmem& sm, const int tau, const i
         const int s = (int)(km >> 8);
         const int d = min(exc, min(s, cap));                        // line 15
         if (d < u_min) { dead = s < u_min; break; }                 // line 16 (or line 13: T empty)
+        // owner lane (lines 17-19): its key becomes key - delta << 8, or 0 when the rank is full
+        // (no slack or no slot left)
+        const unsigned nk = (s > d) ? km - ((unsigned)d << 8) : 0u;
         int slot = 0;
 #pragma unroll
         for (int i = 0; i < RPL; ++i) {
-          if (key[i] == km) {                                       // owner lane: lines 17-19
-            slot = used[i];
-            used[i] += 1;
-            key[i] = (s > d && used[i] < n_slot) ? km - ((unsigned)d << 8) : 0u;
+          if (key[i] == km) {
+            if (LOG) slot = n_slot - left[i];
+            left[i] -= 1;
+            key[i] = (left[i] > 0) ? nk : 0u;
           }
         }
         if (LOG) {
@@ -151,7 +154,7 @@ __device__ __forceinline__ bool probe(const PlanSmem& sm, const int tau, const i
         ++nl;
         exc -= d;
         cap -= d;
-      } while (exc > 0 && cap > 0);
+      } while (min(exc, cap) > 0);
       if (dead) break;
     }
     // line 20 per rank (S21 early exit): strict needs exc == 0, tolerant exc < u_min (S8)
