@@ -45,6 +45,9 @@ def parse_args():
     ap.add_argument("--workload", default="dsv3_prefill",
                     choices=["tiny", "glm_air", "dsv3_prefill", "dsv3_train"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--size-sweep", action="store_true",
+                    help="instead of the bench line: stage times and roofline fractions at E=256, k=8, "
+                         "R=64 over S = 256 Ki .. 16 Mi slots, one JSON line per size (DESIGN.md §7)")
     ap.add_argument("--state-scale", type=float, default=1.0,
                     help="shrink bytes per expert (debug only; the line then says so)")
     return ap.parse_args()
@@ -523,8 +526,60 @@ def run_reference(args):
             "gpu_launches": 0}
 
 
+def run_size_sweep(args):
+    """Stage times vs problem size (same kernels, same launch rules as the library picks): shows
+    which part of a stage time is fixed (launch ramp, one memory round trip, tails) and which part
+    scales with bytes.  Each stage is graph-captured over 4-8 distinct instances, CUDA events."""
+    import torch
+    from paper_2606_04101_b200 import binding, synth
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device; no CPU fallback"
+    dev = torch.device("cuda", torch.cuda.current_device())
+    peak_gbs, peak_src = measured_peaks()
+    k, E, R, ns = 8, 256, 64, 2
+    for T in (1 << 15, 1 << 16, 1 << 17, 1 << 18, 1 << 19, 1 << 20, (1 << 21) - 8):
+        S = T * k
+        um = synth.stress_u_min(S, R)
+        n_inst = 8 if S <= (1 << 22) else 4
+        ctx = binding.Context(T, k, E, R, ns, um, device=dev)
+        ids = [synth.zipf_topk_ids(T, k, E, 1.0, 100 + i, device=dev) for i in range(n_inst)]
+        gates = [synth.gates_uniform_renorm(T, k, i, device=dev) for i in range(n_inst)]
+        ws = [ctx.new_workspace() for _ in range(n_inst)]
+        plans = [ctx.new_plan() for _ in range(n_inst)]
+        cnt = [torch.zeros(E, dtype=torch.int32, device=dev) for _ in range(n_inst)]
+        outs = [ctx.new_outputs(gates[i]) for i in range(n_inst)]
+        stream = torch.cuda.Stream(dev)
+        torch.cuda.synchronize(dev)                 # workspace init ran on the default stream
+        stages = {
+            "histogram": lambda i: ctx.uep_histogram(ids[i], cnt[i], ws[i]),
+            "plan": lambda i: ctx.uep_plan(cnt[i], plans[i], ws[i]),
+            "remap_rank": lambda i: ctx.uep_remap_rank(ids[i], ws[i]),
+            "remap_lookup": lambda i: ctx.uep_remap_lookup(gates[i], plans[i], *outs[i], ws[i]),
+            "chain": lambda i: ctx.uep_balance(ids[i], gates[i], cnt[i], plans[i], *outs[i], [], [], ws[i]),
+        }
+        with torch.cuda.stream(stream):
+            for i in range(n_inst):
+                stages["chain"](i)
+        stream.synchronize()
+        us = {}
+        for name, fn in stages.items():
+            g = capture([lambda i=i, fn=fn: fn(i) for i in range(n_inst)], stream)
+            ms, _ = time_graph(g, stream, 5)
+            us[name] = ms * 1e3 / n_inst
+        frac = lambda nbytes, t: round(nbytes / (t * 1e-6) / 1e9 / peak_gbs, 3)
+        print(json.dumps({"slots": S, "instances": n_inst, "stages_us": {n: round(v, 2) for n, v in us.items()},
+                          "frac_of_peak": {"hist_kernel (4 B/slot)": frac(4 * S, us["histogram"]),
+                                           "rank+prefix (8 B/slot)": frac(8 * S, us["remap_rank"]),
+                                           "lookup_kernel (24 B/slot)": frac(24 * S, us["remap_lookup"])},
+                          "peak_gbs": peak_gbs, "peak_source": peak_src}), flush=True)
+        del ctx, ids, gates, ws, plans, cnt, outs
+        torch.cuda.synchronize(dev)
+
+
 def main():
     args = parse_args()
+    if args.size_sweep:
+        run_size_sweep(args)
+        return
     if args.impl == "reference":
         out = run_reference(args)
         if out is not None:
