@@ -318,6 +318,13 @@ def run_uep(args):
     n_pack = min(n_inst, 8)
     g_pack = capture([lambda i=i: rig.pack(i) for i in range(n_pack)], stream)
     pack_ms, _ = time_graph(g_pack, stream, 3, warm=1)
+    # NEXT-4: all instances' planners in ONE launch, one cluster per instance
+    import torch as _t
+    counts_all = _t.stack(rig.counts).contiguous()
+    bplan = rig.ctx.new_plan(batch=n_inst)
+    _t.cuda.synchronize(device)
+    g_bplan = capture([lambda: rig.ctx.uep_plan_batched(n_inst, counts_all, bplan)], stream)
+    bplan_ms, _ = time_graph(g_bplan, stream, reps)
     clocks = sampler.stop()
     chain_ms = barrier_and_max(world, chain_ms, device)
     # whole-job aggregate: `world` ranks each planned n_inst layers in chain_ms (max over ranks)
@@ -386,6 +393,9 @@ def run_uep(args):
                     "n_replicas_mean": round(statistics.mean(n_rep), 1),
                     "max_fanout_max": max(int(s[binding.SC_MAX_FANOUT]) for s in sc),
                     "n_probes_mean": round(statistics.mean(int(s[binding.SC_N_PROBES]) for s in sc), 1)},
+        "batched_plan": {"instances": n_inst, "us_total": round(bplan_ms * 1e3, 2),
+                         "us_per_layer": round(bplan_ms * 1e3 / n_inst, 3),
+                         "note": "uep_plan_batched: one launch, one 8-CTA cluster per instance"},
         "roofline": {k: r_pack[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")},
         "rooflines": rooflines,
         "gpu_launches": 6 * K,

@@ -145,6 +145,17 @@ int uep_histogram(const uep_ctx* ctx, const int32_t* topk_ids, int32_t* expert_c
 int uep_plan(const uep_ctx* ctx, const int32_t* expert_count, const uep_plan_out* plan, void* ws,
              void* stream);
 
+/* Batched SolveReplication: n_inst independent instances (layers x microbatches whose loads are
+ * known together, e.g. replay or simulation as in Fig. 15) in ONE launch, one
+ * thread-block cluster per instance, all clusters concurrent on different SMs.
+ *   expert_count  DEVICE int32 [n_inst][E]
+ *   plan0         HOST struct of DEVICE pointers to the arrays of instance 0; every array must be
+ *                 allocated n_inst times its uep_plan_sizes element count, instance b starting
+ *                 b * count elements after instance 0 (U may be NULL).
+ * Each instance's result is bit-identical to uep_plan on its counts. */
+int uep_plan_batched(const uep_ctx* ctx, int32_t n_inst, const int32_t* expert_count,
+                     const uep_plan_out* plan0, void* stream);
+
 /* Token assignment (§5.2): slot s of expert e with global stable rank j goes to the first
  * instance whose cumulative quota exceeds j.
  *   gate          DEVICE [T,k] of cfg.gate_dtype, or NULL

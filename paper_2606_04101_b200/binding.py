@@ -23,7 +23,7 @@ SC_TAU, SC_N_REPLICAS, SC_MAX_LOAD, SC_MAX_FANOUT, SC_N_PROBES, SC_N_INVALID, SC
     SC_TAU_HI0, SC_N_GROUPS = range(9)
 
 EXPORTS = ["uep_create", "uep_destroy", "uep_workspace_bytes", "uep_workspace_init",
-           "uep_plan_bytes", "uep_histogram", "uep_plan", "uep_remap", "uep_remap_rank",
+           "uep_plan_bytes", "uep_histogram", "uep_plan", "uep_plan_batched", "uep_remap", "uep_remap_rank",
            "uep_remap_lookup", "uep_pack", "uep_balance",
            "uep_balance_host", "uep_strerror", "uep_last_cuda_error", "uep_get_launch_info"]
 
@@ -120,13 +120,17 @@ class Plan:
     scalars: torch.Tensor
     U: torch.Tensor | None
     c: _PlanOut = field(default=None, repr=False)
+    batch: int = 1
 
-    def host(self):
-        """Host (numpy) copy with the attribute names the checkers use."""
+    def host(self, b: int = 0):
+        """Host (numpy) copy of instance b with the attribute names the checkers use."""
         import types
         h = types.SimpleNamespace(E=self.E, R=self.R, n_slot=self.n_slot, M=self.M, P=self.P)
         for n in _PLAN_FIELDS:
             t = getattr(self, n)
+            if t is not None:
+                per = t.numel() // self.batch
+                t = t[b * per:(b + 1) * per]
             setattr(h, n, None if t is None else t.cpu().numpy())
         h.slot_expert = h.slot_expert[:self.R * self.n_slot].reshape(self.R, self.n_slot)
         h.phys_count = h.phys_count.reshape(self.R, self.P)
@@ -181,13 +185,16 @@ class Context:
         _check(lib().uep_workspace_init(self._h, _ptr(ws), _stream(stream)))
         return ws
 
-    def new_plan(self, dense_U=False) -> Plan:
+    def new_plan(self, dense_U=False, batch: int = 1) -> Plan:
+        """Plan arrays for `batch` instances (uep_plan_batched layout: instance b of every array
+        starts b * its element count after instance 0)."""
         sz = self.sizes
-        z = lambda n: torch.zeros(max(int(n), 1), dtype=torch.int32, device=self.device)
+        z = lambda n: torch.zeros(max(int(n), 1) * batch, dtype=torch.int32, device=self.device)
         p = Plan(self.E, self.R, self.n_slot, sz.M, sz.P, z(sz.slot_expert), z(sz.inst_off),
                  z(sz.inst_cap), z(sz.inst_cap), z(sz.inst_cap), z(sz.inst_cap), z(sz.phys), z(sz.phys),
                  z(sz.rank_load), z(sz.rank_base), z(sz.scalars), z(sz.U) if dense_U else None)
         p.c = _PlanOut(*[_ptr(getattr(p, n)).value or 0 for n in _PLAN_FIELDS])
+        p.batch = batch
         return p
 
     def new_outputs(self, gate: torch.Tensor | None = None):
@@ -209,6 +216,11 @@ class Context:
         _check(lib().uep_remap(self._h, _ptr(topk_ids), _ptr(gate), ctypes.byref(plan.c),
                                _ptr(out_replica), _ptr(out_rank), _ptr(out_offset), _ptr(out_gate),
                                _ptr(ws), _stream(stream)))
+
+    def uep_plan_batched(self, n_inst: int, expert_count, plan: Plan, stream=None):
+        assert plan.batch >= n_inst and expert_count.numel() >= n_inst * self.E
+        _check(lib().uep_plan_batched(self._h, int(n_inst), _ptr(expert_count), ctypes.byref(plan.c),
+                                      _stream(stream)))
 
     def uep_remap_rank(self, topk_ids, ws, stream=None):
         _check(lib().uep_remap_rank(self._h, _ptr(topk_ids), _ptr(ws), _stream(stream)))

@@ -177,6 +177,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
             int log_cap, int levels) {
   cg::cluster_group cluster = cg::this_cluster();
   const int csize = (int)cluster.num_blocks(), crank = (int)cluster.block_rank();
+  // batched solve (uep_plan_batched): cluster b solves instance b; every array of instance b
+  // starts b * (its element count) after instance 0's
+  const int batch_b = (int)blockIdx.x / csize;
+  expert_count += (size_t)batch_b * E;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   PlanSmem& sm = *reinterpret_cast<PlanSmem*>(smem_raw);
   // accept logs: n_bufs buffers of log_cap entries {e, t, slot, delta}; buffer 0 serves the
@@ -365,6 +369,23 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   const int log_node = sm.log_buf;
   const int owner = log_node < 0 ? 0 : log_node % csize;
   if (crank != owner) return;
+  uep_plan_out o = out;            // this instance's arrays (offset only here: the probes above
+  {                                // must not carry eleven pointers in registers)
+    const size_t bb = (size_t)batch_b;
+    const int n_inst_cap = E + R * n_slot;
+    o.slot_expert += bb * max(1, R * n_slot);
+    o.inst_off += bb * (E + 1);
+    o.inst_rank += bb * n_inst_cap;
+    o.inst_phys += bb * n_inst_cap;
+    o.inst_cum += bb * n_inst_cap;
+    o.inst_base += bb * n_inst_cap;
+    o.phys_count += bb * R * P;
+    o.phys_base += bb * R * P;
+    o.rank_load += bb * R;
+    o.rank_base += bb * (R + 1);
+    o.scalars += bb * UEP_N_SCALARS;
+    if (o.U) o.U += bb * E * R;
+  }
   const int log_buf = log_node < 0 ? 0 : 1 + log_node / csize;
   if (warp == 0 && sm.n_probes > 0 && log_node < 0) {
     int nl;
@@ -375,10 +396,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   if (tid < E) { sm.u_main[tid] = sm.lam[tid]; sm.n_rep[tid] = 0; sm.first[tid] = 0x7fffffff; }
   const int RP = R * P;
   const bool pc_in_smem = RP <= kPcSmem;
-  int* pc = pc_in_smem ? sm.pc : out.phys_count;
+  int* pc = pc_in_smem ? sm.pc : o.phys_count;
   for (int i = tid; i < RP; i += kPlanThreads) pc[i] = 0;
-  for (int i = tid; i < R * n_slot; i += kPlanThreads) out.slot_expert[i] = -1;
-  if (out.U) for (int i = tid; i < E * R; i += kPlanThreads) out.U[i] = 0;
+  for (int i = tid; i < R * n_slot; i += kPlanThreads) o.slot_expert[i] = -1;
+  if (o.U) for (int i = tid; i < E * R; i += kPlanThreads) o.U[i] = 0;
   __syncthreads();
   const int n_log = sm.n_log;
 #ifdef UEP_PLAN_TIMING
@@ -404,15 +425,15 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (tid < n_log) sm.dscan[tid] = ds;
   }
   __syncthreads();
-  if (tid <= E) out.inst_off[tid] = sm.inst_off[tid];
+  if (tid <= E) o.inst_off[tid] = sm.inst_off[tid];
   int fan = 0;
   if (tid < E) {
     const int pos = sm.inst_off[tid], h = sm.home[tid], um = sm.u_main[tid];
-    out.inst_rank[pos] = h;
-    out.inst_phys[pos] = sm.main_phys[tid];
-    out.inst_cum[pos] = um;
+    o.inst_rank[pos] = h;
+    o.inst_phys[pos] = sm.main_phys[tid];
+    o.inst_cum[pos] = um;
     pc[h * P + sm.main_phys[tid]] = um;
-    if (out.U) out.U[tid * R + h] = um;
+    if (o.U) o.U[tid * R + h] = um;
     fan = 1 + sm.n_rep[tid];
   }
   if (tid < n_log) {
@@ -420,15 +441,15 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     const int f = sm.first[e];
     const int pos = sm.inst_off[e] + 1 + (tid - f);                 // S11: acceptance order
     const int before = (f > 0) ? sm.dscan[f - 1] : 0;
-    out.inst_rank[pos] = t;
-    out.inst_phys[pos] = M + sl;
-    out.inst_cum[pos] = sm.u_main[e] + sm.dscan[tid] - before;
-    out.slot_expert[t * n_slot + sl] = e;                           // X
+    o.inst_rank[pos] = t;
+    o.inst_phys[pos] = M + sl;
+    o.inst_cum[pos] = sm.u_main[e] + sm.dscan[tid] - before;
+    o.slot_expert[t * n_slot + sl] = e;                           // X
     pc[t * P + M + sl] = d;
-    if (out.U) out.U[e * R + t] = d;
+    if (o.U) o.U[e * R + t] = d;
   }
   for (int i = E + n_log + tid; i < E + R * n_slot; i += kPlanThreads) {   // unused CSR tail
-    out.inst_rank[i] = -1; out.inst_phys[i] = -1; out.inst_cum[i] = 0; out.inst_base[i] = 0;
+    o.inst_rank[i] = -1; o.inst_phys[i] = -1; o.inst_cum[i] = 0; o.inst_base[i] = 0;
   }
   // max fan-out and number of replicated experts
   {
@@ -442,20 +463,20 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   if (tid < R) {
     for (int q = 0; q < P; ++q) {
       const int cnt = pc[tid * P + q];
-      out.phys_base[tid * P + q] = load;
-      if (pc_in_smem) { out.phys_count[tid * P + q] = cnt; pc[tid * P + q] = load; }
+      o.phys_base[tid * P + q] = load;
+      if (pc_in_smem) { o.phys_count[tid * P + q] = cnt; pc[tid * P + q] = load; }
       load += cnt;
     }
-    out.rank_load[tid] = load;
+    o.rank_load[tid] = load;
   }
   __syncthreads();
   // inst_base: offset of each instance's first token in its rank's receive buffer (S13)
   {
-    const int* pb = pc_in_smem ? pc : out.phys_base;      // bases (global ones are CTA-visible now)
-    if (tid < E) out.inst_base[sm.inst_off[tid]] = pb[sm.home[tid] * P + sm.main_phys[tid]];
+    const int* pb = pc_in_smem ? pc : o.phys_base;      // bases (global ones are CTA-visible now)
+    if (tid < E) o.inst_base[sm.inst_off[tid]] = pb[sm.home[tid] * P + sm.main_phys[tid]];
     if (tid < n_log) {
       const int e = lg[tid].x;
-      out.inst_base[sm.inst_off[e] + 1 + (tid - sm.first[e])] = pb[lg[tid].y * P + M + lg[tid].z];
+      o.inst_base[sm.inst_off[e] + 1 + (tid - sm.first[e])] = pb[lg[tid].y * P + M + lg[tid].z];
     }
   }
   int max_fan = 0, n_groups = 0;
@@ -463,8 +484,8 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   __syncthreads();
   {
     const int inc = block_incl_scan(load, sm.warp_tmp);
-    if (tid < R) out.rank_base[tid] = inc - load;
-    if (tid == R - 1) out.rank_base[R] = inc;
+    if (tid < R) o.rank_base[tid] = inc - load;
+    if (tid == R - 1) o.rank_base[R] = inc;
     const int mx = __reduce_max_sync(kFull, load);
     __syncthreads();
     if (lane == 0) sm.feas[warp] = mx;
@@ -473,24 +494,24 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   if (tid == 0) {
     int max_load = 0;
     for (int w = 0; w < 32; ++w) max_load = max(max_load, sm.feas[w]);
-    out.scalars[UEP_SC_TAU] = tau;
-    out.scalars[UEP_SC_N_REPLICAS] = n_log;
-    out.scalars[UEP_SC_MAX_LOAD] = max_load;
-    out.scalars[UEP_SC_MAX_FANOUT] = max_fan;
-    out.scalars[UEP_SC_N_PROBES] = sm.n_probes;
-    out.scalars[UEP_SC_N_INVALID] = (int)((long long)S_total - sm.s_valid);
-    out.scalars[UEP_SC_TAU_LO0] = tau_lo0;
-    out.scalars[UEP_SC_TAU_HI0] = tau_hi0;
-    out.scalars[UEP_SC_N_GROUPS] = n_groups;
-    for (int i = UEP_SC_N_GROUPS + 1; i < UEP_N_SCALARS; ++i) out.scalars[i] = 0;
+    o.scalars[UEP_SC_TAU] = tau;
+    o.scalars[UEP_SC_N_REPLICAS] = n_log;
+    o.scalars[UEP_SC_MAX_LOAD] = max_load;
+    o.scalars[UEP_SC_MAX_FANOUT] = max_fan;
+    o.scalars[UEP_SC_N_PROBES] = sm.n_probes;
+    o.scalars[UEP_SC_N_INVALID] = (int)((long long)S_total - sm.s_valid);
+    o.scalars[UEP_SC_TAU_LO0] = tau_lo0;
+    o.scalars[UEP_SC_TAU_HI0] = tau_hi0;
+    o.scalars[UEP_SC_N_GROUPS] = n_groups;
+    for (int i = UEP_SC_N_GROUPS + 1; i < UEP_N_SCALARS; ++i) o.scalars[i] = 0;
 #ifdef UEP_PLAN_TIMING   // developer probe: cycles of setup / bisection / final probe / emit
-    out.scalars[9] = sm.tmax[0];
-    out.scalars[10] = sm.tmax[1];
-    out.scalars[11] = sm.tmax[2];
-    out.scalars[12] = (int)(t_setup - t_start);
-    out.scalars[13] = (int)(t_bisect - t_setup);
-    out.scalars[14] = (int)(t_final - t_bisect);
-    out.scalars[15] = (int)(clock64() - t_final);
+    o.scalars[9] = sm.tmax[0];
+    o.scalars[10] = sm.tmax[1];
+    o.scalars[11] = sm.tmax[2];
+    o.scalars[12] = (int)(t_setup - t_start);
+    o.scalars[13] = (int)(t_bisect - t_setup);
+    o.scalars[14] = (int)(t_final - t_bisect);
+    o.scalars[15] = (int)(clock64() - t_final);
 #endif
   }
 }
@@ -499,7 +520,7 @@ constexpr size_t kLogBudget = 128 * 1024;     // shared memory for the accept lo
 
 template <int RPL>
 static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out& plan,
-                         cudaStream_t s, bool pdl) {
+                         cudaStream_t s, bool pdl, int n_inst) {
   const uep_config& g = c->cfg;
   const int levels = 6;                                        // 63 nodes over kPlanCluster CTAs
   const int cluster = c->plan_cluster;
@@ -508,7 +529,7 @@ static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out&
   const int n_bufs = ((size_t)(1 + warps) * log_cap * sizeof(int4) <= kLogBudget) ? 1 + warps : 1;
   const size_t smem = ((sizeof(PlanSmem) + 15) & ~(size_t)15) + (size_t)n_bufs * log_cap * sizeof(int4);
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(cluster);
+  cfg.gridDim = dim3(cluster * n_inst);
   cfg.blockDim = dim3(kPlanThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = s;
@@ -531,12 +552,13 @@ static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out&
 }
 
 int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
-                bool pdl) {
+                bool pdl, int n_inst) {
   const int R = c->cfg.R;
-  if (R <= 32) return launch_plan_t<1>(c, count, plan, s, pdl);
-  if (R <= 64) return launch_plan_t<2>(c, count, plan, s, pdl);
-  if (R <= 128) return launch_plan_t<4>(c, count, plan, s, pdl);
-  return launch_plan_t<8>(c, count, plan, s, pdl);
+  if (n_inst <= 0) return UEP_OK;
+  if (R <= 32) return launch_plan_t<1>(c, count, plan, s, pdl, n_inst);
+  if (R <= 64) return launch_plan_t<2>(c, count, plan, s, pdl, n_inst);
+  if (R <= 128) return launch_plan_t<4>(c, count, plan, s, pdl, n_inst);
+  return launch_plan_t<8>(c, count, plan, s, pdl, n_inst);
 }
 
 template <int RPL>

@@ -252,6 +252,17 @@ int uep_remap(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
                       static_cast<cudaStream_t>(stream));
 }
 
+int uep_plan_batched(const uep_ctx* ctx, int32_t n_inst, const int32_t* expert_count,
+                     const uep_plan_out* plan0, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || n_inst < 0 || n_inst > 65535 / 16) return UEP_ERR_INVALID_ARG;
+  if (n_inst == 0) return UEP_OK;
+  if (!expert_count || !aligned16(expert_count)) return UEP_ERR_INVALID_ARG;
+  int rc = check_plan_ptrs(c, plan0);
+  if (rc != UEP_OK) return rc;
+  return launch_plan(c, expert_count, *plan0, static_cast<cudaStream_t>(stream), false, n_inst);
+}
+
 static int check_remap_outputs(const Ctx* c, const void* gate, const uep_plan_out* plan,
                                const int32_t* out_replica, const int32_t* out_rank,
                                const int32_t* out_offset, const void* out_gate, const void* ws) {

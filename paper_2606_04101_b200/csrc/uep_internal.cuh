@@ -57,7 +57,7 @@ int set_cuda_error(cudaError_t e);
 
 int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s);
 int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
-                bool pdl = false);
+                bool pdl = false, int n_inst = 1);
 // uep_remap = launch_rank (plan-independent: stable rank of every slot inside its chunk, packed
 // with the expert id into the workspace) + launch_lookup (plan-dependent: cumulative-quota lookup).
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s);

@@ -356,3 +356,29 @@ def test_odd_shapes_parity(T, k, E, R, n_slot):
     o = oracle_chain(ids, gate, E, R, n_slot, um)
     assert_parity(g, o, ids, gate)
     ck.check_remap(ids.numpy(), g["plan"], g["rep"], g["rnk"], g["off"])
+
+
+def test_batched_planning_matches_single_and_oracle():
+    """uep_plan_batched: one launch, one cluster per instance; each instance bit-identical to the
+    oracle (and hence to uep_plan) — including a balanced instance (identity plan) and the
+    all-to-one-expert instance."""
+    E, R, ns, um, T, k = 128, 32, 2, 512, 32768, 8
+    ctx = binding.Context(T, k, E, R, ns, um)
+    lams = []
+    for b, s in enumerate((0.0, 0.6, 1.0, 1.4, 2.0)):
+        ids = synth.zipf_topk_ids(T, k, E, s, 40 + b)
+        lams.append(np.bincount(ids.numpy().ravel(), minlength=E).astype(np.int32))
+    one = np.zeros(E, np.int32); one[77] = T * k
+    lams.append(one)
+    lams.append(np.full(E, T * k // E, np.int32))          # perfectly balanced
+    n = len(lams)
+    counts = torch.from_numpy(np.stack(lams)).to(DEV)
+    plan = ctx.new_plan(dense_U=True, batch=n)
+    ctx.uep_plan_batched(n, counts, plan)
+    torch.cuda.synchronize()
+    for b in range(n):
+        hp = plan.host(b)
+        op = oracle.plan(lams[b], R, ns, um, S_total=T * k)
+        for name in PLAN_ARRAYS:
+            assert np.array_equal(np.asarray(getattr(hp, name)).ravel(),
+                                  np.asarray(getattr(op, name)).ravel()), (b, name)
