@@ -20,7 +20,7 @@
 //     (e,t) leaves slk_t = 0 or ends e's loop, and h(e) is overloaded hence has no slack);
 //   * the probes of the LAST round log their accepted transfers, so the CTA that holds the log
 //     of the final tau's probe (= U~ of the last feasible probe, S10) emits X, the CSR
-//     cumulative quotas and the receive layout with all its 1024 threads; otherwise one logged
+//     cumulative quotas and the receive layout with all its threads; otherwise one logged
 //     probe at the final tau is run (deterministic, so it reproduces that probe).
 #include <algorithm>
 #include <cstdlib>
@@ -33,6 +33,9 @@ namespace cg = cooperative_groups;
 
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kMaxLog = UEP_MAX_R * UEP_MAX_NSLOT;      // 1024 accepted transfers at most
+constexpr int kPlanWarps = kPlanThreads / 32;
+constexpr int kLogPer = kMaxLog / kPlanThreads;        // log entries handled per thread when emitting
+static_assert(kLogPer * kPlanThreads == kMaxLog && UEP_MAX_E <= kPlanThreads && UEP_MAX_R < kPlanThreads, "plan emit");
 // CTAs (SMs) sharing one solve, so that the 63 probes of a round spread over many schedulers:
 // 8 CTAs = two probes per scheduler.  Measured on B200 (DSV3 shape): 4 / 8 / 16 CTAs give
 // 22.9 / 20.6 / 20.4 us of bisection, i.e. from 8 up the probes are bound by the latency of their
@@ -81,7 +84,7 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
   return v;
 }
 
-// Block-wide inclusive scan of one value per thread (1024 threads). tmp: 32 ints of smem.
+// Block-wide inclusive scan of one value per thread (kPlanThreads). tmp: 32 ints of smem.
 __device__ __forceinline__ int block_incl_scan(int v, int* tmp) {
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   int s = warp_incl_scan(v, lane);
@@ -222,7 +225,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   if (tid == 0) {
     long long sv = 0;
     int mx = 0;
-    for (int w = 0; w < 32; ++w) { sv += sm.warp_tmp[w]; mx = max(mx, sm.feas[w]); }
+    for (int w = 0; w < kPlanWarps; ++w) { sv += sm.warp_tmp[w]; mx = max(mx, sm.feas[w]); }
     sm.s_valid = sv;
     sm.max_ell = mx;
     // line 3 (S3): tau_lo = floor(beta * ceil(mean)), tau_hi = max l_r
@@ -236,20 +239,18 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
 #ifdef UEP_PLAN_TIMING
   const long long t_s1 = clock64();
 #endif
-  // rank order: position = number of ranks that come before (l desc, id asc); a warp per rank,
-  // by the upper half of the CTA, while the lower half orders the experts
-  if (warp >= 16) {
-    for (int r = warp - 16; r < R; r += 16) {
-      const int lr = sm.ell[r];
-      int cnt = 0;
-      for (int q = lane; q < R; q += 32) {
-        const int lq = sm.ell[q];
-        cnt += (lq > lr || (lq == lr && q < r)) ? 1 : 0;
-      }
-      cnt = __reduce_add_sync(kFull, cnt);
-      if (lane == 0) sm.order[cnt] = r;
+  // rank order: position = number of ranks that come before (l desc, id asc); a warp per rank
+  for (int r = warp; r < R; r += kPlanWarps) {
+    const int lr = sm.ell[r];
+    int cnt = 0;
+    for (int q = lane; q < R; q += 32) {
+      const int lq = sm.ell[q];
+      cnt += (lq > lr || (lq == lr && q < r)) ? 1 : 0;
     }
-  } else if (tid < E) {
+    cnt = __reduce_add_sync(kFull, cnt);
+    if (lane == 0) sm.order[cnt] = r;
+  }
+  if (tid < E) {
     // per-rank expert order: lambda desc, id asc; a thread per expert counts the experts of its
     // home rank that come before it; positions into u_main (temp)
     const int e = tid, h = sm.home[e], le = sm.lam[e];
@@ -407,11 +408,15 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
 #endif
 
   // ---- emit (line 22 "materialize U~ into X" + cumulative reroute metadata, §5.2) ---------
-  if (tid < n_log) {
-    const int e = lg[tid].x;
-    atomicSub(&sm.u_main[e], lg[tid].w);
-    atomicAdd(&sm.n_rep[e], 1);
-    atomicMin(&sm.first[e], tid);
+#pragma unroll
+  for (int j = 0; j < kLogPer; ++j) {
+    const int l = tid * kLogPer + j;
+    if (l < n_log) {
+      const int e = lg[l].x;
+      atomicSub(&sm.u_main[e], lg[l].w);
+      atomicAdd(&sm.n_rep[e], 1);
+      atomicMin(&sm.first[e], l);
+    }
   }
   __syncthreads();
   {
@@ -420,12 +425,23 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (tid < E) sm.inst_off[tid] = inc - v;
     if (tid == E - 1) sm.inst_off[E] = inc;
     __syncthreads();
-    const int d = (tid < n_log) ? lg[tid].w : 0;
-    const int ds = block_incl_scan(d, sm.warp_tmp);
-    if (tid < n_log) sm.dscan[tid] = ds;
+    int d[kLogPer], dsum = 0;                   // inclusive scan of delta over the log, kLogPer per thread
+#pragma unroll
+    for (int j = 0; j < kLogPer; ++j) {
+      const int l = tid * kLogPer + j;
+      d[j] = (l < n_log) ? lg[l].w : 0;
+      dsum += d[j];
+    }
+    int run = block_incl_scan(dsum, sm.warp_tmp) - dsum;
+#pragma unroll
+    for (int j = 0; j < kLogPer; ++j) {
+      const int l = tid * kLogPer + j;
+      run += d[j];
+      if (l < n_log) sm.dscan[l] = run;
+    }
   }
   __syncthreads();
-  if (tid <= E) o.inst_off[tid] = sm.inst_off[tid];
+  for (int i = tid; i <= E; i += kPlanThreads) o.inst_off[i] = sm.inst_off[i];
   int fan = 0;
   if (tid < E) {
     const int pos = sm.inst_off[tid], h = sm.home[tid], um = sm.u_main[tid];
@@ -436,17 +452,21 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (o.U) o.U[tid * R + h] = um;
     fan = 1 + sm.n_rep[tid];
   }
-  if (tid < n_log) {
-    const int e = lg[tid].x, t = lg[tid].y, sl = lg[tid].z, d = lg[tid].w;
-    const int f = sm.first[e];
-    const int pos = sm.inst_off[e] + 1 + (tid - f);                 // S11: acceptance order
-    const int before = (f > 0) ? sm.dscan[f - 1] : 0;
-    o.inst_rank[pos] = t;
-    o.inst_phys[pos] = M + sl;
-    o.inst_cum[pos] = sm.u_main[e] + sm.dscan[tid] - before;
-    o.slot_expert[t * n_slot + sl] = e;                           // X
-    pc[t * P + M + sl] = d;
-    if (o.U) o.U[e * R + t] = d;
+#pragma unroll
+  for (int j = 0; j < kLogPer; ++j) {
+    const int l = tid * kLogPer + j;
+    if (l < n_log) {
+      const int e = lg[l].x, t = lg[l].y, sl = lg[l].z, dd = lg[l].w;
+      const int f = sm.first[e];
+      const int pos = sm.inst_off[e] + 1 + (l - f);                 // S11: acceptance order
+      const int before = (f > 0) ? sm.dscan[f - 1] : 0;
+      o.inst_rank[pos] = t;
+      o.inst_phys[pos] = M + sl;
+      o.inst_cum[pos] = sm.u_main[e] + sm.dscan[l] - before;
+      o.slot_expert[t * n_slot + sl] = e;                           // X
+      pc[t * P + M + sl] = dd;
+      if (o.U) o.U[e * R + t] = dd;
+    }
   }
   for (int i = E + n_log + tid; i < E + R * n_slot; i += kPlanThreads) {   // unused CSR tail
     o.inst_rank[i] = -1; o.inst_phys[i] = -1; o.inst_cum[i] = 0; o.inst_base[i] = 0;
@@ -474,13 +494,17 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   {
     const int* pb = pc_in_smem ? pc : o.phys_base;      // bases (global ones are CTA-visible now)
     if (tid < E) o.inst_base[sm.inst_off[tid]] = pb[sm.home[tid] * P + sm.main_phys[tid]];
-    if (tid < n_log) {
-      const int e = lg[tid].x;
-      o.inst_base[sm.inst_off[e] + 1 + (tid - sm.first[e])] = pb[lg[tid].y * P + M + lg[tid].z];
+#pragma unroll
+    for (int j = 0; j < kLogPer; ++j) {
+      const int l = tid * kLogPer + j;
+      if (l < n_log) {
+        const int e = lg[l].x;
+        o.inst_base[sm.inst_off[e] + 1 + (l - sm.first[e])] = pb[lg[l].y * P + M + lg[l].z];
+      }
     }
   }
   int max_fan = 0, n_groups = 0;
-  if (tid == 0) for (int w = 0; w < 32; ++w) { max_fan = max(max_fan, sm.feas[w]); n_groups += sm.warp_tmp[w]; }
+  if (tid == 0) for (int w = 0; w < kPlanWarps; ++w) { max_fan = max(max_fan, sm.feas[w]); n_groups += sm.warp_tmp[w]; }
   __syncthreads();
   {
     const int inc = block_incl_scan(load, sm.warp_tmp);
@@ -493,7 +517,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   }
   if (tid == 0) {
     int max_load = 0;
-    for (int w = 0; w < 32; ++w) max_load = max(max_load, sm.feas[w]);
+    for (int w = 0; w < kPlanWarps; ++w) max_load = max(max_load, sm.feas[w]);
     o.scalars[UEP_SC_TAU] = tau;
     o.scalars[UEP_SC_N_REPLICAS] = n_log;
     o.scalars[UEP_SC_MAX_LOAD] = max_load;
