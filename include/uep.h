@@ -18,7 +18,11 @@
  *     no host memory touched => every compute call can be stream-captured.
  *   - ownership: the library never frees or retains caller pointers beyond the call.
  *     Outputs and workspace are caller-allocated DEVICE memory.  A context may be shared by
- *     concurrent calls; a workspace may not (one per in-flight call).
+ *     concurrent calls of uep_histogram / uep_plan / uep_remap* / uep_pack on different streams;
+ *     a workspace may not (one per in-flight call).  uep_balance uses the context's internal
+ *     side stream and events: calls of uep_balance on one context must be issued from one host
+ *     thread at a time (they may target different streams; create one context per concurrent
+ *     host thread).
  *   - data faults that would need a sync to report (an id outside [0,E)) are counted on the
  *     device (scalars[UEP_SC_N_INVALID]) and the slot is skipped (S14).
  *   - all DEVICE pointers must be 16-byte aligned.

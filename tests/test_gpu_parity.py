@@ -382,3 +382,23 @@ def test_batched_planning_matches_single_and_oracle():
         for name in PLAN_ARRAYS:
             assert np.array_equal(np.asarray(getattr(hp, name)).ravel(),
                                   np.asarray(getattr(op, name)).ravel()), (b, name)
+
+
+@pytest.mark.parametrize("layer,mb", [(0, 0), (17, 3), (57, 1)])
+def test_training_sweep_instances_full_size(layer, mb):
+    """BASELINE config 3: (layer, microbatch) instances of the DeepSeek-V3 training sweep at full
+    size (Zipf s ~ U[0.6,1.6] per instance, fresh permutation), four state tensors (bf16 W + fp32
+    grad, m, v; 64 K elements each stand in for 7168 x 2048), through uep_balance."""
+    c = synth.CONFIGS["dsv3_train"]
+    base = 20260604
+    s = synth.train_sweep_s(base, layer, mb)
+    assert 0.6 <= s <= 1.6
+    seed = synth.instance_seed(base, layer, mb)
+    ids = synth.zipf_topk_ids(c["T"], c["k"], c["E"], s, seed, device=DEV).cpu()
+    gate = synth.gates_uniform_renorm(c["T"], c["k"], seed)
+    states = [synth.expert_state(c["E"], 1 << 16, 11, dtype=torch.bfloat16)] + \
+             [synth.expert_state(c["E"], 1 << 16, 12 + j, dtype=torch.float32) for j in range(3)]
+    g = gpu_chain(ids, gate, c["E"], c["R"], c["n_slot"], c["u_min"], states=states, use_balance=True)
+    o = oracle_chain(ids, gate, c["E"], c["R"], c["n_slot"], c["u_min"])
+    assert_parity(g, o, ids, gate, states)
+    ck.check_plan(o[0], with_layout(g["plan"]), c["u_min"])
