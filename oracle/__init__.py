@@ -4,9 +4,11 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 ``--impl reference`` legs may import this package.  It shares no code with the CUDA
 path (``paper_2606_04101_b200``) and never imports it.
 
-The arithmetic lives in ``uep_oracle.cpp`` (plain single-threaded C++, written from
-reference/PAPER.md Algorithm 1 and §5.2); this module only compiles it with g++ and
-marshals numpy arrays through ctypes.
+The arithmetic of O-1..O-4 lives in ``uep_oracle.cpp`` (plain single-threaded C++, written
+from reference/PAPER.md Algorithm 1 and §5.2); this module compiles it with g++ and marshals
+numpy arrays through ctypes.  The backward-path definitions O-5 (gradient reduction, fp64) and
+O-6 (inverse remap) are a few lines of numpy each, below; their pins are in
+tests/test_oracle_pins.py::test_grad_reduce_and_inverse_remap_pins.
 """
 from __future__ import annotations
 
@@ -187,3 +189,38 @@ def pack(slot_expert: np.ndarray, src: np.ndarray, dst: np.ndarray) -> None:
     rc = _load().uep_oracle_pack(_p(se.reshape(-1)), ctypes.c_int32(R), ctypes.c_int32(n_slot),
                                  _p(src), ctypes.c_int64(B), _p(dst))
     assert rc == 0
+
+
+def grad_reduce(pl: Plan, main_grad: np.ndarray, slot_grad: np.ndarray):
+    """O-5 backward gradient reduction ("every main expert aggregates the gradients
+    contributed by all of its remote replicas into the main gradient buffer"; PAPER.md:341
+    "accumulated into the local gradient buffer of main experts, and then cleared in place").
+
+    main_grad [E, B], slot_grad [R, n_slot, B] (any float dtype).  Returns (main_out float64 [E, B],
+    slot_out like slot_grad): main_out[e] = main[e] + sum over the replicas of e of their slot
+    buffer, accumulated in fp64 (the plain definition; a sum has no order in exact arithmetic);
+    slot buffers of USED redundant slots are zero afterwards, empty slots are untouched."""
+    main64 = np.asarray(main_grad, dtype=np.float64).copy()
+    slot_out = np.array(slot_grad, copy=True)
+    R, n_slot = pl.R, pl.n_slot
+    for t in range(R):
+        for s in range(n_slot):
+            e = int(pl.slot_expert[t, s])
+            if e < 0:
+                continue
+            main64[e] += np.asarray(slot_grad[t, s], dtype=np.float64)
+            slot_out[t, s] = 0
+    return main64, slot_out
+
+
+def inverse_remap(pl: Plan, rank: np.ndarray, offset: np.ndarray) -> np.ndarray:
+    """O-6 reverse reroute ("a scatter-to-gather inversion of the forward assignment",
+    PAPER.md:164-166): src[rank_base[rank[s]] + offset[s]] = s for every valid slot s (flat slot
+    index); positions past the number of valid slots are -1."""
+    rank = np.asarray(rank).reshape(-1)
+    offset = np.asarray(offset).reshape(-1)
+    src = np.full(rank.size, -1, dtype=np.int32)
+    for s in range(rank.size):
+        if rank[s] >= 0:
+            src[int(pl.rank_base[rank[s]]) + int(offset[s])] = s
+    return src

@@ -295,3 +295,38 @@ def test_dsv3_shape_plausibility_against_table3():
         assert 1.0 <= imb <= 1.01 + 1024 / mean + 1e-9
         assert 20 <= p.n_replicas <= 128 and int(p.scalars[3]) <= 16
         assert 12 <= int(p.scalars[4]) <= 24
+
+
+def test_grad_reduce_and_inverse_remap_pins():
+    """O-5 / O-6 against what the paper fixes: on worked example A (expert 0 replicated on ranks
+    1, 2, 3) with integer-valued gradients the reduction is a closed form; the total over all
+    buffers is conserved ("preserves equivalence with the no-replica formulation", PAPER.md:164);
+    empty slots are untouched; the inverse remap composed with the forward map is the identity
+    and equals a library stable argsort of the destination index."""
+    lam = np.array([400, 100, 50, 50, 120, 80, 60, 140], np.int32)
+    p = oracle.plan(lam, 4, 1, 10)
+    assert p.slot_expert.reshape(-1).tolist() == [-1, 0, 0, 0]
+    B = 6
+    main = np.arange(8 * B, dtype=np.float32).reshape(8, B)
+    slot = np.stack([np.full((1, B), 1000.0 * (t + 1), np.float32) for t in range(4)])
+    m2, s2 = oracle.grad_reduce(p, main, slot)
+    assert np.array_equal(m2[0], main[0] + 2000.0 + 3000.0 + 4000.0)       # closed form
+    assert np.array_equal(m2[1:], main[1:].astype(np.float64))             # no replica: unchanged
+    assert np.array_equal(s2[0], slot[0]) and not s2[1:].any()             # empty untouched, used cleared
+    assert m2.sum() + s2.sum() == main.astype(np.float64).sum() + slot.astype(np.float64).sum() - 0.0
+    # inverse remap on a random routing of that plan
+    rng = np.random.default_rng(3)
+    ids = np.repeat(np.arange(8, dtype=np.int32), lam)
+    rng.shuffle(ids)
+    rep, rnk, off, _ = oracle.remap(ids.reshape(-1, 1), None, p)
+    src = oracle.inverse_remap(p, rnk, off)
+    dest = p.rank_base[rnk.reshape(-1)] + off.reshape(-1)
+    assert np.array_equal(dest[src], np.arange(ids.size))                  # forward o inverse = id
+    assert np.array_equal(src, np.argsort(dest, kind="stable").astype(np.int32))
+    ids2 = ids.copy(); ids2[::7] = -1                                      # invalid slots drop out
+    rep, rnk, off, _ = oracle.remap(ids2.reshape(-1, 1), None, oracle.plan(
+        np.bincount(ids2[ids2 >= 0], minlength=8).astype(np.int32), 4, 1, 10, S_total=ids2.size))
+    pl2 = oracle.plan(np.bincount(ids2[ids2 >= 0], minlength=8).astype(np.int32), 4, 1, 10, S_total=ids2.size)
+    src2 = oracle.inverse_remap(pl2, rnk, off)
+    nv = int((ids2 >= 0).sum())
+    assert (src2[nv:] == -1).all() and sorted(src2[:nv].tolist()) == np.flatnonzero(ids2 >= 0).tolist()
