@@ -192,6 +192,22 @@ int uep_pack(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,
              const void* const* src, const size_t* bytes_per_expert, void* const* dst,
              void* stream);
 
+/* Backward gradient reduction (§4.2, §6.1), single-GPU part: for every
+ * replicated expert e, main_grad[j][e] += sum of slot_grad[j][t][s] over its replicas (t,s) in
+ * instance order (fp32, bit-reproducible), and those slot buffers are cleared in place; empty
+ * slots are not touched.  main_grad/slot_grad/bytes_per_expert: HOST arrays [n_tensors] of DEVICE
+ * float pointers ([E, B_j/4] and [R, n_slot, B_j/4]) and sizes B_j in bytes, B_j % 16 == 0. */
+int uep_grad_reduce(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,
+                    void* const* main_grad, const size_t* bytes_per_expert, void* const* slot_grad,
+                    void* stream);
+
+/* Reverse reroute ("a scatter-to-gather inversion of the forward assignment"):
+ * out_src[rank_base[rank[s]] + offset[s]] = s for every valid slot s (the gather list of the
+ * combine step / backward dispatch); positions past the number of valid slots are -1.
+ *   out_rank/out_offset  DEVICE int32 [T,k] as written by uep_remap;  out_src  DEVICE int32 [T*k] */
+int uep_remap_inverse(const uep_ctx* ctx, const int32_t* out_rank, const int32_t* out_offset,
+                      const uep_plan_out* plan, int32_t* out_src, void* stream);
+
 /* histogram -> plan -> remap and pack, chained on `stream`.  Internally forked/joined with
  * events on a side stream: uep_remap_rank runs beside histogram + plan (it does not depend on
  * them), and pack runs beside uep_remap_lookup, overlapping the reroute with the weight

@@ -24,7 +24,7 @@ SC_TAU, SC_N_REPLICAS, SC_MAX_LOAD, SC_MAX_FANOUT, SC_N_PROBES, SC_N_INVALID, SC
 
 EXPORTS = ["uep_create", "uep_destroy", "uep_workspace_bytes", "uep_workspace_init",
            "uep_plan_bytes", "uep_histogram", "uep_plan", "uep_plan_batched", "uep_remap", "uep_remap_rank",
-           "uep_remap_lookup", "uep_pack", "uep_balance",
+           "uep_remap_lookup", "uep_remap_inverse", "uep_pack", "uep_grad_reduce", "uep_balance",
            "uep_balance_host", "uep_strerror", "uep_last_cuda_error", "uep_get_launch_info"]
 
 
@@ -244,6 +244,16 @@ class Context:
         """src[j]: [E, ...] contiguous; dst[j]: [R, n_slot, ...] contiguous."""
         n, srcs, bpe, dsts = self._tensor_lists(src, dst)
         _check(lib().uep_pack(self._h, ctypes.byref(plan.c), n, srcs, bpe, dsts, _stream(stream)))
+
+    def uep_grad_reduce(self, plan: Plan, main_grad, slot_grad, stream=None):
+        """main_grad[j] [E, ...] fp32 += replicas' slot_grad[j] [R, n_slot, ...]; used slots cleared."""
+        n, mains, bpe, slots = self._tensor_lists(main_grad, slot_grad)
+        _check(lib().uep_grad_reduce(self._h, ctypes.byref(plan.c), n, mains, bpe, slots,
+                                     _stream(stream)))
+
+    def uep_remap_inverse(self, out_rank, out_offset, plan: Plan, out_src, stream=None):
+        _check(lib().uep_remap_inverse(self._h, _ptr(out_rank), _ptr(out_offset),
+                                       ctypes.byref(plan.c), _ptr(out_src), _stream(stream)))
 
     def uep_balance(self, topk_ids, gate, expert_count, plan: Plan, out_replica, out_rank,
                     out_offset, out_gate, src, dst, ws, stream=None):

@@ -312,6 +312,37 @@ int uep_pack(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,
   return launch_pack(c, *plan, a, static_cast<cudaStream_t>(stream));
 }
 
+int uep_grad_reduce(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,
+                    void* const* main_grad, const size_t* bytes_per_expert, void* const* slot_grad,
+                    void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c) return UEP_ERR_INVALID_ARG;
+  int rc = check_plan_ptrs(c, plan);
+  if (rc != UEP_OK) return rc;
+  if (n_tensors < 0 || n_tensors > UEP_MAX_TENSORS) return UEP_ERR_INVALID_ARG;
+  if (n_tensors && (!main_grad || !bytes_per_expert || !slot_grad)) return UEP_ERR_INVALID_ARG;
+  for (int j = 0; j < n_tensors; ++j) {
+    if (!main_grad[j] || !slot_grad[j] || !aligned16(main_grad[j]) || !aligned16(slot_grad[j]))
+      return UEP_ERR_INVALID_ARG;
+    if (bytes_per_expert[j] == 0 || (bytes_per_expert[j] & 15)) return UEP_ERR_INVALID_ARG;
+  }
+  if (n_tensors == 0 || c->cfg.n_slot == 0) return UEP_OK;
+  return launch_grad_reduce(c, *plan, n_tensors, main_grad, slot_grad, bytes_per_expert,
+                            static_cast<cudaStream_t>(stream));
+}
+
+int uep_remap_inverse(const uep_ctx* ctx, const int32_t* out_rank, const int32_t* out_offset,
+                      const uep_plan_out* plan, int32_t* out_src, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c) return UEP_ERR_INVALID_ARG;
+  int rc = check_plan_ptrs(c, plan);
+  if (rc != UEP_OK) return rc;
+  if (c->S > 0 && (!out_rank || !out_offset || !out_src || !aligned16(out_rank) ||
+                   !aligned16(out_offset) || !aligned16(out_src)))
+    return UEP_ERR_INVALID_ARG;
+  return launch_inverse(c, out_rank, out_offset, *plan, out_src, static_cast<cudaStream_t>(stream));
+}
+
 int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
                 int32_t* expert_count, const uep_plan_out* plan, int32_t* out_replica,
                 int32_t* out_rank, int32_t* out_offset, void* out_gate, int32_t n_tensors,

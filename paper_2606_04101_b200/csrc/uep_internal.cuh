@@ -68,6 +68,10 @@ int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_p
                  int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
                  void* ws, cudaStream_t s);
 int launch_pack(const Ctx* c, const uep_plan_out& plan, const PackArgs& a, cudaStream_t s);
+int launch_grad_reduce(const Ctx* c, const uep_plan_out& plan, int n_tensors, void* const* main_grad,
+                       void* const* slot_grad, const size_t* bytes, cudaStream_t s);
+int launch_inverse(const Ctx* c, const int32_t* out_rank, const int32_t* out_offset,
+                   const uep_plan_out& plan, int32_t* out_src, cudaStream_t s);
 struct Ctx;
 int init_plan_kernels(Ctx* c);    // opt-in shared memory attributes, cluster size
 int init_remap_kernels();

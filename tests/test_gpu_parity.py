@@ -402,3 +402,53 @@ def test_training_sweep_instances_full_size(layer, mb):
     o = oracle_chain(ids, gate, c["E"], c["R"], c["n_slot"], c["u_min"])
     assert_parity(g, o, ids, gate, states)
     ck.check_plan(o[0], with_layout(g["plan"]), c["u_min"])
+
+
+@pytest.mark.parametrize("T,k,E,R,n_slot,s,elems", [
+    (4096, 2, 16, 4, 1, 1.2, 1000 * 4 + 4),        # tiny config, ragged tile (16016 B per expert)
+    (65536, 8, 128, 32, 2, 1.4, 3 * 8192 + 12),    # several tiles and a ragged tail
+    (32768, 8, 64, 8, 4, 2.0, 8192),               # four slots per rank, high fan-out
+])
+def test_grad_reduce_and_inverse_remap(T, k, E, R, n_slot, s, elems):
+    """NEXT-2: backward gradient reduction (fp32) and the inverse remap against the oracle."""
+    um = synth.stress_u_min(T * k, R)
+    ids = synth.zipf_topk_ids(T, k, E, s, 77)
+    ctx = binding.Context(T, k, E, R, n_slot, um, gate_dtype=binding.GATE_NONE)
+    ws, plan = ctx.new_workspace(), ctx.new_plan()
+    d_ids = ids.to(DEV)
+    count = torch.zeros(E, dtype=torch.int32, device=DEV)
+    rep, rnk, off, _ = ctx.new_outputs(None)
+    ctx.uep_balance(d_ids, None, count, plan, rep, rnk, off, None, [], [], ws)
+    g = torch.Generator().manual_seed(5)
+    mains = [torch.randn((E, elems), generator=g), torch.randn((E, 64), generator=g)]
+    slots = [torch.randn((R, n_slot, elems), generator=g), torch.randn((R, n_slot, 64), generator=g)]
+    d_main = [m.to(DEV) for m in mains]
+    d_slot = [x.to(DEV) for x in slots]
+    ctx.uep_grad_reduce(plan, d_main, d_slot)
+    src = torch.full((T * k,), -7, dtype=torch.int32, device=DEV)
+    ctx.uep_remap_inverse(rnk, off, plan, src)
+    torch.cuda.synchronize()
+    lam, _ = oracle.histogram(ids.numpy(), E)
+    p = oracle.plan(lam, R, n_slot, um, S_total=T * k)
+    assert p.n_replicas > 0
+    for m, x, dm, dx in zip(mains, slots, d_main, d_slot):
+        m64, s_ref = oracle.grad_reduce(p, m.numpy(), x.numpy())
+        got = dm.cpu().numpy()
+        # fp32 sum of at most 1 + n_replicas(e) terms vs the exact sum: |err| <= n * 2^-24 * sum|terms|
+        mag = np.abs(m.numpy()).astype(np.float64)
+        nterm = np.ones(E)
+        for t in range(R):
+            for q in range(n_slot):
+                e = int(p.slot_expert[t, q])
+                if e >= 0:
+                    mag[e] += np.abs(x.numpy()[t, q]); nterm[e] += 1
+        assert (np.abs(got - m64) <= (nterm[:, None] * 2.0 ** -24) * mag + 1e-30).all()
+        # and bit-equal to the sequential fp32 sum in instance order (main, replicas as accepted)
+        seq = m.numpy().copy()
+        for e in range(E):
+            for i in range(p.inst_off[e] + 1, p.inst_off[e + 1]):
+                seq[e] = seq[e] + x.numpy()[p.inst_rank[i], p.inst_phys[i] - p.M]
+        assert np.array_equal(got, seq)
+        assert np.array_equal(dx.cpu().numpy(), s_ref)              # used slots cleared, empty untouched
+    o_rep, o_rnk, o_off, _ = oracle.remap(ids.numpy(), None, p)
+    assert np.array_equal(src.cpu().numpy(), oracle.inverse_remap(p, o_rnk, o_off))
