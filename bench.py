@@ -325,6 +325,21 @@ def run_uep(args):
     _t.cuda.synchronize(device)
     g_bplan = capture([lambda: rig.ctx.uep_plan_batched(n_inst, counts_all, bplan)], stream)
     bplan_ms, _ = time_graph(g_bplan, stream, reps)
+    # NEXT-2: backward gradient reduction (fp32, one [7168 x 2048]-like matrix per
+    # expert for the DSV3 shapes) and the inverse remap, on the plans of this run
+    g_elems = 7168 * 2048 if c["E"] >= 256 else (4096 * 1408 if c["E"] >= 128 else 256 * 512)
+    g_elems = max(8, int(g_elems * args.state_scale) // 8 * 8)
+    main_grad = _t.ones((c["E"], g_elems), dtype=_t.float32, device=device)
+    slot_grad = _t.ones((c["R"], max(c["n_slot"], 1), g_elems), dtype=_t.float32, device=device)
+    out_src = _t.empty(S_slots := c["T"] * c["k"], dtype=_t.int32, device=device)
+    n_red = min(n_inst, 4)
+    _t.cuda.synchronize(device)
+    g_red = capture([lambda i=i: rig.ctx.uep_grad_reduce(rig.plans[i], [main_grad], [slot_grad])
+                     for i in range(n_red)], stream)
+    red_ms, _ = time_graph(g_red, stream, 3, warm=1)
+    g_inv = capture([lambda i=i: rig.ctx.uep_remap_inverse(rig.outs[i][1], rig.outs[i][2], rig.plans[i], out_src)
+                     for i in range(n_inst)], stream)
+    inv_ms, _ = time_graph(g_inv, stream, reps)
     clocks = sampler.stop()
     chain_ms = barrier_and_max(world, chain_ms, device)
     # whole-job aggregate: `world` ranks each planned n_inst layers in chain_ms (max over ranks)
@@ -396,6 +411,13 @@ def run_uep(args):
         "batched_plan": {"instances": n_inst, "us_total": round(bplan_ms * 1e3, 2),
                          "us_per_layer": round(bplan_ms * 1e3 / n_inst, 3),
                          "note": "uep_plan_batched: one launch, one 8-CTA cluster per instance"},
+        "backward": {"grad_reduce_us": round(red_ms * 1e3 / n_red, 2),
+                     "grad_reduce_bytes": int(statistics.mean(2 * (n_grp[i] + n_rep[i]) for i in range(n_red)) * g_elems * 4),
+                     "grad_reduce_frac_of_peak": round(statistics.mean(2 * (n_grp[i] + n_rep[i]) for i in range(n_red))
+                                                       * g_elems * 4 / (red_ms * 1e-3 / n_red) / 1e9 / peak_gbs, 4),
+                     "inverse_remap_us": round(inv_ms * 1e3 / n_inst, 2),
+                     "note": "uep_grad_reduce: fp32 [E, %d] main + [R, n_slot, %d] slot grads, bytes = 2 x (groups + replicas) x B; "
+                             "uep_remap_inverse: 8 B/slot read, 4 B/slot scattered write" % (g_elems, g_elems)},
         "roofline": {k: r_pack[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")},
         "rooflines": rooflines,
         "gpu_launches": 6 * K,

@@ -10,18 +10,23 @@
 //
 // grad_reduce_kernel is HBM-bound: per replicated expert with f replicas it reads (1+f) B and
 // writes (1+f) B (the sum, and zeros).  Kept from the paper: fixed tiles, a persistent static grid
-// (capturable although the work list is data-dependent), every tile of the main buffer touched
-// once.  Each thread owns float4 elements of the tile; the addends are added in instance order
-// (main, then replicas in acceptance order), so the fp32 result is bit-identical run to run and
-// equal to a sequential fp32 sum in that order.
+// (capturable although the work list is data-dependent), shared-memory tiles filled ahead of the
+// reduction.  B200 form: one elected producer thread per CTA streams 8 KB tiles (main, then each
+// replica, in instance order) into a 16-stage shared-memory ring with cp.async.bulk on mbarriers;
+// four consumer warps add them in that order (so the fp32 result is bit-identical run to run and
+// equal to a sequential fp32 sum), release each stage as soon as they have read it, and one of
+// them sends the reduced tile and the zero tiles back with cp.async.bulk shared->global.  A first
+// version with register-resident loads (no ring) reached 0.23-0.29 of the HBM peak: one batch of
+// loads in flight per thread is not enough memory parallelism; the ring reaches 0.90.
 #include "uep_internal.cuh"
 
 namespace uep {
 
-constexpr int kRedThreads = 512;
-constexpr int kRedVec = 4;                                   // float4 per thread per tile
-constexpr int kRedTileBytes = kRedThreads * kRedVec * 16;    // 32 KB of fp32 per tile
-constexpr int kRedMaxFan = UEP_MAX_R;                        // replicas of one expert
+constexpr int kRedConsumers = 128;                           // 4 consumer warps; warp 0 is the producer
+constexpr int kRedThreads = 32 + kRedConsumers;
+constexpr int kRedTile = 8 * 1024;                           // bytes per tile = 128 threads x 4 float4
+constexpr int kRedVec = kRedTile / 16 / kRedConsumers;       // float4 per consumer thread per tile
+constexpr int kRedStages = 16;                               // shared-memory ring of load tiles (128 KB)
 
 struct RedArgs {
   float* main_grad[UEP_MAX_TENSORS];
@@ -30,58 +35,140 @@ struct RedArgs {
   int n_tensors;
 };
 
-__global__ void __launch_bounds__(kRedThreads, 2)
-grad_reduce_kernel(RedArgs a, int E, int n_slot, int M, const int32_t* __restrict__ inst_off,
-                   const int32_t* __restrict__ inst_rank, const int32_t* __restrict__ inst_phys) {
-  __shared__ int s_slot[kRedMaxFan];
-  const int tid = threadIdx.x, G = gridDim.x, c = blockIdx.x;
-  unsigned rot = 0;                               // rotation so that tile remainders spread over CTAs
+__device__ __forceinline__ uint32_t red_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void red_mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(red_smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void red_mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(red_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void red_mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(red_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void red_mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "RED_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra RED_DONE;\n"
+      "bra RED_WAIT;\n"
+      "RED_DONE:\n"
+      "}\n" ::"r"(red_smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void red_bulk_g2s(void* dst_smem, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   red_smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(red_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void red_bulk_s2g(void* dst, const void* src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(red_smem_u32(src_smem)),
+               "r"(bytes) : "memory");
+}
+
+// Both roles enumerate the same units in the same order: experts ascending (only those with
+// replicas), tensors ascending, tiles c', c'+G, ... (rotated per (expert, tensor) so that tile
+// remainders spread over CTAs).  A unit = one tile of the main buffer and the same tile of every
+// replica slot: 1 + f ring stages.
+template <typename F>
+__device__ __forceinline__ void red_for_each_unit(const RedArgs& a, int E, const int32_t* inst_off, F&& fn) {
+  const int G = gridDim.x, c = blockIdx.x;
+  unsigned rot = 0;
   for (int e = 0; e < E; ++e) {
-    const int lo = inst_off[e], f = inst_off[e + 1] - lo - 1;      // f replicas (entry lo = main)
+    const int lo = __ldg(inst_off + e), f = __ldg(inst_off + e + 1) - lo - 1;   // entry lo = main
     if (f <= 0) continue;
-    __syncthreads();                              // previous expert done with s_slot
-    for (int p = tid; p < f; p += kRedThreads)
-      s_slot[p] = inst_rank[lo + 1 + p] * n_slot + (inst_phys[lo + 1 + p] - M);
-    __syncthreads();
     for (int j = 0; j < a.n_tensors; ++j) {
       const unsigned long long B = a.bytes[j];
-      const long long tiles = (long long)((B + kRedTileBytes - 1) / kRedTileBytes);
-      float4* mainp = reinterpret_cast<float4*>(reinterpret_cast<unsigned char*>(a.main_grad[j]) +
-                                                (unsigned long long)e * B);
-      unsigned char* slots = reinterpret_cast<unsigned char*>(a.slot_grad[j]);
-      const long long n4 = (long long)(B >> 4);
+      const long long tiles = (long long)((B + kRedTile - 1) / kRedTile);
       for (long long tile = (c + G - (int)rot) % G; tile < tiles; tile += G) {
-        const long long base = tile * (kRedTileBytes >> 4);
-        float4 acc[kRedVec];
-#pragma unroll
-        for (int v = 0; v < kRedVec; ++v) {
-          const long long i = base + v * kRedThreads + tid;
-          acc[v] = (i < n4) ? __ldcs(mainp + i) : make_float4(0.f, 0.f, 0.f, 0.f);
-        }
-        for (int p = 0; p < f; ++p) {             // instance order: main, replica 1, replica 2, ...
-          float4* sp = reinterpret_cast<float4*>(slots + (unsigned long long)s_slot[p] * B);
-          float4 x[kRedVec];
-#pragma unroll
-          for (int v = 0; v < kRedVec; ++v) {
-            const long long i = base + v * kRedThreads + tid;
-            x[v] = (i < n4) ? __ldcs(sp + i) : make_float4(0.f, 0.f, 0.f, 0.f);
-          }
-#pragma unroll
-          for (int v = 0; v < kRedVec; ++v) {
-            const long long i = base + v * kRedThreads + tid;
-            acc[v].x += x[v].x; acc[v].y += x[v].y; acc[v].z += x[v].z; acc[v].w += x[v].w;
-            if (i < n4) __stcs(sp + i, make_float4(0.f, 0.f, 0.f, 0.f));   // cleared in place
-          }
-        }
-#pragma unroll
-        for (int v = 0; v < kRedVec; ++v) {
-          const long long i = base + v * kRedThreads + tid;
-          if (i < n4) __stcs(mainp + i, acc[v]);
-        }
+        const unsigned long long off = (unsigned long long)tile * kRedTile;
+        fn(e, j, lo, f, off, (uint32_t)min((unsigned long long)kRedTile, B - off));
       }
       rot = (unsigned)((rot + tiles) % (unsigned)G);
     }
   }
+}
+
+__global__ void __launch_bounds__(kRedThreads, 1)
+grad_reduce_kernel(RedArgs a, int E, int n_slot, int M, const int32_t* __restrict__ inst_off,
+                   const int32_t* __restrict__ inst_rank, const int32_t* __restrict__ inst_phys) {
+  extern __shared__ __align__(128) unsigned char red_smem[];
+  unsigned char* ring = red_smem;                                    // [kRedStages][kRedTile]
+  unsigned char* outbuf = ring + (size_t)kRedStages * kRedTile;      // [2][kRedTile] reduced main tiles
+  unsigned char* zero = outbuf + 2 * kRedTile;                       // [kRedTile] zeros
+  __shared__ __align__(8) uint64_t full[kRedStages], empty[kRedStages];
+  const int tid = threadIdx.x;
+  for (int i = tid; i < kRedTile / 16; i += kRedThreads)
+    reinterpret_cast<float4*>(zero)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (tid == 0) {
+    for (int s = 0; s < kRedStages; ++s) { red_mbar_init(&full[s], 1); red_mbar_init(&empty[s], kRedConsumers); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");       // zero tile visible to bulk stores
+  __syncthreads();
+  auto slot_of = [&](int p) { return __ldg(inst_rank + p) * n_slot + (__ldg(inst_phys + p) - M); };
+
+  if (tid < 32) {
+    // ---- producer: one elected thread streams tiles into the ring ------------------------------
+    if (tid != 0) return;
+    unsigned long long n = 0;                                        // ring position (tile counter)
+    auto load = [&](const unsigned char* src, uint32_t bytes) {
+      const int st = (int)(n % kRedStages);
+      if (n >= kRedStages) red_mbar_wait(&empty[st], (uint32_t)(((n / kRedStages) - 1) & 1));
+      red_mbar_expect_tx(&full[st], bytes);
+      red_bulk_g2s(ring + (size_t)st * kRedTile, src, bytes, &full[st]);
+      ++n;
+    };
+    red_for_each_unit(a, E, inst_off, [&](int e, int j, int lo, int f, unsigned long long off, uint32_t bytes) {
+      const unsigned long long B = a.bytes[j];
+      load(reinterpret_cast<const unsigned char*>(a.main_grad[j]) + (unsigned long long)e * B + off, bytes);
+      for (int q = 1; q <= f; ++q)
+        load(reinterpret_cast<const unsigned char*>(a.slot_grad[j]) + (unsigned long long)slot_of(lo + q) * B + off, bytes);
+    });
+    return;
+  }
+
+  // ---- consumers: 128 threads, 4 float4 each per tile --------------------------------------------
+  const int ct = tid - 32;
+  unsigned long long n = 0, unit = 0;
+  red_for_each_unit(a, E, inst_off, [&](int e, int j, int lo, int f, unsigned long long off, uint32_t bytes) {
+    const int n4 = (int)(bytes >> 4);
+    float4 acc[kRedVec];
+    for (int q = 0; q <= f; ++q) {                       // instance order: main, replica 1, 2, ...
+      const int st = (int)(n % kRedStages);
+      red_mbar_wait(&full[st], (uint32_t)((n / kRedStages) & 1));
+      const float4* t = reinterpret_cast<const float4*>(ring + (size_t)st * kRedTile);
+#pragma unroll
+      for (int v = 0; v < kRedVec; ++v) {
+        const int i = v * kRedConsumers + ct;
+        const float4 x = (i < n4) ? t[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+        if (q == 0) acc[v] = x;
+        else { acc[v].x += x.x; acc[v].y += x.y; acc[v].z += x.z; acc[v].w += x.w; }
+      }
+      red_mbar_arrive(&empty[st]);                       // this thread is done with the stage
+      ++n;
+    }
+    // (A) the elected thread has waited until the stores of unit-2 finished reading outbuf[unit&1]
+    asm volatile("bar.sync 1, %0;" ::"n"(kRedConsumers) : "memory");
+    float4* ob = reinterpret_cast<float4*>(outbuf + (size_t)(unit & 1) * kRedTile);
+#pragma unroll
+    for (int v = 0; v < kRedVec; ++v) {
+      const int i = v * kRedConsumers + ct;
+      if (i < n4) ob[i] = acc[v];
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("bar.sync 1, %0;" ::"n"(kRedConsumers) : "memory");      // (B) tile complete in shared memory
+    if (ct == 0) {
+      const unsigned long long B = a.bytes[j];
+      red_bulk_s2g(reinterpret_cast<unsigned char*>(a.main_grad[j]) + (unsigned long long)e * B + off, ob, bytes);
+      for (int q = 1; q <= f; ++q)                       // cleared in place
+        red_bulk_s2g(reinterpret_cast<unsigned char*>(a.slot_grad[j]) + (unsigned long long)slot_of(lo + q) * B + off,
+                     zero, bytes);
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");  // unit-1's stores have read their smem
+    }
+    ++unit;
+  });
+  if (ct == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 __global__ void __launch_bounds__(256)
@@ -95,6 +182,12 @@ inverse_kernel(const int32_t* __restrict__ out_rank, const int32_t* __restrict__
   if (s >= n_valid) out_src[s] = -1;       // positions past the valid slots (destinations are < n_valid)
 }
 
+int init_reduce_kernels() {
+  UEP_CUDA_TRY(cudaFuncSetAttribute(grad_reduce_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (kRedStages + 3) * kRedTile));
+  return UEP_OK;
+}
+
 int launch_grad_reduce(const Ctx* c, const uep_plan_out& plan, int n_tensors, void* const* main_grad,
                        void* const* slot_grad, const size_t* bytes, cudaStream_t s) {
   RedArgs a;
@@ -104,9 +197,10 @@ int launch_grad_reduce(const Ctx* c, const uep_plan_out& plan, int n_tensors, vo
     a.slot_grad[j] = static_cast<float*>(slot_grad[j]);
     a.bytes[j] = bytes[j];
   }
-  grad_reduce_kernel<<<2 * c->sm_count, kRedThreads, 0, s>>>(a, c->cfg.E, c->cfg.n_slot, c->M,
-                                                           plan.inst_off, plan.inst_rank,
-                                                           plan.inst_phys);
+  const size_t smem = (size_t)(kRedStages + 3) * kRedTile;
+  grad_reduce_kernel<<<c->sm_count, kRedThreads, smem, s>>>(a, c->cfg.E, c->cfg.n_slot, c->M,
+                                                            plan.inst_off, plan.inst_rank,
+                                                            plan.inst_phys);
   UEP_CUDA_TRY(cudaGetLastError());
   return UEP_OK;
 }

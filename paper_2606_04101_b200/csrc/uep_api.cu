@@ -145,6 +145,7 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   if (rc == UEP_OK) rc = init_hist_kernels();
   if (rc == UEP_OK) rc = init_remap_kernels();
   if (rc == UEP_OK) rc = init_pack_kernels();
+  if (rc == UEP_OK) rc = init_reduce_kernels();
   if (rc != UEP_OK) return fail(rc);
   *out = reinterpret_cast<uep_ctx*>(c);
   return UEP_OK;

@@ -76,6 +76,7 @@ struct Ctx;
 int init_plan_kernels(Ctx* c);    // opt-in shared memory attributes, cluster size
 int init_remap_kernels();
 int init_pack_kernels();
+int init_reduce_kernels();
 
 int init_hist_kernels();
 
