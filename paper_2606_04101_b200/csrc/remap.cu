@@ -10,11 +10,13 @@
 //                 expert inside its chunk, packed with the expert id into one int32 per slot in
 //                 the workspace.  uep_balance runs it on a side stream concurrently with
 //                 uep_histogram and uep_plan, so it is off the critical path gate -> dispatch.
-//   lookup_kernel (plan-DEPENDENT) global rank = chunk base (column sums of the chunk-table rows
-//                 below, independent int4 L2 loads) + rank in chunk; cumulative-quota lookup;
-//                 writes (replica, rank, offset) and the gates in dispatch order.
+//   lookup_kernel (plan-DEPENDENT) global rank = chunk base (the chunk's row of the exclusive
+//                 prefix over chunks, left by prefix_kernel) + rank in chunk; cumulative-quota
+//                 lookup; writes (replica, rank, offset) and the gates in dispatch order.  Under
+//                 programmatic dependent launch everything before its griddepcontrol.wait (packed
+//                 ranks, gates, prefix rows) overlaps the planner.
 //
-// rank_kernel: one CTA per chunk (<= 16384 slots, register-resident), every warp owns a
+// rank_kernel: one CTA per chunk (<= 8192 slots, register-resident, two CTAs per SM), every warp owns a
 // contiguous span and loads its ids up front (coalesced).  Ranking inside a warp uses a
 // warp-private shared-memory row of {peer mask, count} cells: lanes OR their lane bit into the
 // cell of their expert, read {mask, count} back with one 64-bit load, and the lowest peer stores
