@@ -86,9 +86,11 @@ hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
     for (int w = 0; w < kHistWarps; ++w) s += priv[w * pitch + e];
     grow[e] = s;
   }
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) s_last = (atomicAdd(ticket, 1u) == (unsigned)(n_chunks - 1));
+  __syncthreads();                   // the CTA's row is written (barrier orders it before thread 0's fence)
+  if (tid == 0) {
+    __threadfence();                 // cumulative: makes the whole row visible before the ticket
+    s_last = (atomicAdd(ticket, 1u) == (unsigned)(n_chunks - 1));
+  }
   __syncthreads();
   if (!s_last) return;
   __threadfence();

@@ -102,7 +102,7 @@ __device__ __forceinline__ void column_sums(const int32_t* __restrict__ table, i
   if (rg < NRG) {
     int4 acc = make_int4(0, 0, 0, 0);
     const int4* col = reinterpret_cast<const int4*>(table) + cg;
-#pragma unroll 5
+#pragma unroll 10
     for (int r = rg; r < n_rows; r += NRG) {
       const int4 v = __ldcg(col + (size_t)r * CG);
       acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
