@@ -224,3 +224,59 @@ def inverse_remap(pl: Plan, rank: np.ndarray, offset: np.ndarray) -> np.ndarray:
         if rank[s] >= 0:
             src[int(pl.rank_base[rank[s]]) + int(offset[s])] = s
     return src
+
+
+RELAY_THRESHOLD = 4          # "experts whose replica count exceeds the relay threshold (set to 4)"
+
+
+def relay_frontier(f: int) -> int:
+    """Relay frontier "chosen near sqrt(|H(e)|-1)": sqrt(f) rounded to nearest,
+    in integers: k = floor(sqrt(f)), +1 if f > k*k + k."""
+    k = int(np.floor(np.sqrt(f)))
+    while k * k > f:
+        k -= 1
+    while (k + 1) * (k + 1) <= f:
+        k += 1
+    return k + 1 if f > k * k + k else k
+
+
+def relay_plan(pl: Plan):
+    """O-7 load-aware relay scheduling, topology only (§6.2), step by step:
+      1. send volume of every rank = number of replica copies its main experts must push;
+      2. relay-eligible experts (replica count f > 4), one by one in ascending expert id
+         (the paper gives no order; DESIGN.md S24);
+      3. first-stage relays = the k = relay_frontier(f) replica ranks of e with the smallest
+         sending volume (ties -> lower rank id);
+      4. every remaining replica, in instance order, is attached to the relay whose sending volume
+         would remain smallest after taking it (ties -> lower rank id);
+      5. volumes updated: the source now sends k copies instead of f, each relay its leaves.
+    Returns (parent[E + R*n_slot] int32 aligned with the plan's CSR: -1 for main instances and
+    unused entries, else the rank that sends this replica its copy; send_volume[R] int32)."""
+    E, R = pl.E, pl.R
+    parent = np.full(pl.inst_rank.size, -1, dtype=np.int32)
+    vol = np.zeros(R, dtype=np.int64)
+    for e in range(E):
+        lo, hi = int(pl.inst_off[e]), int(pl.inst_off[e + 1])
+        vol[pl.home[e]] += hi - lo - 1
+        parent[lo + 1:hi] = pl.home[e]                      # direct sends unless a relay tree replaces them
+    for e in range(E):
+        lo, hi = int(pl.inst_off[e]), int(pl.inst_off[e + 1])
+        f = hi - lo - 1
+        if f <= RELAY_THRESHOLD:
+            continue
+        k = relay_frontier(f)
+        reps = list(range(lo + 1, hi))                      # CSR indices of the replicas, instance order
+        order = sorted(reps, key=lambda p: (vol[pl.inst_rank[p]], pl.inst_rank[p]))
+        relays = order[:k]
+        relay_set = set(relays)
+        leaves_of = {p: 0 for p in relays}
+        for p in reps:
+            if p in relay_set:
+                continue
+            best = min(relays, key=lambda q: (vol[pl.inst_rank[q]] + leaves_of[q] + 1, pl.inst_rank[q]))
+            parent[p] = pl.inst_rank[best]
+            leaves_of[best] += 1
+        vol[pl.home[e]] += k - f
+        for q in relays:
+            vol[pl.inst_rank[q]] += leaves_of[q]
+    return parent, vol.astype(np.int32)

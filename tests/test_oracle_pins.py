@@ -330,3 +330,47 @@ def test_grad_reduce_and_inverse_remap_pins():
     src2 = oracle.inverse_remap(pl2, rnk, off)
     nv = int((ids2 >= 0).sum())
     assert (src2[nv:] == -1).all() and sorted(src2[:nv].tolist()) == np.flatnonzero(ids2 >= 0).tolist()
+
+
+def test_relay_plan_pins():
+    """O-7 against what §6.2 fixes: frontier = sqrt(f) to nearest; only experts with more than 4
+    replicas get a tree; every replica has one parent in {home} U relays(e), relays hang off the
+    home rank, leaves off relays; a rank's final send volume = the number of children it has;
+    the all-to-one-expert closed form (f = 63: 8 relays, source fan-out 8 instead of 63, leaves
+    7,7,7,7,7,7,7,6 because all relay volumes tie and ties go to the lower rank id)."""
+    assert [oracle.relay_frontier(f) for f in (5, 6, 7, 8, 9, 12, 13, 16, 20, 21, 63, 255)] == \
+        [2, 2, 3, 3, 3, 3, 4, 4, 4, 5, 8, 16]
+    E, R, S = 256, 64, 2097152
+    lam = np.zeros(E, np.int32); lam[0] = S
+    p = oracle.plan(lam, R, 2, 1024)
+    assert p.n_replicas == 63
+    parent, vol = oracle.relay_plan(p)
+    lo, hi = p.inst_off[0], p.inst_off[1]
+    kids = np.bincount(parent[lo + 1:hi], minlength=R)
+    assert kids[0] == 8 and vol[0] == 8                        # the source pushes 8 copies, not 63
+    relays = [r for r in range(1, R) if kids[r] > 0]
+    assert relays == list(range(1, 9)) and kids[1:9].tolist() == [7, 7, 7, 7, 7, 7, 7, 6]
+    assert vol.sum() == 63 and np.array_equal(vol, kids)
+    # general invariants on skewed routing
+    for s, seed in ((1.4, 1), (2.0, 2)):
+        ids = synth.zipf_topk_ids(32768, 8, 128, s, seed).numpy()
+        lam, _ = oracle.histogram(ids, 128)
+        p = oracle.plan(lam, 32, 2, 64)
+        parent, vol = oracle.relay_plan(p)
+        kids = np.zeros(32, np.int64)
+        for e in range(128):
+            lo, hi = p.inst_off[e], p.inst_off[e + 1]
+            f = hi - lo - 1
+            assert parent[lo] == -1
+            reps = list(range(lo + 1, hi))
+            par = parent[lo + 1:hi]
+            np.add.at(kids, par, 1)
+            if f <= oracle.RELAY_THRESHOLD:
+                assert (par == p.home[e]).all()
+                continue
+            relay_ranks = {int(p.inst_rank[q]) for q in reps if parent[q] == p.home[e]}
+            assert len(relay_ranks) == oracle.relay_frontier(f)
+            assert all(int(x) == p.home[e] or int(x) in relay_ranks for x in par)
+            assert all(parent[q] != p.inst_rank[q] for q in reps)          # nobody relays to itself
+        assert np.array_equal(kids, vol) and vol.sum() == p.n_replicas
+        assert (parent[p.inst_off[-1]:] == -1).all()
