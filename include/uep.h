@@ -201,6 +201,16 @@ int uep_grad_reduce(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tens
                     void* const* main_grad, const size_t* bytes_per_expert, void* const* slot_grad,
                     void* stream);
 
+/* Load-aware relay scheduling, topology only (§6.2): for every expert with more
+ * than 4 replicas, sqrt(f) (to nearest) first-stage relays among its replica ranks with the
+ * smallest sending volume, the other replicas attached to the relay whose volume would remain
+ * smallest; experts are processed in ascending id, volumes updated in between (S24).
+ *   relay_parent  DEVICE int32 [E + R*n_slot], aligned with the plan's CSR: -1 for main instances
+ *                 and unused entries, else the rank that sends this replica its copy
+ *   send_volume   DEVICE int32 [R]: copies each rank sends under the resulting trees          */
+int uep_relay_plan(const uep_ctx* ctx, const uep_plan_out* plan, int32_t* relay_parent,
+                   int32_t* send_volume, void* stream);
+
 /* Reverse reroute ("a scatter-to-gather inversion of the forward assignment"):
  * out_src[rank_base[rank[s]] + offset[s]] = s for every valid slot s (the gather list of the
  * combine step / backward dispatch); positions past the number of valid slots are -1.

@@ -24,7 +24,8 @@ SC_TAU, SC_N_REPLICAS, SC_MAX_LOAD, SC_MAX_FANOUT, SC_N_PROBES, SC_N_INVALID, SC
 
 EXPORTS = ["uep_create", "uep_destroy", "uep_workspace_bytes", "uep_workspace_init",
            "uep_plan_bytes", "uep_histogram", "uep_plan", "uep_plan_batched", "uep_remap", "uep_remap_rank",
-           "uep_remap_lookup", "uep_remap_inverse", "uep_pack", "uep_grad_reduce", "uep_balance",
+           "uep_remap_lookup", "uep_remap_inverse", "uep_relay_plan", "uep_pack", "uep_grad_reduce",
+           "uep_balance",
            "uep_balance_host", "uep_strerror", "uep_last_cuda_error", "uep_get_launch_info"]
 
 
@@ -250,6 +251,10 @@ class Context:
         n, mains, bpe, slots = self._tensor_lists(main_grad, slot_grad)
         _check(lib().uep_grad_reduce(self._h, ctypes.byref(plan.c), n, mains, bpe, slots,
                                      _stream(stream)))
+
+    def uep_relay_plan(self, plan: Plan, relay_parent, send_volume, stream=None):
+        _check(lib().uep_relay_plan(self._h, ctypes.byref(plan.c), _ptr(relay_parent),
+                                    _ptr(send_volume), _stream(stream)))
 
     def uep_remap_inverse(self, out_rank, out_offset, plan: Plan, out_src, stream=None):
         _check(lib().uep_remap_inverse(self._h, _ptr(out_rank), _ptr(out_offset),

@@ -332,6 +332,16 @@ int uep_grad_reduce(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tens
                             static_cast<cudaStream_t>(stream));
 }
 
+int uep_relay_plan(const uep_ctx* ctx, const uep_plan_out* plan, int32_t* relay_parent,
+                   int32_t* send_volume, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !relay_parent || !send_volume || !aligned16(relay_parent) || !aligned16(send_volume))
+    return UEP_ERR_INVALID_ARG;
+  int rc = check_plan_ptrs(c, plan);
+  if (rc != UEP_OK) return rc;
+  return launch_relay(c, *plan, relay_parent, send_volume, static_cast<cudaStream_t>(stream));
+}
+
 int uep_remap_inverse(const uep_ctx* ctx, const int32_t* out_rank, const int32_t* out_offset,
                       const uep_plan_out* plan, int32_t* out_src, void* stream) {
   const Ctx* c = reinterpret_cast<const Ctx*>(ctx);

@@ -70,6 +70,8 @@ int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_p
 int launch_pack(const Ctx* c, const uep_plan_out& plan, const PackArgs& a, cudaStream_t s);
 int launch_grad_reduce(const Ctx* c, const uep_plan_out& plan, int n_tensors, void* const* main_grad,
                        void* const* slot_grad, const size_t* bytes, cudaStream_t s);
+int launch_relay(const Ctx* c, const uep_plan_out& plan, int32_t* parent, int32_t* send_volume,
+                 cudaStream_t s);
 int launch_inverse(const Ctx* c, const int32_t* out_rank, const int32_t* out_offset,
                    const uep_plan_out& plan, int32_t* out_src, cudaStream_t s);
 struct Ctx;

@@ -452,3 +452,30 @@ def test_grad_reduce_and_inverse_remap(T, k, E, R, n_slot, s, elems):
         assert np.array_equal(dx.cpu().numpy(), s_ref)              # used slots cleared, empty untouched
     o_rep, o_rnk, o_off, _ = oracle.remap(ids.numpy(), None, p)
     assert np.array_equal(src.cpu().numpy(), oracle.inverse_remap(p, o_rnk, o_off))
+
+
+@pytest.mark.parametrize("T,k,E,R,n_slot,dist", [
+    (262144, 8, 256, 64, 2, "one"),        # f = 63: the closed form of the oracle pin
+    (65536, 8, 128, 32, 2, "zipf1.4"),
+    (65536, 8, 512, 256, 4, "zipf2"),      # fan-outs well above the relay threshold, R = 256
+    (4096, 2, 16, 4, 1, "zipf1.2"),        # nothing eligible: direct sends only
+])
+def test_relay_plan_parity(T, k, E, R, n_slot, dist):
+    """NEXT-3: relay trees and send volumes, bit-exact against the oracle."""
+    um = synth.stress_u_min(T * k, R)
+    ids = synth.one_expert_ids(T, k, 0) if dist == "one" else \
+        synth.zipf_topk_ids(T, k, E, float(dist[4:]), 31)
+    ctx = binding.Context(T, k, E, R, n_slot, um, gate_dtype=binding.GATE_NONE)
+    ws, plan = ctx.new_workspace(), ctx.new_plan()
+    count = torch.zeros(E, dtype=torch.int32, device=DEV)
+    ctx.uep_histogram(ids.to(DEV), count, ws)
+    ctx.uep_plan(count, plan, ws)
+    parent = torch.full((E + R * n_slot,), -5, dtype=torch.int32, device=DEV)
+    vol = torch.full((R,), -5, dtype=torch.int32, device=DEV)
+    ctx.uep_relay_plan(plan, parent, vol)
+    torch.cuda.synchronize()
+    lam, _ = oracle.histogram(ids.numpy(), E)
+    p = oracle.plan(lam, R, n_slot, um, S_total=T * k)
+    o_parent, o_vol = oracle.relay_plan(p)
+    assert np.array_equal(parent.cpu().numpy(), o_parent)
+    assert np.array_equal(vol.cpu().numpy(), o_vol)
