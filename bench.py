@@ -415,6 +415,7 @@ def run_uep(args):
                      "grad_reduce_bytes": int(statistics.mean(2 * (n_grp[i] + n_rep[i]) for i in range(n_red)) * g_elems * 4),
                      "grad_reduce_frac_of_peak": round(statistics.mean(2 * (n_grp[i] + n_rep[i]) for i in range(n_red))
                                                        * g_elems * 4 / (red_ms * 1e-3 / n_red) / 1e9 / peak_gbs, 4),
+                     "grad_reduce_traffic": traffic.get("grad_reduce_kernel"),
                      "inverse_remap_us": round(inv_ms * 1e3 / n_inst, 2),
                      "note": "uep_grad_reduce: fp32 [E, %d] main + [R, n_slot, %d] slot grads, bytes = 2 x (groups + replicas) x B; "
                              "uep_remap_inverse: 8 B/slot read, 4 B/slot scattered write" % (g_elems, g_elems)},

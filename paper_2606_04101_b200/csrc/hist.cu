@@ -5,7 +5,7 @@
 // per thread, 64 KB per SM), then counts into a WARP-PRIVATE shared-memory row (pitch E_pad+1
 // so the same expert in different rows falls into different banks): no contention between
 // warps on a hot expert, only the intra-warp multiplicity.  The CTA's row of the chunk table
-// (raw counts; uep_remap builds its own prefix over chunks from it) is written once.  The last
+// (raw counts, used only by this kernel's own reduction) is written once.  The last
 // CTA to finish (ticket) sums the table's columns with one round of independent int4 L2 loads
 // and emits expert_count.  Integer adds only: bit-identical run to run.
 #include "uep_internal.cuh"
