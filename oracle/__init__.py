@@ -280,3 +280,91 @@ def relay_plan(pl: Plan):
         for q in relays:
             vol[pl.inst_rank[q]] += leaves_of[q]
     return parent, vol.astype(np.int32)
+
+
+def source_rank(T: int, R: int) -> np.ndarray:
+    """S1: token i is routed by source rank floor(i*R/T) ("each rank computes gating for its local
+    tokens", PAPER.md:74)."""
+    return (np.arange(T, dtype=np.int64) * R // max(T, 1)).astype(np.int32)
+
+
+def reroute_split(Lam: np.ndarray, pl: Plan):
+    """O-8a SolveReroute (Alg. 1 lines 26-36; §5.2).  Lam[R,E] =
+    lambda_{r,e}.  Returns a list over experts of q_e[R, n_e] (n_e instances in the plan's CSR
+    order [main, replicas...]):
+      line 29   q[t,e,t] = min(lambda[t,e], u[e,t]) for every host rank t of e  (consume local quota)
+      lines 30-31   residual demand and residual quota
+      lines 32-34   the residual demand of every source is split over the residual quotas.  The
+                paper's round(lambda^ * u^/sum u^) cannot keep both marginals; reading S18: lay the
+                residual demands (ascending source rank) and the residual quotas (instance order)
+                on one number line and give q[r,e,t] the length of the overlap.  Both marginals
+                hold exactly and the split is deterministic."""
+    R, E = Lam.shape
+    out = []
+    for e in range(E):
+        lo, hi = int(pl.inst_off[e]), int(pl.inst_off[e + 1])
+        n = hi - lo
+        host = pl.inst_rank[lo:hi].astype(np.int64)
+        cum = pl.inst_cum[lo:hi].astype(np.int64)
+        u = np.diff(np.concatenate([[0], cum]))
+        lam = Lam[:, e].astype(np.int64)
+        q = np.zeros((R, n), dtype=np.int64)
+        lam_hat, u_hat = lam.copy(), u.copy()
+        for i in range(n):                                  # line 29
+            t = host[i]
+            q[t, i] = min(lam[t], u[i])
+            lam_hat[t] -= q[t, i]
+            u_hat[i] -= q[t, i]
+        d0 = np.concatenate([[0], np.cumsum(lam_hat)])      # number line of residual demands
+        u0 = np.concatenate([[0], np.cumsum(u_hat)])        # ... and of residual quotas
+        for r in range(R):
+            for i in range(n):
+                q[r, i] += max(0, min(d0[r + 1], u0[i + 1]) - max(d0[r], u0[i]))
+        out.append(q)
+    return out
+
+
+def remap_local(ids: np.ndarray, gate: np.ndarray | None, pl: Plan):
+    """O-8b source-aware token assignment (§5.2 "Token Assignment"): "the j-th local
+    token of pair (r, e) is sent to the first physical instance whose cumulative quota covers j",
+    cumulative over q[r,e,.] in instance order.  Receive order inside an instance (the paper leaves
+    it to the dispatch library; reading S25): by source rank ascending, then local order, so
+    offset = inst_base + sum_{r'<r} q[r',e,i] + (j - cumulative before i).
+    Returns (replica, rank, offset, out_gate, q_list, n_inflight[R])."""
+    ids32 = _i32(ids)
+    T, k = ids32.shape
+    E, R = pl.E, pl.R
+    flat = ids32.reshape(-1)
+    S = flat.size
+    src = np.repeat(source_rank(T, R), k)
+    valid = (flat >= 0) & (flat < E)
+    Lam = np.zeros((R, E), dtype=np.int64)
+    np.add.at(Lam, (src[valid], flat[valid]), 1)
+    qs = reroute_split(Lam, pl)
+    rep = np.full(S, -1, np.int32); rnk = np.full(S, -1, np.int32); off = np.full(S, -1, np.int32)
+    inst_base = np.asarray(pl.phys_base).reshape(R, -1)
+    order = np.argsort(np.where(valid, src.astype(np.int64) * E + flat, np.int64(R) * E), kind="stable")
+    keys = (src.astype(np.int64) * E + flat)[order]
+    nv = int(valid.sum())
+    bounds = np.flatnonzero(np.diff(np.concatenate([[-1], keys[:nv]]))).tolist() + [nv]
+    for a, b in zip(bounds[:-1], bounds[1:]):
+        r, e = divmod(int(keys[a]), E)
+        lo = int(pl.inst_off[e])
+        q = qs[e]
+        cum = np.cumsum(q[r])
+        j = np.arange(b - a)
+        i = np.searchsorted(cum, j, side="right")
+        before = np.concatenate([[0], cum])[i]
+        srcpre = q[:r].sum(axis=0)
+        sl = order[a:b]
+        rep[sl] = i
+        rnk[sl] = pl.inst_rank[lo + i]
+        off[sl] = inst_base[pl.inst_rank[lo + i], pl.inst_phys[lo + i]] + srcpre[i] + (j - before)
+    out_gate = None
+    if gate is not None:
+        g = np.ascontiguousarray(gate).reshape(-1)
+        out_gate = np.zeros(S, dtype=g.dtype)
+        out_gate[pl.rank_base[rnk[valid]] + off[valid]] = g[valid]
+    n_inflight = np.bincount(src[valid & (rnk != src)], minlength=R).astype(np.int32)
+    shp = ids32.shape
+    return rep.reshape(shp), rnk.reshape(shp), off.reshape(shp), out_gate, qs, n_inflight

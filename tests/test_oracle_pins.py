@@ -374,3 +374,58 @@ def test_relay_plan_pins():
             assert all(parent[q] != p.inst_rank[q] for q in reps)          # nobody relays to itself
         assert np.array_equal(kids, vol) and vol.sum() == p.n_replicas
         assert (parent[p.inst_off[-1]:] == -1).all()
+
+
+def test_reroute_split_and_local_remap_pins():
+    """O-8 against what the paper fixes: the hand-worked split below; both marginals of Q (Table 1,
+    PAPER.md:133-135: sum_t q = lambda_{r,e}, sum_r q = u_{e,t}); local quota consumed first
+    (Alg. 1 line 29); (rank, offset) a bijection onto the receive buffers with every instance
+    receiving exactly its quota; no replicas => identical to the global remap; and locality can only
+    lower the in-flight token count on the skewed example."""
+    # hand example: E=2 experts on R=2 ranks, expert 0 (home rank 0) split main 3 + replica@rank1 3
+    import types
+    pl = types.SimpleNamespace(E=2, R=2, inst_off=np.array([0, 2, 3]), inst_rank=np.array([0, 1, 1, -1]),
+                               inst_cum=np.array([3, 6, 2, 0]))
+    Lam = np.array([[4, 1], [2, 1]])
+    q0, q1 = oracle.reroute_split(Lam, pl)
+    assert q0.tolist() == [[3, 1], [0, 2]]      # r0: 3 local + 1 spills to the replica; r1: 2 local
+    assert q1.tolist() == [[1], [1]]
+    for s, seed in ((1.0, 5), (2.0, 6)):
+        T, k, E, R, ns = 8192, 4, 64, 16, 2
+        ids = synth.zipf_topk_ids(T, k, E, s, seed).numpy()
+        lam, _ = oracle.histogram(ids, E)
+        p = oracle.plan(lam, R, ns, 64)
+        assert p.n_replicas > 0
+        rep, rnk, off, _, qs, infl = oracle.remap_local(ids, None, p)
+        src = np.repeat(oracle.source_rank(T, R), k)
+        for e in range(E):
+            lo, hi = p.inst_off[e], p.inst_off[e + 1]
+            u = np.diff(np.concatenate([[0], p.inst_cum[lo:hi]]))
+            lam_re = np.bincount(src[ids.reshape(-1) == e], minlength=R)
+            assert np.array_equal(qs[e].sum(axis=1), lam_re) and np.array_equal(qs[e].sum(axis=0), u)
+            for i in range(hi - lo):
+                t = p.inst_rank[lo + i]
+                assert qs[e][t, i] >= min(lam_re[t], u[i])
+        dest = p.rank_base[rnk.reshape(-1)] + off.reshape(-1)      # bijection onto the receive buffers
+        assert np.array_equal(np.sort(dest), np.arange(ids.size))
+        for e in range(E):                                          # every instance receives its quota,
+            lo, hi = p.inst_off[e], p.inst_off[e + 1]               # in its own segment of its rank
+            sel = ids.reshape(-1) == e
+            u = np.diff(np.concatenate([[0], p.inst_cum[lo:hi]]))
+            assert np.array_equal(np.bincount(rep.reshape(-1)[sel], minlength=hi - lo), u)
+            for i in range(hi - lo):
+                m = sel & (rep.reshape(-1) == i)
+                t = p.inst_rank[lo + i]
+                b0 = p.phys_base[t, p.inst_phys[lo + i]]
+                assert (rnk.reshape(-1)[m] == t).all()
+                assert np.array_equal(np.sort(off.reshape(-1)[m]), b0 + np.arange(u[i]))
+        g_rep, g_rnk, g_off, _ = oracle.remap(ids, None, p)
+        assert infl.sum() == (rnk.reshape(-1) != src).sum()
+        assert infl.sum() <= (g_rnk.reshape(-1) != src).sum()
+    ids = synth.zipf_topk_ids(4096, 2, 16, 0.0, 9).numpy()            # balanced: no replicas
+    lam, _ = oracle.histogram(ids, 16)
+    p = oracle.plan(lam, 4, 1, 4096)
+    assert p.n_replicas == 0
+    a = oracle.remap_local(ids, None, p)
+    b = oracle.remap(ids, None, p)
+    assert all(np.array_equal(x, y) for x, y in zip(a[:3], b[:3]))
