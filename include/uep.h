@@ -184,6 +184,20 @@ int uep_remap_lookup(const uep_ctx* ctx, const void* gate, const uep_plan_out* p
                      int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
                      void* ws, void* stream);
 
+/* Source-aware reroute and token assignment (SolveReroute, Alg. 1 lines 26-36, PAPER.md:298-320;
+ * §5.2).  Token i belongs to source rank floor(i*R/T) (S1).  For every
+ * expert the solved quotas U are decomposed into q[r,e,t]: every host rank first consumes its own
+ * quota (line 29), the residual demand is spread over the residual quotas by the number-line
+ * overlap of DESIGN.md S18 (both marginals exact).  The j-th local slot of (r, e) goes to the first
+ * instance whose cumulative q[r,e,.] covers j; inside an instance tokens arrive ordered by source
+ * rank, then local order (S25), so (rank, offset) is again a bijection onto the receive buffers.
+ * Same arguments as uep_remap, plus
+ *   n_inflight  DEVICE int32 [R] or NULL: slots of source rank r sent to another rank.
+ * Needs T % R == 0 (else UEP_ERR_UNSUPPORTED).  Runs four kernels on `stream`; ws as for uep_remap. */
+int uep_remap_local(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
+                    const uep_plan_out* plan, int32_t* out_replica, int32_t* out_rank,
+                    int32_t* out_offset, void* out_gate, int32_t* n_inflight, void* ws, void* stream);
+
 /* Pack the state of every replicated expert into its destination slot:
  *   dst[j][(t*n_slot+s)*B_j .. +B_j) = src[j][e*B_j .. +B_j)  for x_{t,s} = e != empty.
  * Empty slots are not touched.  src/dst/bytes_per_expert: HOST arrays [n_tensors] of DEVICE

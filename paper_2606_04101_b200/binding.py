@@ -23,7 +23,8 @@ SC_TAU, SC_N_REPLICAS, SC_MAX_LOAD, SC_MAX_FANOUT, SC_N_PROBES, SC_N_INVALID, SC
     SC_TAU_HI0, SC_N_GROUPS = range(9)
 
 EXPORTS = ["uep_create", "uep_destroy", "uep_workspace_bytes", "uep_workspace_init",
-           "uep_plan_bytes", "uep_histogram", "uep_plan", "uep_plan_batched", "uep_remap", "uep_remap_rank",
+           "uep_plan_bytes", "uep_histogram", "uep_plan", "uep_plan_batched", "uep_remap", "uep_remap_local",
+           "uep_remap_rank",
            "uep_remap_lookup", "uep_remap_inverse", "uep_relay_plan", "uep_pack", "uep_grad_reduce",
            "uep_balance",
            "uep_balance_host", "uep_strerror", "uep_last_cuda_error", "uep_get_launch_info"]
@@ -222,6 +223,12 @@ class Context:
         assert plan.batch >= n_inst and expert_count.numel() >= n_inst * self.E
         _check(lib().uep_plan_batched(self._h, int(n_inst), _ptr(expert_count), ctypes.byref(plan.c),
                                       _stream(stream)))
+
+    def uep_remap_local(self, topk_ids, gate, plan: Plan, out_replica, out_rank, out_offset, out_gate,
+                        n_inflight, ws, stream=None):
+        _check(lib().uep_remap_local(self._h, _ptr(topk_ids), _ptr(gate), ctypes.byref(plan.c),
+                                     _ptr(out_replica), _ptr(out_rank), _ptr(out_offset),
+                                     _ptr(out_gate), _ptr(n_inflight), _ptr(ws), _stream(stream)))
 
     def uep_remap_rank(self, topk_ids, ws, stream=None):
         _check(lib().uep_remap_rank(self._h, _ptr(topk_ids), _ptr(ws), _stream(stream)))

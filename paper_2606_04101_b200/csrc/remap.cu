@@ -40,14 +40,18 @@ constexpr int kEMask = (1 << kPackedEBits) - 1;
 // rank_kernel.  dynamic shared memory: wrow[kRemapWarps][E_pad] (int2 {mask, count})
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kRemapThreads, 2)
-rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len,
-            int32_t* __restrict__ packed, int32_t* __restrict__ prefix) {
+rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len, int cpg,
+            int group_len, int32_t* __restrict__ packed, int32_t* __restrict__ prefix) {
   extern __shared__ __align__(16) int smem[];
   int2* wrow = reinterpret_cast<int2*>(smem);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
-  const long long cbegin = (long long)blockIdx.x * chunk_len;
-  const int clen = (int)min((long long)chunk_len, (long long)S - cbegin);      // <= kMaxChunk
+  // chunk c = sub-chunk c % cpg of group c / cpg (a group = one source rank's slots in the
+  // source-aware remap; the whole input, cpg = number of chunks, otherwise)
+  const int sub = (int)blockIdx.x % cpg;
+  const long long cbegin = (long long)((int)blockIdx.x / cpg) * group_len + (long long)sub * chunk_len;
+  const int clen = (int)min(min((long long)chunk_len, (long long)group_len - (long long)sub * chunk_len),
+                            (long long)S - cbegin);                            // <= kMaxChunk
   const int items = (clen + kRemapThreads - 1) / kRemapThreads;                // steps per warp
   const bool full = (clen == items * kRemapThreads);
   const int wbeg = warp * items * 32;
@@ -155,14 +159,114 @@ prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG) {
   }
 }
 
-int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s) {
+int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local) {
   if (c->S == 0) return UEP_OK;
+  const int chunks = local ? c->l_chunks : c->r_chunks;
   const size_t smem = sizeof(int2) * (size_t)kRemapWarps * c->E_pad;
-  rank_kernel<<<c->r_chunks, kRemapThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
-                                                      c->r_chunk_len, ws_packed(c, ws),
-                                                      ws_prefix(c, ws));
+  rank_kernel<<<chunks, kRemapThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
+                                                 local ? c->l_chunk_len : c->r_chunk_len,
+                                                 local ? c->l_cpg : c->r_chunks,
+                                                 local ? c->l_group_len : c->S, ws_packed(c, ws),
+                                                 ws_prefix(c, ws));
   UEP_CUDA_TRY(cudaGetLastError());
-  prefix_kernel<<<c->E_pad / 4, 1024, 0, s>>>(ws_prefix(c, ws), c->r_chunks, c->E_pad / 4);
+  prefix_kernel<<<c->E_pad / 4, 1024, 0, s>>>(ws_prefix(c, ws), chunks, c->E_pad / 4);
+  UEP_CUDA_TRY(cudaGetLastError());
+  return UEP_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// reroute_kernel: SolveReroute, Alg. 1 lines 26-36, one
+// CTA per expert.  lambda_{r,e} comes from the prefix table (difference of the rows at the source
+// rank's first and last chunk).  Line 29: every host rank first consumes its own quota.  Lines
+// 32-34 under reading S18: residual demands (ascending source rank) and residual quotas (instance
+// order) are laid on one number line, q[r,e,i] = overlap length (+ the local part): both marginals
+// exact, deterministic.  Emits, per source rank r and CSR instance p of the expert,
+//   cumq[r][p]   inclusive cumulative of q[r,e,.] in instance order   (the lookup table of §5.2)
+//   srcpre[r][p] sum of q[r',e,i] over r' < r                         (receive order: by source rank)
+// ------------------------------------------------------------------------------------------------
+constexpr int kRrThreads = 256;
+constexpr int kRrMaxInst = UEP_MAX_R + 1;
+
+__device__ __forceinline__ int rr_block_excl_scan(int v, int* tmp) {   // 256 threads; returns exclusive prefix
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int s = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int y = __shfl_up_sync(kFullMask, s, o);
+    if (lane >= o) s += y;
+  }
+  __syncthreads();
+  if (lane == 31) tmp[w] = s;
+  __syncthreads();
+  int pre = 0;
+  for (int q = 0; q < w; ++q) pre += tmp[q];
+  return pre + s - v;
+}
+
+__global__ void __launch_bounds__(kRrThreads)
+reroute_kernel(int E_pad, int R, int inst_cap, int cpg, const int32_t* __restrict__ prefix,
+               const int32_t* __restrict__ inst_off, const int32_t* __restrict__ inst_rank,
+               const int32_t* __restrict__ inst_cum, int32_t* __restrict__ cumq,
+               int32_t* __restrict__ srcpre, int32_t* __restrict__ n_inflight) {
+  __shared__ int lam[UEP_MAX_R], lamhat[UEP_MAX_R], d0[UEP_MAX_R + 1];
+  __shared__ int u[kRrMaxInst], uhat[kRrMaxInst], u0[kRrMaxInst + 1], host[kRrMaxInst], locq[kRrMaxInst];
+  __shared__ int tmp[8];
+  const int tid = threadIdx.x, e = blockIdx.x;
+  const int lo = inst_off[e], n = inst_off[e + 1] - lo;
+  if (e == 0 && n_inflight) for (int r = tid; r < R; r += kRrThreads) n_inflight[r] = 0;
+  if (tid < R) {
+    lam[tid] = __ldcg(prefix + (size_t)(tid + 1) * cpg * E_pad + e) - __ldcg(prefix + (size_t)tid * cpg * E_pad + e);
+    lamhat[tid] = lam[tid];
+  }
+  for (int i = tid; i < n; i += kRrThreads) {
+    host[i] = inst_rank[lo + i];
+    u[i] = inst_cum[lo + i] - (i ? inst_cum[lo + i - 1] : 0);
+  }
+  __syncthreads();
+  for (int i = tid; i < n; i += kRrThreads) {               // line 29: consume local quota
+    const int loc = min(lam[host[i]], u[i]);                // hosts of one expert are distinct ranks
+    locq[i] = loc;
+    uhat[i] = u[i] - loc;
+    lamhat[host[i]] -= loc;
+  }
+  __syncthreads();
+  {                                                          // number lines (exclusive prefixes)
+    const int v = (tid < R) ? lamhat[tid] : 0;
+    const int ex = rr_block_excl_scan(v, tmp);
+    if (tid < R) d0[tid] = ex;
+    if (tid == R - 1) d0[R] = ex + v;
+    __syncthreads();
+    const int w0 = (tid < n) ? uhat[tid] : 0;
+    const int ex2 = rr_block_excl_scan(w0, tmp);
+    if (tid < n) u0[tid] = ex2;
+    if (tid == min(n, kRrThreads) - 1) {
+      int run = ex2 + w0;
+      for (int i = kRrThreads; i < n; ++i) { u0[i] = run; run += uhat[i]; }   // n == 257 only
+      u0[n] = run;
+    }
+  }
+  __syncthreads();
+  auto q = [&](int r, int i) {
+    const int ov = min(d0[r + 1], u0[i + 1]) - max(d0[r], u0[i]);
+    return max(ov, 0) + (host[i] == r ? locq[i] : 0);
+  };
+  if (tid < R) {                                             // cumulative over instances, per source
+    int run = 0;
+    for (int i = 0; i < n; ++i) { run += q(tid, i); cumq[(size_t)tid * inst_cap + lo + i] = run; }
+  }
+  for (int i = tid; i < n; i += kRrThreads) {                // exclusive prefix over sources, per instance
+    int run = 0;
+    for (int r = 0; r < R; ++r) { srcpre[(size_t)r * inst_cap + lo + i] = run; run += q(r, i); }
+  }
+}
+
+int launch_reroute(const Ctx* c, const uep_plan_out& plan, int32_t* n_inflight, void* ws, cudaStream_t s) {
+  if (c->S == 0) return UEP_OK;
+  const int inst_cap = c->cfg.E + c->cfg.R * c->cfg.n_slot;
+  int32_t* cumq = ws_reroute(c, ws);
+  reroute_kernel<<<c->cfg.E, kRrThreads, 0, s>>>(c->E_pad, c->cfg.R, inst_cap, c->l_cpg, ws_prefix(c, ws),
+                                                plan.inst_off, plan.inst_rank, plan.inst_cum, cumq,
+                                                cumq + (size_t)c->cfg.R * inst_cap, n_inflight);
   UEP_CUDA_TRY(cudaGetLastError());
   return UEP_OK;
 }
@@ -181,7 +285,7 @@ __host__ __device__ inline size_t lookup_smem_bytes(int E_pad, int R, int inst_c
   return sizeof(int) * fixed + scratch;
 }
 
-template <typename GateT, bool STAGE>
+template <typename GateT, bool STAGE, bool LOCAL>
 __global__ void __launch_bounds__(kRemapThreads, 2)
 lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate, int S, int E,
               int E_pad, int R, int inst_cap, int chunk_len, const int32_t* __restrict__ prefix,
@@ -189,7 +293,14 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
               const int32_t* __restrict__ g_inst_cum, const int32_t* __restrict__ g_inst_base,
               const int32_t* __restrict__ g_rank_base, int32_t* __restrict__ out_replica,
               int32_t* __restrict__ out_rank, int32_t* __restrict__ out_offset,
-              GateT* __restrict__ out_gate) {
+              GateT* __restrict__ out_gate, int cpg, int group_len,
+              const int32_t* __restrict__ cumq, const int32_t* __restrict__ srcpre,
+              int32_t* __restrict__ n_inflight) {
+  // Source-aware mode (LOCAL): a group of cpg chunks is one source rank r;
+  // ranks are LOCAL to (r, e): base0 = prefix row of the chunk - prefix row of the group's first
+  // chunk, the cumulative quotas are row r of cumq (the split q[r,e,.] of SolveReroute) and an
+  // instance's base is inst_base + srcpre[r][.] (receive order: by source rank).  Everything else
+  // is the same lookup.
   extern __shared__ __align__(16) int smem[];
   int4* rec = reinterpret_cast<int4*>(smem);     // [E_pad] fast-path record per expert
   int* base0 = reinterpret_cast<int*>(rec + E_pad);   // [E_pad] global rank of the chunk's first slot of e
@@ -207,8 +318,12 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int c = blockIdx.x;
-  const long long cbegin = (long long)c * chunk_len;
-  const int clen = (int)min((long long)chunk_len, (long long)S - cbegin);
+  constexpr bool local = LOCAL;
+  const int grp = LOCAL ? c / cpg : 0, sub = LOCAL ? c % cpg : c;
+  const long long cbegin = (long long)grp * group_len + (long long)sub * chunk_len;
+  const int clen = LOCAL ? (int)min(min((long long)chunk_len, (long long)group_len - (long long)sub * chunk_len),
+                                    (long long)S - cbegin)
+                         : (int)min((long long)chunk_len, (long long)S - cbegin);
   const int items = (clen + kRemapThreads - 1) / kRemapThreads;
   const bool full = (clen == items * kRemapThreads);
   const int wbeg = warp * items * 32;
@@ -228,8 +343,9 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   }
 
   // ---- chunk base ranks: row c of the exclusive prefix over chunks that rank_kernel left ----------
-  const int b0_own = (tid < E) ? __ldcg(prefix + (size_t)c * E_pad + tid) : 0;
-  const int n_own = (tid < E) ? __ldcg(prefix + (size_t)(c + 1) * E_pad + tid) - b0_own : 0;
+  const int p_own = (tid < E) ? __ldcg(prefix + (size_t)c * E_pad + tid) : 0;
+  const int n_own = (tid < E) ? __ldcg(prefix + (size_t)(c + 1) * E_pad + tid) - p_own : 0;
+  const int b0_own = (local && tid < E) ? p_own - __ldcg(prefix + (size_t)grp * cpg * E_pad + tid) : p_own;
   int el_inc = n_own;                            // inclusive scan of n_own over experts
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
@@ -243,10 +359,10 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   for (int e = tid; e <= E; e += kRemapThreads) s_off[e] = g_inst_off[e];
   for (int r = tid; r <= R; r += kRemapThreads) rbase[r] = g_rank_base[r];
   for (int p = tid; p < inst_cap; p += kRemapThreads) {
-    const int cum = g_inst_cum[p];
+    const int cum = local ? __ldcg(cumq + (size_t)grp * inst_cap + p) : g_inst_cum[p];
     i_cum[p] = cum;
     i_rank[p] = g_inst_rank[p];
-    i_gbase[p] = g_inst_base[p];                 // raw inst_base for now
+    i_gbase[p] = g_inst_base[p] + (local ? __ldcg(srcpre + (size_t)grp * inst_cap + p) : 0);   // raw base for now
     if (p + 1 < inst_cap) i_dbase[p + 1] = cum;  // cum_prev of the next entry
     if (p == 0) i_dbase[0] = 0;
   }
@@ -280,6 +396,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   }
   __syncthreads();
 
+  int n_fly = 0;
   // two slots at a time: their records are loaded before any of them stores to shared memory
   // (the compiler cannot prove that the staging stores do not alias the records)
 #pragma unroll
@@ -324,9 +441,14 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
           out_replica[i * 32] = rep;
           out_rank[i * 32] = rk;
           out_offset[i * 32] = of;
+          if (LOCAL) n_fly += (rk >= 0 && rk != grp) ? 1 : 0;
         }
       }
     }
+  }
+  if (local && n_inflight) {                             // tokens of source rank grp that leave it
+    n_fly = __reduce_add_sync(kFullMask, n_fly);
+    if (lane == 0 && n_fly) atomicAdd(n_inflight + grp, n_fly);
   }
 
   if (STAGE && has_gate) {                               // staged gates leave as contiguous runs
@@ -343,14 +465,16 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
 template <typename GateT>
 static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& p,
                            int32_t* out_replica, int32_t* out_rank, int32_t* out_offset,
-                           GateT* out_gate, void* ws, cudaStream_t s, bool pdl) {
+                           GateT* out_gate, void* ws, cudaStream_t s, bool pdl, bool local,
+                           int32_t* n_inflight) {
   const uep_config& g = c->cfg;
   const int inst_cap = g.E + g.R * g.n_slot;
   const bool stage = gate != nullptr;
   const size_t smem = lookup_smem_bytes(c->E_pad, g.R, inst_cap, stage, sizeof(GateT));
-  auto k = stage ? lookup_kernel<GateT, true> : lookup_kernel<GateT, false>;
+  auto k = local ? (stage ? lookup_kernel<GateT, true, true> : lookup_kernel<GateT, false, true>)
+                 : (stage ? lookup_kernel<GateT, true, false> : lookup_kernel<GateT, false, false>);
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(c->r_chunks);
+  cfg.gridDim = dim3(local ? c->l_chunks : c->r_chunks);
   cfg.blockDim = dim3(kRemapThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = s;
@@ -359,12 +483,16 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = pdl ? 1 : 0;
+  const int32_t* cumq = local ? ws_reroute(c, ws) : nullptr;
+  const int32_t* srcpre = local ? cumq + (size_t)g.R * inst_cap : nullptr;
   UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, k, (const int32_t*)ws_packed(c, ws), gate, c->S, g.E, c->E_pad,
-                                  g.R, inst_cap, c->r_chunk_len, (const int32_t*)ws_prefix(c, ws),
+                                  g.R, inst_cap, local ? c->l_chunk_len : c->r_chunk_len,
+                                  (const int32_t*)ws_prefix(c, ws),
                                   (const int32_t*)p.inst_off, (const int32_t*)p.inst_rank,
                                   (const int32_t*)p.inst_cum, (const int32_t*)p.inst_base,
                                   (const int32_t*)p.rank_base, out_replica, out_rank, out_offset,
-                                  out_gate));
+                                  out_gate, local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S,
+                                  cumq, srcpre, n_inflight));
   return UEP_OK;
 }
 
@@ -372,22 +500,26 @@ int init_remap_kernels() {
   const int rank_bytes = (int)(sizeof(int2) * (size_t)kRemapWarps * UEP_MAX_E);
   const int bytes = (int)lookup_smem_bytes(UEP_MAX_E, UEP_MAX_R, UEP_MAX_E + UEP_MAX_R * UEP_MAX_NSLOT, true, 4);
   UEP_CUDA_TRY(cudaFuncSetAttribute(rank_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rank_bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint16_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint16_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint16_t, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint16_t, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint16_t, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint16_t, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   return UEP_OK;
 }
 
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& p, int32_t* out_replica,
                   int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
-                  bool pdl) {
+                  bool pdl, bool local, int32_t* n_inflight) {
   if (c->S == 0) return UEP_OK;
   if (c->cfg.gate_dtype == UEP_GATE_BF16 && gate)
     return launch_lookup_t<uint16_t>(c, static_cast<const uint16_t*>(gate), p, out_replica, out_rank,
-                                     out_offset, static_cast<uint16_t*>(out_gate), ws, s, pdl);
+                                     out_offset, static_cast<uint16_t*>(out_gate), ws, s, pdl, local, n_inflight);
   return launch_lookup_t<uint32_t>(c, static_cast<const uint32_t*>(gate), p, out_replica, out_rank,
-                                   out_offset, static_cast<uint32_t*>(out_gate), ws, s, pdl);
+                                   out_offset, static_cast<uint32_t*>(out_gate), ws, s, pdl, local, n_inflight);
 }
 
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& p,
@@ -395,7 +527,7 @@ int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_p
                  void* ws, cudaStream_t s) {
   int rc = launch_rank(c, ids, ws, s);
   if (rc != UEP_OK) return rc;
-  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s, false);
+  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s, false, false, nullptr);
 }
 
 }  // namespace uep

@@ -122,6 +122,18 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
     rper = std::min<long long>(rper, kMaxChunk);
     c->r_chunk_len = (int)rper;
     c->r_chunks = (int)std::max<long long>(1, (S + rper - 1) / rper);
+    // source-aware geometry: every source rank's block of (T/R)*k slots is cut into l_cpg chunks
+    c->l_cpg = c->l_chunk_len = c->l_chunks = c->l_group_len = 0;
+    if (cfg->T > 0 && cfg->T % R == 0) {
+      const long long block = (long long)(cfg->T / R) * cfg->k;
+      const long long cpg = (block + kMaxChunk - 1) / kMaxChunk;
+      long long len = (block + cpg - 1) / cpg;
+      len = std::min<long long>((len + 31) / 32 * 32, kMaxChunk);
+      c->l_cpg = (int)cpg;
+      c->l_chunk_len = (int)len;
+      c->l_chunks = (int)(cpg * R);
+      c->l_group_len = (int)block;
+    }
   }
   c->pack_ctas = c->sm_count;
 
@@ -168,7 +180,8 @@ void uep_destroy(uep_ctx* ctx) {
 size_t uep_workspace_bytes(const uep_ctx* ctx) {
   const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
   if (!c) return 0;
-  return (size_t)kWsHeaderBytes + ws_table_bytes(c) + ws_prefix_bytes(c) + sizeof(int32_t) * (((size_t)c->S + 63) & ~(size_t)63);
+  return (size_t)kWsHeaderBytes + ws_table_bytes(c) + ws_prefix_bytes(c) + ws_packed_bytes(c) +
+         sizeof(int32_t) * ws_reroute_ints(c);
 }
 
 int uep_workspace_init(const uep_ctx* ctx, void* ws, void* stream) {
@@ -311,6 +324,25 @@ int uep_pack(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,
   if (rc != UEP_OK) return rc;
   if (n_tensors == 0 || c->cfg.n_slot == 0) return UEP_OK;
   return launch_pack(c, *plan, a, static_cast<cudaStream_t>(stream));
+}
+
+int uep_remap_local(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
+                    const uep_plan_out* plan, int32_t* out_replica, int32_t* out_rank,
+                    int32_t* out_offset, void* out_gate, int32_t* n_inflight, void* ws, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c) return UEP_ERR_INVALID_ARG;
+  if (c->S > 0 && c->l_cpg == 0) return UEP_ERR_UNSUPPORTED;           // T must be a multiple of R
+  int rc = check_remap_outputs(c, gate, plan, out_replica, out_rank, out_offset, out_gate, ws);
+  if (rc != UEP_OK) return rc;
+  if (c->S > 0 && (!topk_ids || !aligned16(topk_ids))) return UEP_ERR_INVALID_ARG;
+  if (n_inflight && !aligned16(n_inflight)) return UEP_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  rc = launch_rank(c, topk_ids, ws, s, /*local=*/true);
+  if (rc == UEP_OK) rc = launch_reroute(c, *plan, n_inflight, ws, s);
+  if (rc == UEP_OK)
+    rc = launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s, false,
+                       /*local=*/true, n_inflight);
+  return rc;
 }
 
 int uep_grad_reduce(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,

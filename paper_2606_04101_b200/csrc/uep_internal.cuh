@@ -33,6 +33,10 @@ struct Ctx {
   int E_pad;              // E rounded up to a multiple of 4 (row pitch of the chunk table)
   int n_chunks, chunk_len;        // histogram geometry: one CTA per chunk, one chunk per SM
   int r_chunks, r_chunk_len;      // remap geometry (rank + lookup kernels): <= kMaxChunk slots per CTA
+  // source-aware remap (uep_remap_local): chunks never straddle a source rank's block of T/R
+  // tokens; l_cpg chunks per source rank, the last one of a block may be shorter.  l_cpg == 0:
+  // unsupported shape (T not a multiple of R)
+  int l_cpg, l_chunk_len, l_chunks, l_group_len;
   int sm_count;
   int pack_ctas;
   int plan_cluster;       // CTAs per plan solve (thread-block cluster size)
@@ -60,10 +64,11 @@ int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cu
                 bool pdl = false, int n_inst = 1);
 // uep_remap = launch_rank (plan-independent: stable rank of every slot inside its chunk, packed
 // with the expert id into the workspace) + launch_lookup (plan-dependent: cumulative-quota lookup).
-int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s);
+int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local = false);
+int launch_reroute(const Ctx* c, const uep_plan_out& plan, int32_t* n_inflight, void* ws, cudaStream_t s);
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& plan, int32_t* out_replica,
                   int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
-                  bool pdl = false);
+                  bool pdl = false, bool local = false, int32_t* n_inflight = nullptr);
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& plan,
                  int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
                  void* ws, cudaStream_t s);
@@ -128,8 +133,15 @@ inline unsigned* ws_ticket(void* ws) { return reinterpret_cast<unsigned*>(ws); }
 inline size_t ws_table_bytes(const Ctx* c) {
   return (sizeof(int32_t) * (size_t)c->n_chunks * c->E_pad + 255) & ~(size_t)255;
 }
-inline size_t ws_prefix_bytes(const Ctx* c) {            // [r_chunks + 1][E_pad]
-  return (sizeof(int32_t) * ((size_t)c->r_chunks + 1) * c->E_pad + 255) & ~(size_t)255;
+inline size_t ws_prefix_bytes(const Ctx* c) {            // [max(r_chunks, l_chunks) + 1][E_pad]
+  const size_t rows = (size_t)(c->r_chunks > c->l_chunks ? c->r_chunks : c->l_chunks) + 1;
+  return (sizeof(int32_t) * rows * c->E_pad + 255) & ~(size_t)255;
+}
+inline size_t ws_packed_bytes(const Ctx* c) {
+  return sizeof(int32_t) * (((size_t)c->S + 63) & ~(size_t)63);
+}
+inline size_t ws_reroute_ints(const Ctx* c) {             // cumq and srcpre: [R][E + R*n_slot] each
+  return c->l_cpg ? 2 * (size_t)c->cfg.R * (size_t)(c->cfg.E + c->cfg.R * c->cfg.n_slot) : 0;
 }
 inline int32_t* ws_prefix(const Ctx* c, void* ws) {      // exclusive prefix over remap chunks (+ totals row)
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c));
@@ -137,6 +149,10 @@ inline int32_t* ws_prefix(const Ctx* c, void* ws) {      // exclusive prefix ove
 inline int32_t* ws_packed(const Ctx* c, void* ws) {      // [S] packed (expert, rank in chunk)
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c) +
                                     ws_prefix_bytes(c));
+}
+inline int32_t* ws_reroute(const Ctx* c, void* ws) {     // source-aware split tables (uep_remap_local)
+  return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c) +
+                                    ws_prefix_bytes(c) + ws_packed_bytes(c));
 }
 
 }  // namespace uep

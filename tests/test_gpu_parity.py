@@ -479,3 +479,40 @@ def test_relay_plan_parity(T, k, E, R, n_slot, dist):
     o_parent, o_vol = oracle.relay_plan(p)
     assert np.array_equal(parent.cpu().numpy(), o_parent)
     assert np.array_equal(vol.cpu().numpy(), o_vol)
+
+
+@pytest.mark.parametrize("T,k,E,R,n_slot,s,gate_bf16", [
+    (4096, 2, 16, 4, 1, 1.2, False),         # tiny config
+    (8192, 4, 64, 16, 2, 2.0, True),         # the oracle-pin shape, bf16 gates
+    (65536, 8, 128, 32, 2, 1.0, False),      # GLM-Air-like: two chunks per source rank
+    (4096, 8, 512, 256, 4, 2.0, False),      # R = 256: 16 tokens per source rank
+    (262144, 8, 256, 64, 2, 1.0, False),     # DeepSeek-V3 prefill at full size
+])
+def test_remap_local_parity(T, k, E, R, n_slot, s, gate_bf16):
+    """NEXT-1: source-aware reroute + token assignment, bit-exact against the oracle (O-8)."""
+    um = synth.stress_u_min(T * k, R) if T * k < 2000000 else 1024
+    ids = synth.zipf_topk_ids(T, k, E, s, 123)
+    gate = synth.gates_softmax_bf16(T, k, 4) if gate_bf16 else synth.gates_uniform_renorm(T, k, 4)
+    gd = binding.GATE_BF16 if gate_bf16 else binding.GATE_F32
+    ctx = binding.Context(T, k, E, R, n_slot, um, gate_dtype=gd)
+    ws, plan = ctx.new_workspace(), ctx.new_plan()
+    d_ids, d_gate = ids.to(DEV), gate.to(DEV)
+    count = torch.zeros(E, dtype=torch.int32, device=DEV)
+    ctx.uep_histogram(d_ids, count, ws)
+    ctx.uep_plan(count, plan, ws)
+    rep, rnk, off, og = ctx.new_outputs(d_gate)
+    infl = torch.full((R,), -3, dtype=torch.int32, device=DEV)
+    ctx.uep_remap_local(d_ids, d_gate, plan, rep, rnk, off, og, infl, ws)
+    torch.cuda.synchronize()
+    lam, _ = oracle.histogram(ids.numpy(), E)
+    p = oracle.plan(lam, R, n_slot, um, S_total=T * k)
+    gbits = gate.view(torch.int16).numpy().view(np.uint16) if gate_bf16 \
+        else gate.view(torch.int32).numpy().view(np.uint32)
+    o_rep, o_rnk, o_off, o_og, _, o_infl = oracle.remap_local(ids.numpy(), gbits, p)
+    assert np.array_equal(rep.cpu().numpy(), o_rep)
+    assert np.array_equal(rnk.cpu().numpy(), o_rnk)
+    assert np.array_equal(off.cpu().numpy(), o_off)
+    got = og.cpu()
+    got = got.view(torch.int16).numpy().view(np.uint16) if gate_bf16 else got.view(torch.int32).numpy().view(np.uint32)
+    assert np.array_equal(got, o_og)
+    assert np.array_equal(infl.cpu().numpy(), o_infl)
