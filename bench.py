@@ -340,6 +340,30 @@ def run_uep(args):
     g_inv = capture([lambda i=i: rig.ctx.uep_remap_inverse(rig.outs[i][1], rig.outs[i][2], rig.plans[i], out_src)
                      for i in range(n_inst)], stream)
     inv_ms, _ = time_graph(g_inv, stream, reps)
+    # NEXT-1: source-aware reroute; in-flight token ratio against the global remap
+    local = None
+    if c["T"] % c["R"] == 0:
+        infl = [_t.zeros(c["R"], dtype=_t.int32, device=device) for _ in range(n_inst)]
+        src_rank = (_t.arange(c["T"], device=device, dtype=_t.int64) * c["R"] // c["T"]).to(_t.int32)
+        glob_fly = []
+        for i in range(min(n_inst, 4)):      # the global remap's outputs are still in rig.outs
+            glob_fly.append(int((rig.outs[i][1] != src_rank[:, None]).sum()))
+        g_loc = capture([lambda i=i: rig.ctx.uep_remap_local(rig.ids[i], rig.gates[i], rig.plans[i], rig.outs[i][0],
+                                                            rig.outs[i][1], rig.outs[i][2], rig.outs[i][3],
+                                                            infl[i], rig.ws[i]) for i in range(n_inst)], stream)
+        loc_ms, _ = time_graph(g_loc, stream, reps)
+        loc_fly = [int(infl[i].sum()) for i in range(min(n_inst, 4))]
+        S_all = c["T"] * c["k"]
+        local = {"remap_local_us": round(loc_ms * 1e3 / n_inst, 2),
+                 "inflight_ratio_global": round(statistics.mean(glob_fly) / S_all, 4),
+                 "inflight_ratio_local": round(statistics.mean(loc_fly) / S_all, 4),
+                 "note": "uep_remap_local = rank + prefix + reroute + lookup on one stream; in-flight = slots whose "
+                         "destination rank differs from their source rank floor(i*R/T) (paper: 96.0 % vs 98.4 %, "
+                         "PAPER.md:440, its own traces)"}
+        with _t.cuda.stream(stream):         # leave the global remap's outputs in place again
+            for i in range(n_inst):
+                rig.remap(i)
+        stream.synchronize()
     clocks = sampler.stop()
     chain_ms = barrier_and_max(world, chain_ms, device)
     # whole-job aggregate: `world` ranks each planned n_inst layers in chain_ms (max over ranks)
@@ -419,6 +443,7 @@ def run_uep(args):
                      "inverse_remap_us": round(inv_ms * 1e3 / n_inst, 2),
                      "note": "uep_grad_reduce: fp32 [E, %d] main + [R, n_slot, %d] slot grads, bytes = 2 x (groups + replicas) x B; "
                              "uep_remap_inverse: 8 B/slot read, 4 B/slot scattered write" % (g_elems, g_elems)},
+        "source_aware_remap": local,
         "roofline": {k: r_pack[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")},
         "rooflines": rooflines,
         "gpu_launches": 6 * K,
