@@ -386,11 +386,16 @@ int uep_remap_inverse(const uep_ctx* ctx, const int32_t* out_rank, const int32_t
   return launch_inverse(c, out_rank, out_offset, *plan, out_src, static_cast<cudaStream_t>(stream));
 }
 
-int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
-                int32_t* expert_count, const uep_plan_out* plan, int32_t* out_replica,
-                int32_t* out_rank, int32_t* out_offset, void* out_gate, int32_t n_tensors,
-                const void* const* src, const size_t* bytes_per_expert, void* const* dst,
-                void* ws, void* stream) {
+}  // extern "C"
+
+// uep_balance proper.  join_pack = false leaves the side stream (pack) un-joined: the caller
+// enqueues more work on `stream` first and then waits on ctx->ev_join itself (uep_balance_host
+// overlaps its device->host copies with the pack that way).
+static int balance_impl(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
+                        int32_t* expert_count, const uep_plan_out* plan, int32_t* out_replica,
+                        int32_t* out_rank, int32_t* out_offset, void* out_gate, int32_t n_tensors,
+                        const void* const* src, const size_t* bytes_per_expert, void* const* dst,
+                        void* ws, void* stream, bool join_pack) {
   const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
   if (!c) return UEP_ERR_INVALID_ARG;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -435,8 +440,19 @@ int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
   UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_rank, 0));          // join the rank kernel
   if (rc == UEP_OK && rc2 == UEP_OK)
     rc2 = launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s, /*pdl=*/true);
-  UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_join, 0));          // join the side stream (pack)
+  if (join_pack) UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_join, 0));   // join the side stream (pack)
   return rc != UEP_OK ? rc : rc2;
+}
+
+extern "C" {
+
+int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
+                int32_t* expert_count, const uep_plan_out* plan, int32_t* out_replica,
+                int32_t* out_rank, int32_t* out_offset, void* out_gate, int32_t n_tensors,
+                const void* const* src, const size_t* bytes_per_expert, void* const* dst,
+                void* ws, void* stream) {
+  return balance_impl(ctx, topk_ids, gate, expert_count, plan, out_replica, out_rank, out_offset,
+                      out_gate, n_tensors, src, bytes_per_expert, dst, ws, stream, true);
 }
 
 int uep_balance_host(const uep_ctx* ctx, const int32_t* topk_ids_host, const void* gate_host,
@@ -454,15 +470,18 @@ int uep_balance_host(const uep_ctx* ctx, const int32_t* topk_ids_host, const voi
   UEP_CUDA_TRY(cudaMemcpyAsync(dev_topk_ids, topk_ids_host, S * 4, cudaMemcpyHostToDevice, s));
   const bool has_gate = gate_host && dev_gate && gb;
   if (has_gate) UEP_CUDA_TRY(cudaMemcpyAsync(dev_gate, gate_host, S * gb, cudaMemcpyHostToDevice, s));
-  int rc = uep_balance(ctx, dev_topk_ids, has_gate ? dev_gate : nullptr, expert_count, plan,
-                       out_replica, out_rank, out_offset, has_gate ? out_gate : nullptr, n_tensors,
-                       src, bytes_per_expert, dst, ws, stream);
-  if (rc != UEP_OK) return rc;
+  // the pack (side stream) is joined only after the device->host copies are enqueued: the copies
+  // of the remap outputs run over PCIe while the pack streams HBM
+  int rc = balance_impl(ctx, dev_topk_ids, has_gate ? dev_gate : nullptr, expert_count, plan,
+                        out_replica, out_rank, out_offset, has_gate ? out_gate : nullptr, n_tensors,
+                        src, bytes_per_expert, dst, ws, stream, /*join_pack=*/false);
+  if (rc != UEP_OK) { cudaStreamWaitEvent(s, c->ev_join, 0); return rc; }
   if (out_replica_host) UEP_CUDA_TRY(cudaMemcpyAsync(out_replica_host, out_replica, S * 4, cudaMemcpyDeviceToHost, s));
   if (out_rank_host) UEP_CUDA_TRY(cudaMemcpyAsync(out_rank_host, out_rank, S * 4, cudaMemcpyDeviceToHost, s));
   if (out_offset_host) UEP_CUDA_TRY(cudaMemcpyAsync(out_offset_host, out_offset, S * 4, cudaMemcpyDeviceToHost, s));
   if (has_gate && out_gate_host) UEP_CUDA_TRY(cudaMemcpyAsync(out_gate_host, out_gate, S * gb, cudaMemcpyDeviceToHost, s));
   if (scalars_host) UEP_CUDA_TRY(cudaMemcpyAsync(scalars_host, plan->scalars, sizeof(int32_t) * UEP_N_SCALARS, cudaMemcpyDeviceToHost, s));
+  UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_join, 0));          // join the side stream (pack)
   UEP_CUDA_TRY(cudaStreamSynchronize(s));
   return UEP_OK;
 }

@@ -516,3 +516,38 @@ def test_remap_local_parity(T, k, E, R, n_slot, s, gate_bf16):
     got = got.view(torch.int16).numpy().view(np.uint16) if gate_bf16 else got.view(torch.int32).numpy().view(np.uint32)
     assert np.array_equal(got, o_og)
     assert np.array_equal(infl.cpu().numpy(), o_infl)
+
+
+def test_balance_host_end_to_end():
+    """uep_balance_host (the bench's e2e leg): pinned HOST ids and gates in, HOST remap outputs and
+    scalars back, expert state packed meanwhile; the device->host copies overlap the pack."""
+    T, k, E, R, ns, um = 32768, 8, 128, 32, 2, 256
+    ids = synth.zipf_topk_ids(T, k, E, 1.2, 8)
+    gate = synth.gates_uniform_renorm(T, k, 8)
+    state = synth.expert_state(E, 1 << 18, 2)
+    ctx = binding.Context(T, k, E, R, ns, um)
+    ws, plan = ctx.new_workspace(), ctx.new_plan()
+    h_ids, h_gate = ids.pin_memory(), gate.pin_memory()
+    d_ids, d_gate = torch.empty_like(ids, device=DEV), torch.empty_like(gate, device=DEV)
+    count = torch.zeros(E, dtype=torch.int32, device=DEV)
+    rep, rnk, off, og = ctx.new_outputs(d_gate)
+    pin = lambda t: torch.empty(t.shape, dtype=t.dtype).pin_memory()
+    h_rep, h_rnk, h_off, h_og = pin(rep), pin(rnk), pin(off), pin(og)
+    h_sc = torch.zeros(16, dtype=torch.int32).pin_memory()
+    d_state = state.to(DEV)
+    dst = torch.zeros((R, ns, state.shape[1]), dtype=state.dtype, device=DEV)
+    torch.cuda.synchronize()
+    stream = torch.cuda.Stream()
+    for _ in range(2):                                        # twice: the side stream is re-joined
+        ctx.uep_balance_host(h_ids, h_gate, d_ids, d_gate, count, plan, rep, rnk, off, og, h_rep, h_rnk,
+                             h_off, h_og, h_sc, [d_state], [dst], ws, stream)
+    lam, _ = oracle.histogram(ids.numpy(), E)
+    p = oracle.plan(lam, R, ns, um, S_total=T * k)
+    o_rep, o_rnk, o_off, o_og = oracle.remap(ids.numpy(), gate.numpy().view(np.uint32), p)
+    assert np.array_equal(h_rep.numpy(), o_rep) and np.array_equal(h_rnk.numpy(), o_rnk)
+    assert np.array_equal(h_off.numpy(), o_off)
+    assert np.array_equal(h_og.numpy().view(np.uint32), o_og)
+    assert np.array_equal(h_sc.numpy(), p.scalars)
+    ref = np.zeros((R, ns, state.shape[1]), dtype=np.int16)
+    oracle.pack(p.slot_expert, state.view(torch.int16).numpy(), ref)
+    assert np.array_equal(dst.cpu().view(torch.int16).numpy(), ref)   # uep_balance_host returned after the pack
