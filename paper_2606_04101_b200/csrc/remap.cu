@@ -16,6 +16,10 @@
 //                 programmatic dependent launch everything before its griddepcontrol.wait (packed
 //                 ranks, gates, prefix rows) overlaps the planner.
 //
+// The source-aware variant (uep_remap_local, SolveReroute of Alg. 1 lines 26-36) reuses the same
+// kernels on chunks that never straddle a source rank's block of tokens, with reroute_kernel
+// (below) in between to decompose the quotas per source rank.
+//
 // rank_kernel: one CTA per chunk (<= 8192 slots, register-resident, two CTAs per SM), every warp owns a
 // contiguous span and loads its ids up front (coalesced).  Ranking inside a warp uses a
 // warp-private shared-memory row of {peer mask, count} cells: lanes OR their lane bit into the
