@@ -31,6 +31,12 @@ __host__ __device__ inline size_t hist_smem_ints(int E_pad) {
   return (size_t)kHistWarps * (E_pad + 1) + kColPartInts + E_pad;
 }
 
+// RED = false: the CTA's row goes to the chunk table, the last CTA (ticket) sums the columns into
+// expert_count.  RED = true (uep_balance): the ticket, the fence and the last CTA's serial pass cost
+// 4.8 of the kernel's 9.4 us at the DeepSeek-V3 shape, so every CTA instead adds its counts to an
+// accumulator in the workspace with fire-and-forget reductions (integer adds: order-free) and
+// exits; the planner reads the accumulator, publishes expert_count and clears it.
+template <bool RED>
 __global__ void __launch_bounds__(kHistThreads, 1)
 hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len,
             int n_chunks, int32_t* __restrict__ table, unsigned* __restrict__ ticket,
@@ -84,8 +90,10 @@ hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
     int s = 0;
 #pragma unroll 8
     for (int w = 0; w < kHistWarps; ++w) s += priv[w * pitch + e];
-    grow[e] = s;
+    if (RED) { if (s != 0 && e < E) atomicAdd(expert_count + e, s); }   // expert_count = the accumulator
+    else grow[e] = s;
   }
+  if (RED) return;
   __syncthreads();                   // the CTA's row is written (barrier orders it before thread 0's fence)
   if (tid == 0) {
     __threadfence();                 // cumulative: makes the whole row visible before the ticket
@@ -110,19 +118,27 @@ __global__ void hist_empty_kernel(int E, int E_pad, int32_t* table, int32_t* exp
 }
 
 int init_hist_kernels() {
-  UEP_CUDA_TRY(cudaFuncSetAttribute(hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  UEP_CUDA_TRY(cudaFuncSetAttribute(hist_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)(sizeof(int) * (hist_smem_ints(UEP_MAX_E) + 4))));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(hist_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(sizeof(int) * (hist_smem_ints(UEP_MAX_E) + 4))));
   return UEP_OK;
 }
 
-int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s) {
+int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s,
+                     bool red) {
   if (c->S == 0) {
-    hist_empty_kernel<<<1, 256, 0, s>>>(c->cfg.E, c->E_pad, ws_table(ws), count);
+    if (!red) hist_empty_kernel<<<1, 256, 0, s>>>(c->cfg.E, c->E_pad, ws_table(ws), count);
   } else {
     const size_t smem = sizeof(int) * (hist_smem_ints(c->E_pad) + 4);
-    hist_kernel<<<c->n_chunks, kHistThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
-                                                        c->chunk_len, c->n_chunks, ws_table(ws),
-                                                        ws_ticket(ws), count);
+    if (red)
+      hist_kernel<true><<<c->n_chunks, kHistThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
+                                                                c->chunk_len, c->n_chunks, ws_table(ws),
+                                                                ws_ticket(ws), ws_acc(ws));
+    else
+      hist_kernel<false><<<c->n_chunks, kHistThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
+                                                                 c->chunk_len, c->n_chunks, ws_table(ws),
+                                                                 ws_ticket(ws), count);
   }
   UEP_CUDA_TRY(cudaGetLastError());
   return UEP_OK;

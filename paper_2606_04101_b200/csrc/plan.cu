@@ -177,7 +177,9 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
             const int32_t* __restrict__ g_main_phys, const int32_t* __restrict__ g_roff,
             const int32_t* __restrict__ g_rexp, uep_plan_out out, int E, int R, int n_slot, int M,
             int P, int u_min, int beta_num, int beta_den, int strict_i, int S_total, int n_bufs,
-            int log_cap, int levels) {
+            int log_cap, int levels, const int32_t* __restrict__ acc, int32_t* __restrict__ count_out) {
+  // acc != nullptr (uep_balance): lambda_e comes from the histogram's accumulator in the workspace
+  // and the CTA that emits the plan also publishes it as expert_count (count_out)
   cg::cluster_group cluster = cg::this_cluster();
   const int csize = (int)cluster.num_blocks(), crank = (int)cluster.block_rank();
   // batched solve (uep_plan_batched): cluster b solves instance b; every array of instance b
@@ -205,7 +207,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   }
   if (tid <= R) sm.roff[tid] = g_roff[tid];
   pdl_wait();                      // the histogram (preceding kernel) is complete
-  if (tid < E) sm.lam[tid] = expert_count[tid];
+  if (tid < E) sm.lam[tid] = acc ? __ldcg(acc + tid) : expert_count[tid];
   __syncthreads();
   // line 2: l_r
   if (tid < R) {
@@ -370,6 +372,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   const int log_node = sm.log_buf;
   const int owner = log_node < 0 ? 0 : log_node % csize;
   if (crank != owner) return;
+  if (acc && tid < E) count_out[tid] = sm.lam[tid];
   uep_plan_out o = out;            // this instance's arrays (offset only here: the probes above
   {                                // must not carry eleven pointers in registers)
     const size_t bb = (size_t)batch_b;
@@ -544,7 +547,7 @@ constexpr size_t kLogBudget = 128 * 1024;     // shared memory for the accept lo
 
 template <int RPL>
 static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out& plan,
-                         cudaStream_t s, bool pdl, int n_inst) {
+                         cudaStream_t s, bool pdl, int n_inst, const int32_t* acc, int32_t* count_out) {
   const uep_config& g = c->cfg;
   const int levels = 6;                                        // 63 nodes over kPlanCluster CTAs
   const int cluster = c->plan_cluster;
@@ -571,18 +574,18 @@ static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out&
                                   (const int32_t*)c->d_rexp, plan, g.E, g.R, g.n_slot, c->M, c->P,
                                   g.u_min, g.beta_num, g.beta_den,
                                   g.floor_mode == UEP_FLOOR_STRICT ? 1 : 0, c->S, n_bufs, log_cap,
-                                  levels));
+                                  levels, acc, count_out));
   return UEP_OK;
 }
 
 int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
-                bool pdl, int n_inst) {
+                bool pdl, int n_inst, int32_t* acc, int32_t* count_out) {
   const int R = c->cfg.R;
   if (n_inst <= 0) return UEP_OK;
-  if (R <= 32) return launch_plan_t<1>(c, count, plan, s, pdl, n_inst);
-  if (R <= 64) return launch_plan_t<2>(c, count, plan, s, pdl, n_inst);
-  if (R <= 128) return launch_plan_t<4>(c, count, plan, s, pdl, n_inst);
-  return launch_plan_t<8>(c, count, plan, s, pdl, n_inst);
+  if (R <= 32) return launch_plan_t<1>(c, count, plan, s, pdl, n_inst, acc, count_out);
+  if (R <= 64) return launch_plan_t<2>(c, count, plan, s, pdl, n_inst, acc, count_out);
+  if (R <= 128) return launch_plan_t<4>(c, count, plan, s, pdl, n_inst, acc, count_out);
+  return launch_plan_t<8>(c, count, plan, s, pdl, n_inst, acc, count_out);
 }
 
 template <int RPL>

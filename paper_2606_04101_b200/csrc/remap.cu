@@ -299,7 +299,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
               int32_t* __restrict__ out_rank, int32_t* __restrict__ out_offset,
               GateT* __restrict__ out_gate, int cpg, int group_len,
               const int32_t* __restrict__ cumq, const int32_t* __restrict__ srcpre,
-              int32_t* __restrict__ n_inflight) {
+              int32_t* __restrict__ n_inflight, int32_t* __restrict__ acc_clear) {
   // Source-aware mode (LOCAL): a group of cpg chunks is one source rank r;
   // ranks are LOCAL to (r, e): base0 = prefix row of the chunk - prefix row of the group's first
   // chunk, the cumulative quotas are row r of cumq (the split q[r,e,.] of SolveReroute) and an
@@ -360,6 +360,9 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   // ---- everything above is independent of the plan: under programmatic dependent launch it
   // overlaps the planner (uep_balance); now wait for it and stage the plan (coalesced, in L2) ------
   pdl_wait();
+  // uep_balance: the planner (now complete) has consumed the histogram's accumulator; clear it for
+  // the next call
+  if (acc_clear && c == 0) for (int e = tid; e < E; e += kRemapThreads) acc_clear[e] = 0;
   for (int e = tid; e <= E; e += kRemapThreads) s_off[e] = g_inst_off[e];
   for (int r = tid; r <= R; r += kRemapThreads) rbase[r] = g_rank_base[r];
   for (int p = tid; p < inst_cap; p += kRemapThreads) {
@@ -470,7 +473,7 @@ template <typename GateT>
 static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& p,
                            int32_t* out_replica, int32_t* out_rank, int32_t* out_offset,
                            GateT* out_gate, void* ws, cudaStream_t s, bool pdl, bool local,
-                           int32_t* n_inflight) {
+                           int32_t* n_inflight, int32_t* acc_clear) {
   const uep_config& g = c->cfg;
   const int inst_cap = g.E + g.R * g.n_slot;
   const bool stage = gate != nullptr;
@@ -496,7 +499,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
                                   (const int32_t*)p.inst_cum, (const int32_t*)p.inst_base,
                                   (const int32_t*)p.rank_base, out_replica, out_rank, out_offset,
                                   out_gate, local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S,
-                                  cumq, srcpre, n_inflight));
+                                  cumq, srcpre, n_inflight, acc_clear));
   return UEP_OK;
 }
 
@@ -517,13 +520,13 @@ int init_remap_kernels() {
 
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& p, int32_t* out_replica,
                   int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
-                  bool pdl, bool local, int32_t* n_inflight) {
+                  bool pdl, bool local, int32_t* n_inflight, int32_t* acc_clear) {
   if (c->S == 0) return UEP_OK;
   if (c->cfg.gate_dtype == UEP_GATE_BF16 && gate)
     return launch_lookup_t<uint16_t>(c, static_cast<const uint16_t*>(gate), p, out_replica, out_rank,
-                                     out_offset, static_cast<uint16_t*>(out_gate), ws, s, pdl, local, n_inflight);
+                                     out_offset, static_cast<uint16_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear);
   return launch_lookup_t<uint32_t>(c, static_cast<const uint32_t*>(gate), p, out_replica, out_rank,
-                                   out_offset, static_cast<uint32_t*>(out_gate), ws, s, pdl, local, n_inflight);
+                                   out_offset, static_cast<uint32_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear);
 }
 
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& p,
@@ -531,7 +534,7 @@ int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_p
                  void* ws, cudaStream_t s) {
   int rc = launch_rank(c, ids, ws, s);
   if (rc != UEP_OK) return rc;
-  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s, false, false, nullptr);
+  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s, false, false, nullptr, nullptr);
 }
 
 }  // namespace uep

@@ -422,13 +422,14 @@ static int balance_impl(const uep_ctx* ctx, const int32_t* topk_ids, const void*
   // rank launched first 58.9 us, histogram first 54.5 us, rank made dependent on the histogram
   // 62.5 us (its CTAs then race the plan's cluster for SMs).
   UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
-  int rc2 = uep_histogram(ctx, topk_ids, expert_count, ws, stream);
+  if (!expert_count || !aligned16(expert_count)) return UEP_ERR_INVALID_ARG;
+  int rc2 = launch_histogram(c, topk_ids, expert_count, ws, s, /*red=*/true);
   UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
   rc = launch_rank(c, topk_ids, ws, c->side);
   UEP_CUDA_TRY(cudaEventRecord(c->ev_rank, c->side));
   // planner and lookup are launched programmatically dependent on their predecessor: their
   // prologues (static layout; packed ranks, gates, prefix rows) overlap it
-  if (rc2 == UEP_OK) rc2 = launch_plan(c, expert_count, *plan, s, /*pdl=*/true);
+  if (rc2 == UEP_OK) rc2 = launch_plan(c, expert_count, *plan, s, /*pdl=*/true, 1, ws_acc(ws), expert_count);
   const bool do_pack = n_tensors > 0 && c->cfg.n_slot > 0;
   if (do_pack && rc2 == UEP_OK) {   // pack depends only on the plan and overlaps the lookup (Eq. 1)
     UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
@@ -439,7 +440,8 @@ static int balance_impl(const uep_ctx* ctx, const int32_t* topk_ids, const void*
   UEP_CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
   UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_rank, 0));          // join the rank kernel
   if (rc == UEP_OK && rc2 == UEP_OK)
-    rc2 = launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s, /*pdl=*/true);
+    rc2 = launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s, /*pdl=*/true,
+                        false, nullptr, ws_acc(ws));
   if (join_pack) UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_join, 0));   // join the side stream (pack)
   return rc != UEP_OK ? rc : rc2;
 }

@@ -12,7 +12,8 @@
 
 namespace uep {
 
-constexpr int kWsHeaderBytes = 256;      // [0] ticket of the histogram's last-CTA reduction, [1] of rank_kernel's
+constexpr int kWsHeaderBytes = 256 + 4 * UEP_MAX_E;   // [0] ticket of the histogram's last-CTA reduction;
+                                                     // from byte 256: acc[E] of uep_balance's histogram (zero between calls)
 constexpr int kHistThreads = 1024;
 constexpr int kRemapThreads = 512;
 constexpr int kRemapWarps = kRemapThreads / 32;
@@ -59,16 +60,21 @@ struct PackArgs {
 
 int set_cuda_error(cudaError_t e);
 
-int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s);
+// red = true (uep_balance): no ticket, no last-CTA pass; every CTA adds its counts to ws_acc(ws)
+// with fire-and-forget reductions and the planner (launch_plan with from_acc) reads them there,
+// publishes expert_count and zeroes the accumulator again.
+int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s,
+                     bool red = false);
 int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
-                bool pdl = false, int n_inst = 1);
+                bool pdl = false, int n_inst = 1, int32_t* acc = nullptr, int32_t* count_out = nullptr);
 // uep_remap = launch_rank (plan-independent: stable rank of every slot inside its chunk, packed
 // with the expert id into the workspace) + launch_lookup (plan-dependent: cumulative-quota lookup).
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local = false);
 int launch_reroute(const Ctx* c, const uep_plan_out& plan, int32_t* n_inflight, void* ws, cudaStream_t s);
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& plan, int32_t* out_replica,
                   int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
-                  bool pdl = false, bool local = false, int32_t* n_inflight = nullptr);
+                  bool pdl = false, bool local = false, int32_t* n_inflight = nullptr,
+                  int32_t* acc_clear = nullptr);
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& plan,
                  int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
                  void* ws, cudaStream_t s);
@@ -130,6 +136,7 @@ inline int32_t* ws_table(void* ws) {
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes);
 }
 inline unsigned* ws_ticket(void* ws) { return reinterpret_cast<unsigned*>(ws); }
+inline int32_t* ws_acc(void* ws) { return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + 256); }
 inline size_t ws_table_bytes(const Ctx* c) {
   return (sizeof(int32_t) * (size_t)c->n_chunks * c->E_pad + 255) & ~(size_t)255;
 }
