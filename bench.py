@@ -387,10 +387,12 @@ def run_uep(args):
     # DRAM traffic per launch from the committed ncu --set full capture (dsv3_prefill only; that
     # capture is not re-taken here: a number printed under a profiler is never a bench value)
     traffic = {}
-    tpath = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r01_final_traffic.json")
+    tpath = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r01_final_traffic.csv")
     if args.workload == "dsv3_prefill" and args.state_scale == 1.0 and os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f)
+            for line in f.read().splitlines()[1:]:
+                k_, v_ = line.rsplit(",", 1)
+                traffic[k_] = int(v_)
 
     def roof(name, nbytes, dur_us, tkey=None):
         a = nbytes / (dur_us * 1e-6) / 1e9 if dur_us > 0 else 0.0
