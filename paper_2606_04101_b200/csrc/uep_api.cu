@@ -415,6 +415,7 @@ static int balance_impl(const uep_ctx* ctx, const int32_t* topk_ids, const void*
   if ((gate == nullptr) != (out_gate == nullptr)) return UEP_ERR_INVALID_ARG;
   if (gate && (c->cfg.gate_dtype == UEP_GATE_NONE || !aligned16(gate) || !aligned16(out_gate)))
     return UEP_ERR_INVALID_ARG;
+  if (!expert_count || !aligned16(expert_count)) return UEP_ERR_INVALID_ARG;
   // fork: the plan-independent half of the remap (stable ranks inside each chunk) runs on the side
   // stream beside histogram + plan.  The histogram is LAUNCHED first (the fork event precedes it,
   // so the rank kernel does not depend on it): its CTAs take the SMs first, the rank CTAs fill in
@@ -422,7 +423,6 @@ static int balance_impl(const uep_ctx* ctx, const int32_t* topk_ids, const void*
   // rank launched first 58.9 us, histogram first 54.5 us, rank made dependent on the histogram
   // 62.5 us (its CTAs then race the plan's cluster for SMs).
   UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
-  if (!expert_count || !aligned16(expert_count)) return UEP_ERR_INVALID_ARG;
   int rc2 = launch_histogram(c, topk_ids, expert_count, ws, s, /*red=*/true);
   UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
   rc = launch_rank(c, topk_ids, ws, c->side);

@@ -551,3 +551,19 @@ def test_balance_host_end_to_end():
     ref = np.zeros((R, ns, state.shape[1]), dtype=np.int16)
     oracle.pack(p.slot_expert, state.view(torch.int16).numpy(), ref)
     assert np.array_equal(dst.cpu().view(torch.int16).numpy(), ref)   # uep_balance_host returned after the pack
+
+
+def test_more_error_codes():
+    ctx = binding.Context(1000, 2, 16, 3, 1, 8)          # T % R != 0: no source-aware remap
+    ws, plan = ctx.new_workspace(), ctx.new_plan()
+    ids = torch.zeros((1000, 2), dtype=torch.int32, device=DEV)
+    rep, rnk, off, _ = ctx.new_outputs(None)
+    with pytest.raises(binding.UepError, match="unsupported"):
+        ctx.uep_remap_local(ids, None, plan, rep, rnk, off, None, None, ws)
+    ctx2 = binding.Context(1024, 2, 16, 4, 1, 8, gate_dtype=binding.GATE_NONE)
+    plan2 = ctx2.new_plan()
+    count = torch.zeros(16, dtype=torch.int32, device=DEV)
+    ctx2.uep_plan_batched(0, count, plan2)                 # nothing to do is not an error
+    with pytest.raises(binding.UepError):
+        ctx2.uep_grad_reduce(plan2, [torch.zeros((16, 6), device=DEV)], [torch.zeros((4, 1, 6), device=DEV)])  # 24 B
+    torch.cuda.synchronize()
