@@ -198,6 +198,39 @@ int uep_remap_local(const uep_ctx* ctx, const int32_t* topk_ids, const void* gat
                     const uep_plan_out* plan, int32_t* out_replica, int32_t* out_rank,
                     int32_t* out_offset, void* out_gate, int32_t* n_inflight, void* ws, void* stream);
 
+/* Token-sharded path for G real GPUs (§4.2 "each rank computes gating for its local tokens ...
+ * exchanges the count matrix ... every rank solves the same plan").
+ * GPU g of G (G divides R, T % R == 0) owns the tokens of source ranks [g*R/G, (g+1)*R/G), i.e.
+ * the contiguous slot range [g*S/G, (g+1)*S/G).  One layer is
+ *   uep_shard_count   on every GPU: ranks its LOCAL slots inside their chunks and leaves this
+ *                     shard's rows of the count table (per-chunk lambda: the rows of Lambda[R,E],
+ *                     subdivided) in ws;
+ *   an all-gather     of those rows, by the caller (NCCL / torch.distributed; the only exchange).
+ *                     uep_shard_rows gives the byte range of shard g's rows inside ws: the ranges
+ *                     of shards 0..G-1 are equal-sized, contiguous and in shard order, so an
+ *                     in-place all-gather on ws[offset(0) .. offset(0) + G*bytes) does it;
+ *   uep_shard_finish  on every GPU, redundantly and deterministically: prefix over the gathered
+ *                     table, lambda_e = its totals row -> expert_count, the SAME plan everywhere,
+ *                     then the lookup of the local slots with their GLOBAL stable ranks.
+ * The concatenation of the shards' outputs equals uep_remap on the whole input (global stable
+ * order, S12), bit for bit; G = 1 is the whole problem.
+ *   topk_ids_local / gate_local / out_*_local   DEVICE, the shard's S/G slots, 16-B aligned
+ *   out_gate     DEVICE [T*k], GLOBAL dispatch order: only the entries of this shard's slots are
+ *                written (in the deployment the dispatch carries the gate with the token)
+ *   n_inflight   DEVICE int32 [R] or NULL: entries of this shard's source ranks are set to the
+ *                number of their slots that leave the rank
+ *   ws           sized by uep_workspace_bytes (of the whole problem), initialised once
+ * Errors: UEP_ERR_UNSUPPORTED if T % R != 0; UEP_ERR_INVALID_ARG if G does not divide R, g is
+ * out of range, or a pointer is NULL / misaligned. */
+int uep_shard_count(const uep_ctx* ctx, int32_t shard, int32_t n_shards,
+                    const int32_t* topk_ids_local, void* ws, void* stream);
+int uep_shard_rows(const uep_ctx* ctx, int32_t shard, int32_t n_shards, size_t* ws_byte_offset,
+                   size_t* n_bytes);
+int uep_shard_finish(const uep_ctx* ctx, int32_t shard, int32_t n_shards, const void* gate_local,
+                     int32_t* expert_count, const uep_plan_out* plan, int32_t* out_replica_local,
+                     int32_t* out_rank_local, int32_t* out_offset_local, void* out_gate,
+                     int32_t* n_inflight, void* ws, void* stream);
+
 /* Pack the state of every replicated expert into its destination slot:
  *   dst[j][(t*n_slot+s)*B_j .. +B_j) = src[j][e*B_j .. +B_j)  for x_{t,s} = e != empty.
  * Empty slots are not touched.  src/dst/bytes_per_expert: HOST arrays [n_tensors] of DEVICE

@@ -24,7 +24,7 @@ SC_TAU, SC_N_REPLICAS, SC_MAX_LOAD, SC_MAX_FANOUT, SC_N_PROBES, SC_N_INVALID, SC
 
 EXPORTS = ["uep_create", "uep_destroy", "uep_workspace_bytes", "uep_workspace_init",
            "uep_plan_bytes", "uep_histogram", "uep_plan", "uep_plan_batched", "uep_remap", "uep_remap_local",
-           "uep_remap_rank",
+           "uep_remap_rank", "uep_shard_count", "uep_shard_rows", "uep_shard_finish",
            "uep_remap_lookup", "uep_remap_inverse", "uep_relay_plan", "uep_pack", "uep_grad_reduce",
            "uep_balance",
            "uep_balance_host", "uep_strerror", "uep_last_cuda_error", "uep_get_launch_info"]
@@ -229,6 +229,25 @@ class Context:
         _check(lib().uep_remap_local(self._h, _ptr(topk_ids), _ptr(gate), ctypes.byref(plan.c),
                                      _ptr(out_replica), _ptr(out_rank), _ptr(out_offset),
                                      _ptr(out_gate), _ptr(n_inflight), _ptr(ws), _stream(stream)))
+
+    # ---- token-sharded path (uep.h: uep_shard_*): GPU `shard` of `n_shards` --------------------
+    def uep_shard_count(self, shard: int, n_shards: int, topk_ids_local, ws, stream=None):
+        _check(lib().uep_shard_count(self._h, int(shard), int(n_shards), _ptr(topk_ids_local), _ptr(ws),
+                                     _stream(stream)))
+
+    def uep_shard_rows(self, shard: int, n_shards: int) -> tuple[int, int]:
+        """(byte offset inside ws, byte count) of the shard's rows of the count table."""
+        off, n = ctypes.c_size_t(0), ctypes.c_size_t(0)
+        _check(lib().uep_shard_rows(self._h, int(shard), int(n_shards), ctypes.byref(off), ctypes.byref(n)))
+        return int(off.value), int(n.value)
+
+    def uep_shard_finish(self, shard: int, n_shards: int, gate_local, expert_count, plan: Plan,
+                         out_replica_local, out_rank_local, out_offset_local, out_gate, n_inflight, ws,
+                         stream=None):
+        _check(lib().uep_shard_finish(self._h, int(shard), int(n_shards), _ptr(gate_local),
+                                      _ptr(expert_count), ctypes.byref(plan.c), _ptr(out_replica_local),
+                                      _ptr(out_rank_local), _ptr(out_offset_local), _ptr(out_gate),
+                                      _ptr(n_inflight), _ptr(ws), _stream(stream)))
 
     def uep_remap_rank(self, topk_ids, ws, stream=None):
         _check(lib().uep_remap_rank(self._h, _ptr(topk_ids), _ptr(ws), _stream(stream)))

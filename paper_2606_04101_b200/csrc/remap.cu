@@ -45,15 +45,16 @@ constexpr int kEMask = (1 << kPackedEBits) - 1;
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kRemapThreads, 2)
 rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len, int cpg,
-            int group_len, int32_t* __restrict__ packed, int32_t* __restrict__ prefix) {
+            int group_len, int32_t* __restrict__ packed, int32_t* __restrict__ prefix, int chunk0) {
   extern __shared__ __align__(16) int smem[];
   int2* wrow = reinterpret_cast<int2*>(smem);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
+  const int cb = (int)blockIdx.x + chunk0;       // chunk0 > 0: a token shard's CTAs (uep_shard_count)
   // chunk c = sub-chunk c % cpg of group c / cpg (a group = one source rank's slots in the
   // source-aware remap; the whole input, cpg = number of chunks, otherwise)
-  const int sub = (int)blockIdx.x % cpg;
-  const long long cbegin = (long long)((int)blockIdx.x / cpg) * group_len + (long long)sub * chunk_len;
+  const int sub = cb % cpg;
+  const long long cbegin = (long long)(cb / cpg) * group_len + (long long)sub * chunk_len;
   const int clen = (int)min(min((long long)chunk_len, (long long)group_len - (long long)sub * chunk_len),
                             (long long)S - cbegin);                            // <= kMaxChunk
   const int items = (clen + kRemapThreads - 1) / kRemapThreads;                // steps per warp
@@ -106,7 +107,7 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
         run += x;
       }
     }
-    prefix[(size_t)(blockIdx.x + 1) * E_pad + e] = run;
+    prefix[(size_t)(cb + 1) * E_pad + e] = run;
   }
   __syncthreads();
 
@@ -163,17 +164,27 @@ prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG) {
   }
 }
 
-int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local) {
+// chunk0 / n_launch: the chunk range a token shard owns (uep_shard_count; `ids` is then the
+// virtual base of the global [S] array, only the shard's slots are dereferenced); n_launch < 0:
+// all chunks.  with_prefix = false leaves the raw per-chunk counts for the exchange step.
+int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local, int chunk0,
+                int n_launch, bool with_prefix) {
   if (c->S == 0) return UEP_OK;
   const int chunks = local ? c->l_chunks : c->r_chunks;
   const size_t smem = sizeof(int2) * (size_t)kRemapWarps * c->E_pad;
-  rank_kernel<<<chunks, kRemapThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
-                                                 local ? c->l_chunk_len : c->r_chunk_len,
-                                                 local ? c->l_cpg : c->r_chunks,
-                                                 local ? c->l_group_len : c->S, ws_packed(c, ws),
-                                                 ws_prefix(c, ws));
+  rank_kernel<<<n_launch < 0 ? chunks : n_launch, kRemapThreads, smem, s>>>(
+      ids, c->S, c->cfg.E, c->E_pad, local ? c->l_chunk_len : c->r_chunk_len,
+      local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S, ws_packed(c, ws),
+      ws_prefix(c, ws), chunk0);
   UEP_CUDA_TRY(cudaGetLastError());
-  prefix_kernel<<<c->E_pad / 4, 1024, 0, s>>>(ws_prefix(c, ws), chunks, c->E_pad / 4);
+  if (with_prefix) return launch_prefix(c, ws, s, local);
+  return UEP_OK;
+}
+
+int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local) {
+  if (c->S == 0) return UEP_OK;
+  prefix_kernel<<<c->E_pad / 4, 1024, 0, s>>>(ws_prefix(c, ws), local ? c->l_chunks : c->r_chunks,
+                                              c->E_pad / 4);
   UEP_CUDA_TRY(cudaGetLastError());
   return UEP_OK;
 }
@@ -299,7 +310,10 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
               int32_t* __restrict__ out_rank, int32_t* __restrict__ out_offset,
               GateT* __restrict__ out_gate, int cpg, int group_len,
               const int32_t* __restrict__ cumq, const int32_t* __restrict__ srcpre,
-              int32_t* __restrict__ n_inflight, int32_t* __restrict__ acc_clear) {
+              int32_t* __restrict__ n_inflight, int32_t* __restrict__ acc_clear, int chunk0) {
+  // Token-sharded mode (LOCAL with cumq == nullptr): the grouped chunk geometry and
+  // the per-source in-flight count of the source-aware mode, but GLOBAL ranks and the plan's own
+  // cumulative quotas, on the chunks [chunk0, chunk0 + gridDim.x) that this GPU owns.
   // Source-aware mode (LOCAL): a group of cpg chunks is one source rank r;
   // ranks are LOCAL to (r, e): base0 = prefix row of the chunk - prefix row of the group's first
   // chunk, the cumulative quotas are row r of cumq (the split q[r,e,.] of SolveReroute) and an
@@ -321,8 +335,8 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   int* sd = reinterpret_cast<int*>(sg + kMaxChunk);   // their out_gate index
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int c = blockIdx.x;
-  constexpr bool local = LOCAL;
+  const int c = LOCAL ? (int)blockIdx.x + chunk0 : (int)blockIdx.x;
+  const bool local = LOCAL && cumq != nullptr;   // ranks local to (source rank, expert)
   const int grp = LOCAL ? c / cpg : 0, sub = LOCAL ? c % cpg : c;
   const long long cbegin = (long long)grp * group_len + (long long)sub * chunk_len;
   const int clen = LOCAL ? (int)min(min((long long)chunk_len, (long long)group_len - (long long)sub * chunk_len),
@@ -453,7 +467,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
       }
     }
   }
-  if (local && n_inflight) {                             // tokens of source rank grp that leave it
+  if (LOCAL && n_inflight) {                             // tokens of source rank grp that leave it
     n_fly = __reduce_add_sync(kFullMask, n_fly);
     if (lane == 0 && n_fly) atomicAdd(n_inflight + grp, n_fly);
   }
@@ -473,7 +487,8 @@ template <typename GateT>
 static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& p,
                            int32_t* out_replica, int32_t* out_rank, int32_t* out_offset,
                            GateT* out_gate, void* ws, cudaStream_t s, bool pdl, bool local,
-                           int32_t* n_inflight, int32_t* acc_clear) {
+                           int32_t* n_inflight, int32_t* acc_clear, int chunk0, int n_launch,
+                           bool src_aware) {
   const uep_config& g = c->cfg;
   const int inst_cap = g.E + g.R * g.n_slot;
   const bool stage = gate != nullptr;
@@ -481,7 +496,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
   auto k = local ? (stage ? lookup_kernel<GateT, true, true> : lookup_kernel<GateT, false, true>)
                  : (stage ? lookup_kernel<GateT, true, false> : lookup_kernel<GateT, false, false>);
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(local ? c->l_chunks : c->r_chunks);
+  cfg.gridDim = dim3(n_launch >= 0 ? n_launch : (local ? c->l_chunks : c->r_chunks));
   cfg.blockDim = dim3(kRemapThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = s;
@@ -490,8 +505,8 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = pdl ? 1 : 0;
-  const int32_t* cumq = local ? ws_reroute(c, ws) : nullptr;
-  const int32_t* srcpre = local ? cumq + (size_t)g.R * inst_cap : nullptr;
+  const int32_t* cumq = (local && src_aware) ? ws_reroute(c, ws) : nullptr;
+  const int32_t* srcpre = cumq ? cumq + (size_t)g.R * inst_cap : nullptr;
   UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, k, (const int32_t*)ws_packed(c, ws), gate, c->S, g.E, c->E_pad,
                                   g.R, inst_cap, local ? c->l_chunk_len : c->r_chunk_len,
                                   (const int32_t*)ws_prefix(c, ws),
@@ -499,7 +514,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
                                   (const int32_t*)p.inst_cum, (const int32_t*)p.inst_base,
                                   (const int32_t*)p.rank_base, out_replica, out_rank, out_offset,
                                   out_gate, local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S,
-                                  cumq, srcpre, n_inflight, acc_clear));
+                                  cumq, srcpre, n_inflight, acc_clear, chunk0));
   return UEP_OK;
 }
 
@@ -520,13 +535,16 @@ int init_remap_kernels() {
 
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& p, int32_t* out_replica,
                   int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
-                  bool pdl, bool local, int32_t* n_inflight, int32_t* acc_clear) {
+                  bool pdl, bool local, int32_t* n_inflight, int32_t* acc_clear, int chunk0,
+                  int n_launch, bool src_aware) {
   if (c->S == 0) return UEP_OK;
   if (c->cfg.gate_dtype == UEP_GATE_BF16 && gate)
     return launch_lookup_t<uint16_t>(c, static_cast<const uint16_t*>(gate), p, out_replica, out_rank,
-                                     out_offset, static_cast<uint16_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear);
+                                     out_offset, static_cast<uint16_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear,
+                                     chunk0, n_launch, src_aware);
   return launch_lookup_t<uint32_t>(c, static_cast<const uint32_t*>(gate), p, out_replica, out_rank,
-                                   out_offset, static_cast<uint32_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear);
+                                   out_offset, static_cast<uint32_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear,
+                                   chunk0, n_launch, src_aware);
 }
 
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& p,

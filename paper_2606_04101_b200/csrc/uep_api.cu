@@ -345,6 +345,89 @@ int uep_remap_local(const uep_ctx* ctx, const int32_t* topk_ids, const void* gat
   return rc;
 }
 
+// ---- token-sharded path ----------------------------------------------------------
+// Shard g of G owns source ranks [g*R/G, (g+1)*R/G): chunks [g*cps, (g+1)*cps) of the grouped
+// geometry (cps = R/G * l_cpg) and slots [g*S/G, (g+1)*S/G).  The kernels index the GLOBAL slot
+// arrays; a shard's local buffers are addressed through a virtual base (local pointer minus the
+// shard's first slot) of which only the shard's own range is ever dereferenced.
+struct ShardGeom { int chunk0, chunks; long long slot0; };
+
+static int shard_geom(const Ctx* c, int32_t shard, int32_t n_shards, ShardGeom* g) {
+  if (n_shards < 1 || shard < 0 || shard >= n_shards || c->cfg.R % n_shards != 0) return UEP_ERR_INVALID_ARG;
+  if (c->S > 0 && c->l_cpg == 0) return UEP_ERR_UNSUPPORTED;           // T must be a multiple of R
+  const int rps = c->cfg.R / n_shards;
+  g->chunks = rps * c->l_cpg;
+  g->chunk0 = shard * g->chunks;
+  g->slot0 = (long long)shard * rps * c->l_group_len;
+  return UEP_OK;
+}
+
+static void* virtual_base(const void* local, long long slot0, size_t elem) {
+  return local ? reinterpret_cast<void*>(reinterpret_cast<uintptr_t>(local) - (uintptr_t)slot0 * elem) : nullptr;
+}
+
+int uep_shard_rows(const uep_ctx* ctx, int32_t shard, int32_t n_shards, size_t* ws_byte_offset,
+                   size_t* n_bytes) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !ws_byte_offset || !n_bytes) return UEP_ERR_INVALID_ARG;
+  ShardGeom g;
+  int rc = shard_geom(c, shard, n_shards, &g);
+  if (rc != UEP_OK) return rc;
+  // chunk ch's counts live in row ch + 1 of the prefix table (row 0 stays zero)
+  const size_t row = sizeof(int32_t) * (size_t)c->E_pad;
+  *ws_byte_offset = (size_t)kWsHeaderBytes + ws_table_bytes(c) + row * (size_t)(g.chunk0 + 1);
+  *n_bytes = row * (size_t)g.chunks;
+  return UEP_OK;
+}
+
+int uep_shard_count(const uep_ctx* ctx, int32_t shard, int32_t n_shards,
+                    const int32_t* topk_ids_local, void* ws, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !ws || !aligned16(ws)) return UEP_ERR_INVALID_ARG;
+  ShardGeom g;
+  int rc = shard_geom(c, shard, n_shards, &g);
+  if (rc != UEP_OK) return rc;
+  if (c->S == 0) return UEP_OK;
+  if (!topk_ids_local || !aligned16(topk_ids_local)) return UEP_ERR_INVALID_ARG;
+  return launch_rank(c, static_cast<const int32_t*>(virtual_base(topk_ids_local, g.slot0, 4)), ws,
+                     static_cast<cudaStream_t>(stream), /*local=*/true, g.chunk0, g.chunks,
+                     /*with_prefix=*/false);
+}
+
+int uep_shard_finish(const uep_ctx* ctx, int32_t shard, int32_t n_shards, const void* gate_local,
+                     int32_t* expert_count, const uep_plan_out* plan, int32_t* out_replica_local,
+                     int32_t* out_rank_local, int32_t* out_offset_local, void* out_gate,
+                     int32_t* n_inflight, void* ws, void* stream) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  if (!c || !expert_count || !aligned16(expert_count)) return UEP_ERR_INVALID_ARG;
+  ShardGeom g;
+  int rc = shard_geom(c, shard, n_shards, &g);
+  if (rc != UEP_OK) return rc;
+  rc = check_remap_outputs(c, gate_local, plan, out_replica_local, out_rank_local, out_offset_local,
+                           out_gate, ws);
+  if (rc != UEP_OK) return rc;
+  if (n_inflight && !aligned16(n_inflight)) return UEP_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (c->S == 0) {                                                     // identity plan of an empty batch
+    UEP_CUDA_TRY(cudaMemsetAsync(expert_count, 0, sizeof(int32_t) * c->cfg.E, s));
+    return launch_plan(c, expert_count, *plan, s);
+  }
+  const int rps = c->cfg.R / n_shards;
+  if (n_inflight) UEP_CUDA_TRY(cudaMemsetAsync(n_inflight + shard * rps, 0, sizeof(int32_t) * rps, s));
+  rc = launch_prefix(c, ws, s, /*local=*/true);
+  // lambda_e = totals row of the scanned table; the planner publishes it as expert_count
+  int32_t* totals = ws_prefix(c, ws) + (size_t)c->l_chunks * c->E_pad;
+  if (rc == UEP_OK) rc = launch_plan(c, nullptr, *plan, s, /*pdl=*/false, 1, totals, expert_count);
+  const size_t gb = c->cfg.gate_dtype == UEP_GATE_BF16 ? 2 : 4;
+  if (rc == UEP_OK)
+    rc = launch_lookup(c, virtual_base(gate_local, g.slot0, gb), *plan,
+                       static_cast<int32_t*>(virtual_base(out_replica_local, g.slot0, 4)),
+                       static_cast<int32_t*>(virtual_base(out_rank_local, g.slot0, 4)),
+                       static_cast<int32_t*>(virtual_base(out_offset_local, g.slot0, 4)), out_gate, ws, s, /*pdl=*/true,
+                       /*local=*/true, n_inflight, nullptr, g.chunk0, g.chunks, /*src_aware=*/false);
+  return rc;
+}
+
 int uep_grad_reduce(const uep_ctx* ctx, const uep_plan_out* plan, int32_t n_tensors,
                     void* const* main_grad, const size_t* bytes_per_expert, void* const* slot_grad,
                     void* stream) {

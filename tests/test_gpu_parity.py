@@ -567,3 +567,106 @@ def test_more_error_codes():
     with pytest.raises(binding.UepError):
         ctx2.uep_grad_reduce(plan2, [torch.zeros((16, 6), device=DEV)], [torch.zeros((4, 1, 6), device=DEV)])  # 24 B
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("T,k,E,R,n_slot,s,G,gate_bf16", [
+    (4096, 2, 16, 4, 1, 1.2, 2, False),          # tiny config on two GPUs
+    (8192, 4, 64, 16, 2, 2.0, 4, True),          # bf16 gates, four shards
+    (65536, 8, 128, 32, 2, 1.0, 8, False),       # GLM-Air-like on 8 GPUs (two chunks per source rank)
+    (4100 * 8, 4, 64, 8, 2, 1.4, 2, False),      # ragged last chunk of every source rank's block
+    (262144, 8, 256, 64, 2, 1.0, 1, False),      # full DeepSeek-V3 shape, G = 1 (the whole problem)
+    (262144, 8, 256, 64, 2, 1.0, 8, False),      # and on 8 GPUs
+])
+def test_token_sharded_path_matches_global_remap(T, k, E, R, n_slot, s, G, gate_bf16):
+    """G token shards (one per real GPU), run here one after the other on one GPU
+    with the all-gather done by copying count rows between the shards' workspaces.  Every shard
+    must publish the oracle's lambda and plan; the concatenated outputs must equal the oracle's
+    global stable-order remap bit for bit; out_gate entries of other shards' slots stay untouched."""
+    from paper_2606_04101_b200 import shard as shard_mod
+    um = synth.stress_u_min(T * k, R) if T * k < 2000000 else 1024
+    ids = synth.zipf_topk_ids(T, k, E, s, 77)
+    ids[5, 0] = -1                                             # an invalid id on shard 0
+    gate = synth.gates_softmax_bf16(T, k, 5) if gate_bf16 else synth.gates_uniform_renorm(T, k, 5)
+    gd = binding.GATE_BF16 if gate_bf16 else binding.GATE_F32
+    ctx = binding.Context(T, k, E, R, n_slot, um, gate_dtype=gd)
+    S, Sl = T * k, T * k // G
+    layers = [shard_mod.TokenShardedLayer(ctx, g, G) for g in range(G)]
+    d_ids = ids.to(DEV).reshape(-1)
+    d_gate = gate.to(DEV).reshape(-1)
+    off0, nb = ctx.uep_shard_rows(0, G)
+    for g, L in enumerate(layers):
+        assert ctx.uep_shard_rows(g, G) == (off0 + g * nb, nb)
+        L.out_gate = torch.full((S,), 0x7fff if gate_bf16 else 0x7fc0dead, dtype=torch.int32, device=DEV) \
+            .to(torch.int16 if gate_bf16 else torch.int32).view(gate.dtype)
+        ctx.uep_shard_count(g, G, d_ids[g * Sl:(g + 1) * Sl], L.ws)
+    torch.cuda.synchronize()
+    # the exchange, emulated: every workspace receives every shard's rows
+    rows = torch.cat([L.ws[off0 + g * nb: off0 + (g + 1) * nb] for g, L in enumerate(layers)])
+    for L in layers:
+        L.ws[off0: off0 + G * nb] = rows
+    for g, L in enumerate(layers):
+        L.n_inflight.fill_(-3)
+        ctx.uep_shard_finish(g, G, d_gate[g * Sl:(g + 1) * Sl], L.expert_count, L.plan, L.out_replica,
+                             L.out_rank, L.out_offset, L.out_gate, L.n_inflight, L.ws)
+    torch.cuda.synchronize()
+
+    lam, p, o_rep, o_rnk, o_off, o_og = oracle_chain(ids, gate, E, R, n_slot, um)
+    # per-chunk count rows = plain bincount of each chunk (the subdivided rows of Lambda[R,E])
+    E_pad = (E + 3) // 4 * 4
+    block = (T // R) * k
+    got_rows = rows.view(torch.int32).cpu().numpy().reshape(-1, E_pad)
+    cpg = got_rows.shape[0] // R
+    flat = ids.numpy().reshape(-1)
+    Lam = np.zeros((R, E), dtype=np.int64)
+    for r in range(R):
+        Lam[r] = got_rows[r * cpg:(r + 1) * cpg, :E].sum(axis=0)
+        blk = flat[r * block:(r + 1) * block]
+        assert np.array_equal(Lam[r], np.bincount(blk[(blk >= 0) & (blk < E)], minlength=E))
+    assert np.array_equal(Lam.sum(axis=0), lam)
+    for g, L in enumerate(layers):
+        assert np.array_equal(L.expert_count.cpu().numpy()[:E], lam)
+        hp = L.plan.host()
+        for n in PLAN_ARRAYS:
+            if n == "U":                                       # the layers' plans carry no dense U
+                continue
+            assert np.array_equal(np.asarray(getattr(hp, n)).reshape(-1), np.asarray(getattr(p, n)).reshape(-1)), (g, n)
+    cat = lambda name: torch.cat([getattr(L, name)[:Sl] for L in layers]).cpu().numpy().reshape(T, k)
+    assert np.array_equal(cat("out_replica"), o_rep)
+    assert np.array_equal(cat("out_rank"), o_rnk)
+    assert np.array_equal(cat("out_offset"), o_off)
+    # gates: shard g wrote exactly the dispatch positions of its own slots
+    bits = lambda t: t.view(torch.int16).cpu().numpy().view(np.uint16) if gate_bf16 \
+        else t.view(torch.int32).cpu().numpy().view(np.uint32)
+    sentinel = np.uint16(0x7fff) if gate_bf16 else np.uint32(0x7fc0dead)
+    rank_base = np.asarray(p.rank_base)
+    dest = np.where(o_rnk.reshape(-1) >= 0, rank_base[np.maximum(o_rnk.reshape(-1), 0)] + o_off.reshape(-1), -1)
+    for g, L in enumerate(layers):
+        mine = dest[g * Sl:(g + 1) * Sl]
+        mine = mine[mine >= 0]
+        gb = bits(L.out_gate)
+        assert np.array_equal(gb[mine], o_og[mine])
+        other = np.ones(S, dtype=bool)
+        other[mine] = False
+        assert (gb[other] == sentinel).all()
+    # in-flight slots per source rank (slots whose destination is not their source rank)
+    src = np.arange(S) // block
+    fly = np.bincount(src[(o_rnk.reshape(-1) >= 0) & (o_rnk.reshape(-1) != src)], minlength=R)
+    rps = R // G
+    for g, L in enumerate(layers):
+        got = L.n_inflight.cpu().numpy()[:R]
+        assert np.array_equal(got[g * rps:(g + 1) * rps], fly[g * rps:(g + 1) * rps])
+        assert (np.delete(got, np.s_[g * rps:(g + 1) * rps]) == -3).all()
+
+
+def test_token_shard_argument_errors():
+    ctx = binding.Context(4096, 2, 16, 4, 1, 64)
+    ws = ctx.new_workspace()
+    ids = torch.zeros(4096, dtype=torch.int32, device=DEV)
+    for shard, G in ((0, 3), (2, 2), (-1, 2), (0, 0)):          # G must divide R; 0 <= shard < G
+        with pytest.raises(binding.UepError):
+            ctx.uep_shard_count(shard, G, ids, ws)
+        with pytest.raises(binding.UepError):
+            ctx.uep_shard_rows(shard, G)
+    with pytest.raises(binding.UepError):                        # T % R != 0: unsupported
+        c2 = binding.Context(4098, 2, 16, 4, 1, 64)
+        c2.uep_shard_count(0, 2, ids, c2.new_workspace())

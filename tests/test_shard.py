@@ -1,5 +1,6 @@
-"""N>1 host logic on CPU: world_size-2 gloo. The path shards by independent instances (weak
-scaling, no data-path collective); the only cross-rank traffic is a barrier and a MAX reduce."""
+"""N>1 host logic on CPU: world_size-2 gloo.  bench.py shards independent instances (weak
+scaling, no data-path collective: a barrier and a MAX reduce only); the token-sharded path of
+SURVEY §8(e) has one exchange, the in-place all-gather of the shards' count rows."""
 import os
 import socket
 
@@ -16,6 +17,10 @@ def _free_port():
         return s.getsockname()[1]
 
 
+def E_pad_row_bytes(E_pad):
+    return 4 * E_pad                       # row 0 of the prefix table stays zero in the real layout
+
+
 def _worker(rank, world, port, q):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
@@ -28,8 +33,17 @@ def _worker(rank, world, port, q):
     # the check on a real box; here we gather the owned instance ids
     got = [None] * world
     dist.all_gather_object(got, owned)
+    # token-sharded path: the exchange of count rows inside a workspace-shaped byte tensor.
+    # Shard g's rows (E_pad int32 per chunk) sit at off0 + g*nb; the kernels that fill and consume
+    # them need a GPU, the exchange itself does not.
+    E_pad, chunks, off0 = 16, 3, 256 + 2048 + 64 + E_pad_row_bytes(16)
+    nb = chunks * E_pad * 4
+    ws = torch.full((off0 + world * nb + 128,), 0xAB, dtype=torch.uint8)
+    mine = (torch.arange(chunks * E_pad, dtype=torch.int32) + 1000 * (rank + 1))
+    ws[off0 + rank * nb: off0 + (rank + 1) * nb] = mine.view(torch.uint8)
+    shard.exchange_counts(ws, off0, nb, rank, world)
     dist.barrier()
-    q.put((rank, sched, owned, t, got))
+    q.put((rank, sched, owned, t, got, ws.numpy().copy(), off0, nb))
     dist.destroy_process_group()
 
 
@@ -44,7 +58,13 @@ def test_world_size_2_gloo():
     for p in ps:
         p.join(timeout=60)
         assert p.exitcode == 0
-    (r0, s0, o0, t0, g0), (r1, s1, o1, t1, g1) = res
+    (r0, s0, o0, t0, g0, w0, off0, nb), (r1, s1, o1, t1, g1, w1, _, _) = res
+    import numpy as np
+    assert np.array_equal(w0, w1)                                          # every rank holds every row
+    rows = w0[off0: off0 + 2 * nb].view(np.int32).reshape(2, -1)
+    assert np.array_equal(rows[0], np.arange(rows.shape[1]) + 1000)
+    assert np.array_equal(rows[1], np.arange(rows.shape[1]) + 2000)
+    assert (w0[:off0] == 0xAB).all() and (w0[off0 + 2 * nb:] == 0xAB).all()  # nothing else touched
     assert s0 == s1 == [0, 1, 2, 3, 0, 1]                  # every rank runs `steps` steps
     assert set(o0).isdisjoint(o1) and sorted(o0 + o1) == list(range(8))   # disjoint instances
     assert t0 == t1 == 15.0                                  # max over ranks
@@ -53,6 +73,9 @@ def test_world_size_2_gloo():
 
 
 def test_single_process_paths():
+    ws = torch.arange(64, dtype=torch.uint8)
+    shard.exchange_counts(ws, 16, 32, 0, 1)                               # world 1: a no-op
+    assert torch.equal(ws, torch.arange(64, dtype=torch.uint8))
     assert shard.reduce_max_time(3.5) == 3.5
     assert shard.step_schedule(0, 3, 0, 1) == []
     assert shard.step_schedule(5, 2, 0, 1) == [0, 1, 0, 1, 0]
