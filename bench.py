@@ -237,7 +237,7 @@ def dist_setup(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    if world > 1:
+    if world > 1 or (os.environ.get("UEP_BENCH_FORCE_PG") == "1" and "RANK" in os.environ):
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         backend = "nccl" if torch.cuda.is_available() else "gloo"
@@ -253,6 +253,70 @@ def barrier_and_max(world, value_ms, device):
         return value_ms
     from paper_2606_04101_b200 import shard
     return shard.reduce_max_time(value_ms)
+
+
+def run_token_sharded(c, rig, world, rank, device, stream, reps):
+    """ONE layer's tokens sharded over the `world` GPUs (the paper's deployment,
+    PAPER.md:162): uep_shard_count -> in-place all-gather of the count rows -> uep_shard_finish
+    (identical plan on every GPU, lookup of the local slots).  world == 1 is the whole problem on
+    one GPU.  All ranks take their slice of the SAME seeded instances."""
+    import torch
+    import torch.distributed as dist
+    from paper_2606_04101_b200 import binding, shard
+    n = min(4, rig.n_inst)
+    S = c["T"] * c["k"]
+    Sl = S // world
+    ids_l, gate_l = [], []
+    for i in range(n):
+        if world == 1:
+            ids, gate = rig.ids[i], rig.gates[i]
+        else:                               # same instance on every rank, then this rank's slots
+            ids, gate, _ = instance_inputs(c, 100000 + i, device)
+        ids_l.append(ids.reshape(-1)[rank * Sl:(rank + 1) * Sl].clone())
+        gate_l.append(gate.reshape(-1)[rank * Sl:(rank + 1) * Sl].clone())
+        del ids, gate
+    layers = [shard.TokenShardedLayer(rig.ctx, rank, world) for _ in range(n)]
+    with torch.cuda.stream(stream):
+        for _ in range(3):
+            for i in range(n):
+                layers[i].step(ids_l[i], gate_l[i])
+    stream.synchronize()
+    use_graph = not (dist.is_available() and dist.is_initialized())
+    if use_graph:
+        g = capture([lambda i=i: layers[i].step(ids_l[i], gate_l[i]) for i in range(n)], stream)
+        ms, _ = time_graph(g, stream, reps)
+        ms /= n
+    else:                                   # the collective is enqueued by torch.distributed: timed as launched
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        dist.barrier()
+        torch.cuda.synchronize(device)
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for _ in range(reps):
+                for i in range(n):
+                    layers[i].step(ids_l[i], gate_l[i])
+            e1.record(stream)
+        stream.synchronize()
+        ms = shard.reduce_max_time(e0.elapsed_time(e1) / (reps * n))
+    # every rank must hold the identical plan: compare a digest of (lambda, plan arrays) over ranks
+    L0 = layers[0]
+    dig = torch.stack([L0.expert_count.sum(dtype=torch.int64), L0.plan.inst_cum.sum(dtype=torch.int64),
+                       L0.plan.inst_rank.sum(dtype=torch.int64), L0.plan.scalars[binding.SC_TAU].to(torch.int64)])
+    same = True
+    if not use_graph:
+        lo, hi = dig.clone(), dig.clone()
+        dist.all_reduce(lo, op=dist.ReduceOp.MIN)
+        dist.all_reduce(hi, op=dist.ReduceOp.MAX)
+        same = bool((lo == hi).all())
+    rps = c["R"] // world
+    fly = int(L0.n_inflight[rank * rps:(rank + 1) * rps].sum())
+    return {"us_per_layer": round(ms * 1e3, 2), "n_shards": world, "slots_per_gpu": Sl,
+            "allgather_bytes_per_gpu": layers[0].n_bytes, "cuda_graph": use_graph,
+            "plans_identical_over_ranks": same, "lambda_sum": int(dig[0]),
+            "inflight_ratio_this_shard": round(fly / max(Sl, 1), 4),
+            "note": "uep_shard_count -> all-gather of count rows (torch.distributed, in place in the workspace) -> "
+                    "uep_shard_finish; one layer of T tokens split over the GPUs (strong scaling of the plan "
+                    "latency), max over ranks; `value` above is the weak-scaling instance-sharded number"}
 
 
 def run_uep(args):
@@ -364,6 +428,12 @@ def run_uep(args):
             for i in range(n_inst):
                 rig.remap(i)
         stream.synchronize()
+    tok = None
+    if c["T"] % c["R"] == 0 and c["R"] % world == 0 and (c["T"] * c["k"]) % world == 0:
+        try:
+            tok = run_token_sharded(c, rig, world, rank, device, stream, reps)
+        except Exception as ex:              # an extra line must never take the bench line down
+            tok = {"error": repr(ex)[:300]}
     clocks = sampler.stop()
     chain_ms = barrier_and_max(world, chain_ms, device)
     # whole-job aggregate: `world` ranks each planned n_inst layers in chain_ms (max over ranks)
@@ -446,6 +516,7 @@ def run_uep(args):
                      "note": "uep_grad_reduce: fp32 [E, %d] main + [R, n_slot, %d] slot grads, bytes = 2 x (groups + replicas) x B; "
                              "uep_remap_inverse: 8 B/slot read, 4 B/slot scattered write" % (g_elems, g_elems)},
         "source_aware_remap": local,
+        "token_sharded": tok,
         "roofline": {k: r_pack[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")},
         "rooflines": rooflines,
         "gpu_launches": 6 * K,
@@ -651,8 +722,8 @@ def main():
     result["e2e"] = run_e2e(rig, info, max(4, min(args.steps, 16)))
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         result["cpu_baseline"] = cpu_baseline(rig.c)
-    if world > 1:
-        import torch.distributed as dist
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
         dist.barrier()
         dist.destroy_process_group()
     if rank == 0:

@@ -51,7 +51,8 @@ def exchange_counts(ws, offset0: int, n_bytes: int, rank: int, world: int, group
     after the call every rank holds all of them.  Enqueued on the current stream under NCCL."""
     import torch.distributed as dist
     assert 0 <= rank < world and n_bytes >= 0
-    if world == 1 or n_bytes == 0:
+    if n_bytes == 0 or not (dist.is_available() and dist.is_initialized()):
+        assert world == 1 or n_bytes == 0, "world > 1 needs an initialised process group"
         return
     region = ws[offset0:offset0 + world * n_bytes]
     mine = region[rank * n_bytes:(rank + 1) * n_bytes]
