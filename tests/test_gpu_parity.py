@@ -670,3 +670,51 @@ def test_token_shard_argument_errors():
     with pytest.raises(binding.UepError):                        # T % R != 0: unsupported
         c2 = binding.Context(4098, 2, 16, 4, 1, 64)
         c2.uep_shard_count(0, 2, ids, c2.new_workspace())
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_random_shapes_fuzz(seed):
+    """Seeded random walk over the argument space (shapes incl. E, R not powers of two and E < R,
+    k, n_slot 0..4, u_min, beta, both floor modes, home maps, skew, invalid ids, with/without
+    gates, uep_balance or the four calls): everything bit-exact against the oracle."""
+    import random
+    rng = random.Random(seed)
+    for _ in range(120):
+        k = rng.choice([1, 2, 4, 8])
+        E = rng.choice([1, 2, 3, 7, 16, 33, 64, 100, 128, 255, 256, 300, 512, rng.randint(1, 512)])
+        R = rng.choice([1, 2, 4, 8, 16, 32, 64, 128, 256, rng.randint(1, 256)])
+        n_slot = rng.randint(0, 4)
+        T = rng.choice([1, 5, 64, 1000, 4096, 10000, rng.randint(1, 20000)])
+        k = k if k <= E else 1
+        S = T * k
+        u_min = rng.choice([1, 2, 7, max(1, S // R // 32), max(1, S // R // 8), max(1, S // R // 2),
+                            rng.randint(1, max(1, S // R))])
+        beta = rng.choice([(101, 100), (1, 1), (11, 10), (3, 2), (1001, 1000)])
+        strict = rng.random() < 0.5
+        kind = rng.choice(["zipf", "zipf", "zipf", "uniform", "one", "few"])
+        sd = rng.randint(0, 1 << 30)
+        g = torch.Generator().manual_seed(sd)
+        if kind == "zipf":
+            ids = synth.zipf_topk_ids(T, k, E, rng.choice([0.0, 0.6, 1.0, 1.4, 2.0, 3.0]), sd)
+        elif kind == "uniform":
+            ids = torch.randint(0, E, (T, k), dtype=torch.int32, generator=g)
+        elif kind == "one":
+            ids = torch.full((T, k), rng.randrange(E), dtype=torch.int32)
+        else:
+            few = torch.tensor([rng.randrange(E) for _ in range(3)], dtype=torch.int32)
+            ids = few[torch.randint(0, 3, (T, k), generator=g)]
+        if rng.random() < 0.3:
+            bad = torch.tensor(rng.choice([-1, E, 1 << 20]), dtype=torch.int32)
+            ids = torch.where(torch.rand((T, k), generator=g) < 0.01, bad, ids)
+        gate = None if rng.random() < 0.2 else synth.gates_uniform_renorm(T, k, sd)
+        home = np.random.default_rng(sd).integers(0, R, size=E).astype(np.int32) if rng.random() < 0.25 else None
+        case = dict(T=T, k=k, E=E, R=R, n_slot=n_slot, u_min=u_min, beta=beta, strict=strict, kind=kind, sd=sd)
+        try:
+            go = gpu_chain(ids, gate, E, R, n_slot, u_min,
+                           binding.FLOOR_STRICT if strict else binding.FLOOR_TOLERANT, home, beta=beta,
+                           use_balance=rng.random() < 0.5)
+            oo = oracle_chain(ids, gate, E, R, n_slot, u_min,
+                              oracle.FLOOR_STRICT if strict else oracle.FLOOR_TOLERANT, home, beta=beta)
+            assert_parity(go, oo, ids, gate)
+        except Exception as ex:                                  # name the case that failed
+            raise AssertionError(f"fuzz case {case}") from ex
