@@ -48,6 +48,9 @@ def parse_args():
     ap.add_argument("--size-sweep", action="store_true",
                     help="instead of the bench line: stage times and roofline fractions at E=256, k=8, "
                          "R=64 over S = 256 Ki .. 16 Mi slots, one JSON line per size (DESIGN.md §7)")
+    ap.add_argument("--pack-grid-sweep", action="store_true",
+                    help="instead of the bench line: uep_pack and uep_grad_reduce throughput over the number of "
+                         "streaming CTAs (developer override UEP_PACK_CTAS), one JSON line per grid size")
     ap.add_argument("--state-scale", type=float, default=1.0,
                     help="shrink bytes per expert (debug only; the line then says so)")
     return ap.parse_args()
@@ -707,10 +710,73 @@ def run_size_sweep(args):
         torch.cuda.synchronize(dev)
 
 
+def run_pack_grid_sweep(args):
+    """uep_pack / uep_grad_reduce throughput against the number of persistent CTAs (the library's
+    own choice is printed first).  Same workload, plans and buffers for every grid size; every
+    launch event-timed alone, median of 16; bytes = the algorithmic bytes of DESIGN.md §6."""
+    import torch
+    from paper_2606_04101_b200 import binding, synth
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device; no CPU fallback"
+    dev = torch.device("cuda", torch.cuda.current_device())
+    peak_gbs, peak_src = measured_peaks()
+    c = workload(args.workload, args.state_scale)
+    n_inst = 4
+    inputs = [instance_inputs(c, i, dev) for i in range(n_inst)]
+    elems = c["state"][0][1]
+    src = [synth.expert_state(c["E"], elems, 7, dtype=torch.bfloat16, device=dev)]
+    dst = [torch.zeros((c["R"], c["n_slot"], elems), dtype=torch.bfloat16, device=dev)]
+    g_elems = elems // 2                       # fp32 gradients of the same byte size
+    mg = [torch.zeros((c["E"], g_elems), dtype=torch.float32, device=dev)]
+    sg = [torch.ones((c["R"], c["n_slot"], g_elems), dtype=torch.float32, device=dev)]
+    st = torch.cuda.Stream(dev)
+    for n_ctas in [None, 64, 96, 112, 120, 124, 126, 128, 130, 131, 132, 133, 134, 136, 140, 144, 148]:
+        if n_ctas is None:
+            os.environ.pop("UEP_PACK_CTAS", None)
+        else:
+            os.environ["UEP_PACK_CTAS"] = str(n_ctas)
+        ctx = binding.Context(c["T"], c["k"], c["E"], c["R"], c["n_slot"], c["u_min"], device=dev)
+        ws = ctx.new_workspace()
+        plans = [ctx.new_plan() for _ in range(n_inst)]
+        cnt = torch.zeros(c["E"], dtype=torch.int32, device=dev)
+        tp, tr = [], []
+        with torch.cuda.stream(st):
+            for i in range(n_inst):
+                ctx.uep_histogram(inputs[i][0], cnt, ws)
+                ctx.uep_plan(cnt, plans[i], ws)
+            st.synchronize()
+            moved = []
+            for i in range(n_inst):
+                sc = plans[i].scalars.cpu().numpy()
+                moved.append(int(sc[binding.SC_N_GROUPS]) + int(sc[binding.SC_N_REPLICAS]))
+            for rep in range(5):               # first pass = warm-up
+                for i in range(n_inst):
+                    e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+                    e[0].record(st)
+                    ctx.uep_pack(plans[i], src, dst)
+                    e[1].record(st)
+                    ctx.uep_grad_reduce(plans[i], mg, sg)
+                    e[2].record(st)
+                    st.synchronize()
+                    if rep:
+                        tp.append(moved[i] * elems * 2 / (e[0].elapsed_time(e[1]) * 1e-3) / 1e9)
+                        tr.append(2 * moved[i] * g_elems * 4 / (e[1].elapsed_time(e[2]) * 1e-3) / 1e9)
+        print(json.dumps({"workload": args.workload, "pack_ctas": ctx.launch_info["pack_ctas"],
+                          "library_default": n_ctas is None,
+                          "pack_gbs": round(statistics.median(tp), 1), "pack_frac": round(statistics.median(tp) / peak_gbs, 4),
+                          "grad_reduce_gbs": round(statistics.median(tr), 1),
+                          "grad_reduce_frac": round(statistics.median(tr) / peak_gbs, 4),
+                          "peak_gbs": peak_gbs, "peak_source": peak_src}), flush=True)
+        del ctx, ws, plans
+    os.environ.pop("UEP_PACK_CTAS", None)
+
+
 def main():
     args = parse_args()
     if args.size_sweep:
         run_size_sweep(args)
+        return
+    if args.pack_grid_sweep:
+        run_pack_grid_sweep(args)
         return
     if args.impl == "reference":
         out = run_reference(args)

@@ -9,9 +9,9 @@
 // CTA drives a ring of kPackStages shared-memory tiles: cp.async.bulk global->shared
 // (complete_tx on an mbarrier), then one cp.async.bulk shared->global per destination,
 // committed as a bulk group; a stage is refilled once the group that read it has drained
-// (cp.async.bulk.wait_group.read).  The grid is static (graph-capturable); the work list is
-// read from the plan on the device: CTA c takes tiles c, c+G, ... of every replicated expert,
-// rotated per (expert, tensor) so that remainders spread evenly.
+// (cp.async.bulk.wait_group.read).  The grid is static and persistent (graph-capturable); the
+// work list is read from the plan on the device and handed out in batches from a self-resetting
+// counter (see pack_kernel).
 #include "uep_internal.cuh"
 
 namespace uep {
@@ -61,15 +61,9 @@ __device__ __forceinline__ void bulk_wait_read() {
 }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-// Enumerates this CTA's units in a fixed order: experts ascending (only those with replicas),
-// tensors ascending, tiles c' , c'+G, ...   A unit = one source tile and its destinations.
-struct UnitIter {
-  int e, j;
-  long long tile;        // tile index inside tensor j of expert e
-  unsigned rot;          // running rotation so that tile remainders spread over CTAs
-  __device__ void init() { e = -1; j = 0; tile = 0; rot = 0; }
-};
-
+// A unit = one source tile and its destinations.  Units are numbered expert-major over the
+// replicated experts only: u = (index of e among replicated experts) * TPE + (tile index over the
+// expert's tensors in order), TPE = sum_j ceil(B_j / kPackTile).
 struct Unit {
   const unsigned char* src;
   unsigned long long dst_off;   // byte offset of the tile inside a slot of tensor j
@@ -77,52 +71,84 @@ struct Unit {
   int e, j;
 };
 
+constexpr unsigned kPackBatch = 8;       // units taken from the shared counter at a time (128 KB)
+
+// Work distribution is DYNAMIC: CTAs take batches of kPackBatch consecutive units from a counter
+// in global memory (ctr[0]; the next batch is requested while the current one is being
+// processed, so the L2 round trip is hidden).  With a static equal split the kernel ran at the
+// pace of its slowest SM: SMs do not all see the same bandwidth (148 streaming CTAs: 0.89 of the
+// copy peak; the same static split on 128: 0.97; and 0.86 again when the CTAs landed unevenly
+// behind a still-running lookup_kernel).  The last CTA to finish resets the counters (ctr[1]
+// counts finished CTAs), so the launch stays graph-replayable.
 __global__ void __launch_bounds__(kPackThreads, 1)
 pack_kernel(PackArgs a, int E, int n_slot, int M, const int32_t* __restrict__ inst_off,
-            const int32_t* __restrict__ inst_rank, const int32_t* __restrict__ inst_phys) {
+            const int32_t* __restrict__ inst_rank, const int32_t* __restrict__ inst_phys,
+            unsigned* __restrict__ ctr) {
   extern __shared__ __align__(128) unsigned char pack_smem[];
   __shared__ __align__(8) uint64_t full[kPackStages];
   __shared__ Unit ring[kPackStages];
-  if (threadIdx.x != 0) return;                         // one elected thread drives the TMA engine
-  const int G = gridDim.x, c = blockIdx.x;
+  __shared__ short rexp[UEP_MAX_E];                     // replicated experts, ascending
+  const int lane = threadIdx.x;
+  int n_rexp = 0;
+  for (int base = 0; base < E; base += 32) {            // warp-cooperative compaction
+    const int e = base + lane;
+    const bool r = e < E && __ldg(inst_off + e + 1) - __ldg(inst_off + e) > 1;
+    const unsigned m = __ballot_sync(0xffffffffu, r);
+    if (r) rexp[n_rexp + __popc(m & ((1u << lane) - 1u))] = (short)e;
+    n_rexp += __popc(m);
+  }
+  __syncwarp();
+  if (lane != 0) return;                                // one elected thread drives the TMA engine
   for (int s = 0; s < kPackStages; ++s) mbar_init(&full[s], 1);
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 
-  UnitIter it;
-  it.init();
-  // advance the iterator to this CTA's next unit; false when exhausted
+  unsigned tiles_of[UEP_MAX_TENSORS];
+  unsigned tpe = 0;
+#pragma unroll
+  for (int j = 0; j < UEP_MAX_TENSORS; ++j) {
+    tiles_of[j] = j < a.n_tensors ? (unsigned)((a.bytes[j] + kPackTile - 1) / kPackTile) : 0u;
+    tpe += tiles_of[j];
+  }
+  const unsigned total = (unsigned)n_rexp * tpe;        // < 2^31: checked by launch_pack
+
+  // batch state: units [cur, cur_end) decoded incrementally as (ri, j, tile)
+  unsigned cur = 0, cur_end = 0, ri = 0, tile = 0;
+  int j = 0;
+  unsigned nxt = atomicAdd(ctr, kPackBatch);            // first batch
+  bool more = true;
   auto next = [&](Unit& u) -> bool {
-    while (true) {
-      if (it.e >= 0 && it.e < E) {
-        while (it.j < a.n_tensors) {
-          const unsigned long long B = a.bytes[it.j];
-          const long long tiles = (long long)((B + kPackTile - 1) / kPackTile);
-          if (it.tile < tiles) {
-            const unsigned long long off = (unsigned long long)it.tile * kPackTile;
-            u.src = a.src[it.j] + (unsigned long long)it.e * B + off;
-            u.dst_off = off;
-            u.bytes = (uint32_t)min((unsigned long long)kPackTile, B - off);
-            u.e = it.e; u.j = it.j;
-            it.tile += G;
-            return true;
-          }
-          it.rot = (unsigned)((it.rot + tiles) % (unsigned)G);
-          it.j += 1;
-          it.tile = (c + G - (int)it.rot) % G;
-        }
-      }
-      // next replicated expert
-      int e = it.e + 1;
-      while (e < E && inst_off[e + 1] - inst_off[e] <= 1) ++e;
-      if (e >= E) { it.e = E; return false; }
-      it.e = e; it.j = 0;
-      it.tile = (c + G - (int)it.rot) % G;
+    if (cur == cur_end) {
+      if (nxt >= total) return false;
+      cur = nxt;
+      cur_end = min(nxt + kPackBatch, total);
+      nxt = atomicAdd(ctr, kPackBatch);                 // requested now, needed a batch later
+      ri = cur / tpe;
+      unsigned r = cur - ri * tpe;
+      j = 0;
+      while (r >= tiles_of[j]) { r -= tiles_of[j]; ++j; }
+      tile = r;
     }
+    const unsigned long long B = a.bytes[j];
+    const unsigned long long off = (unsigned long long)tile * kPackTile;
+    u.e = rexp[ri]; u.j = j;
+    u.src = a.src[j] + (unsigned long long)u.e * B + off;
+    u.dst_off = off;
+    u.bytes = (uint32_t)min((unsigned long long)kPackTile, B - off);
+    ++cur;
+    if (++tile == tiles_of[j]) {
+      tile = 0;
+      do { ++j; } while (j < a.n_tensors && tiles_of[j] == 0);
+      if (j >= a.n_tensors) {
+        ++ri;
+        j = 0;
+        while (j < a.n_tensors && tiles_of[j] == 0) ++j;
+      }
+    }
+    return true;
   };
 
   long long n_loaded = 0, n_stored = 0;
-  bool more = true;
   auto issue_load = [&]() {
     Unit u;
     if (!more || !(more = next(u))) return;
@@ -154,6 +180,13 @@ pack_kernel(PackArgs a, int E, int n_slot, int M, const int32_t* __restrict__ in
     bulk_commit();
     ++n_stored;
   }
+  // every request of this CTA has returned; the last CTA to get here rearms the counters
+  __threadfence();
+  if (atomicAdd(ctr + 1, 1u) == gridDim.x - 1) {
+    ctr[0] = 0u;
+    ctr[1] = 0u;
+    __threadfence();
+  }
   bulk_wait_all();
 }
 
@@ -164,8 +197,11 @@ int init_pack_kernels() {
 }
 
 int launch_pack(const Ctx* c, const uep_plan_out& plan, const PackArgs& a, cudaStream_t s) {
+  unsigned long long tpe = 0;
+  for (int j = 0; j < a.n_tensors; ++j) tpe += (a.bytes[j] + kPackTile - 1) / kPackTile;
+  if (tpe * (unsigned long long)c->cfg.E >= (1ull << 31) - (unsigned long long)kPackBatch * 4096) return UEP_ERR_UNSUPPORTED;
   pack_kernel<<<c->pack_ctas, kPackThreads, kPackStages * kPackTile, s>>>(
-      a, c->cfg.E, c->cfg.n_slot, c->M, plan.inst_off, plan.inst_rank, plan.inst_phys);
+      a, c->cfg.E, c->cfg.n_slot, c->M, plan.inst_off, plan.inst_rank, plan.inst_phys, next_counter(c));
   UEP_CUDA_TRY(cudaGetLastError());
   return UEP_OK;
 }

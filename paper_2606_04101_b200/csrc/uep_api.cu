@@ -19,6 +19,12 @@ int set_cuda_error(cudaError_t e) {
   return UEP_ERR_CUDA;
 }
 
+unsigned* next_counter(const Ctx* c) {
+  Ctx* m = const_cast<Ctx*>(c);                // the round-robin index is the context's only mutable state
+  const unsigned i = __atomic_fetch_add(&m->ctr_next, 1u, __ATOMIC_RELAXED);
+  return m->d_ctr + 2 * (i % kCtrSlots);
+}
+
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
 static int check_plan_ptrs(const Ctx* c, const uep_plan_out* p) {
@@ -135,7 +141,13 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
       c->l_group_len = (int)block;
     }
   }
+  // pack / grad_reduce grid: one persistent streaming CTA per SM; the tiles are handed out
+  // dynamically (profiles/r01_pack_grid.md: a static split is bound by the slowest SM)
   c->pack_ctas = c->sm_count;
+  if (const char* v = getenv("UEP_PACK_CTAS")) {        // developer sweeps only
+    const int n = atoi(v);
+    if (n >= 1 && n <= 16 * c->sm_count) c->pack_ctas = n;
+  }
 
   auto fail = [&](int rc) { uep_destroy(reinterpret_cast<uep_ctx*>(c)); return rc; };
   cudaError_t e;
@@ -144,6 +156,8 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   UEP_TRY_OR_FAIL(cudaMalloc(&c->d_main_phys, sizeof(int32_t) * E));
   UEP_TRY_OR_FAIL(cudaMalloc(&c->d_roff, sizeof(int32_t) * (R + 1)));
   UEP_TRY_OR_FAIL(cudaMalloc(&c->d_rexp, sizeof(int32_t) * E));
+  UEP_TRY_OR_FAIL(cudaMalloc(&c->d_ctr, sizeof(unsigned) * 2 * kCtrSlots));
+  UEP_TRY_OR_FAIL(cudaMemset(c->d_ctr, 0, sizeof(unsigned) * 2 * kCtrSlots));
   UEP_TRY_OR_FAIL(cudaMemcpy(c->d_home, home.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
   UEP_TRY_OR_FAIL(cudaMemcpy(c->d_main_phys, main_phys.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
   UEP_TRY_OR_FAIL(cudaMemcpy(c->d_roff, roff.data(), sizeof(int32_t) * (R + 1), cudaMemcpyHostToDevice));
@@ -170,6 +184,7 @@ void uep_destroy(uep_ctx* ctx) {
   if (c->d_main_phys) cudaFree(c->d_main_phys);
   if (c->d_roff) cudaFree(c->d_roff);
   if (c->d_rexp) cudaFree(c->d_rexp);
+  if (c->d_ctr) cudaFree(c->d_ctr);
   if (c->side) cudaStreamDestroy(c->side);
   if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->ev_join) cudaEventDestroy(c->ev_join);

@@ -46,10 +46,18 @@ struct Ctx {
   int32_t* d_main_phys;   // [E]   index of e among E_{h(e)} ascending
   int32_t* d_roff;        // [R+1] CSR of E_r
   int32_t* d_rexp;        // [E]   experts grouped by home rank, ascending e
+  // work counters of the streaming kernels (pack, grad_reduce): kCtrSlots pairs {next unit,
+  // finished CTAs}, zero between launches (the kernels rearm them); launches take the pairs round
+  // robin, so up to kCtrSlots such kernels of one context may be in flight at a time
+  unsigned* d_ctr;
+  unsigned ctr_next;      // host, advanced atomically
   // fork/join for uep_balance
   cudaStream_t side;
   cudaEvent_t ev_fork, ev_join, ev_rank;
 };
+
+constexpr int kCtrSlots = 64;
+unsigned* next_counter(const Ctx* c);     // the next {unit, done} counter pair (thread-safe)
 
 struct PackArgs {
   const unsigned char* src[UEP_MAX_TENSORS];
