@@ -22,7 +22,10 @@
  *     a workspace may not (one per in-flight call).  uep_balance uses the context's internal
  *     side stream and events: calls of uep_balance on one context must be issued from one host
  *     thread at a time (they may target different streams; create one context per concurrent
- *     host thread).
+ *     host thread).  uep_pack / uep_grad_reduce take their work counter from a pool of 64 the
+ *     context owns (round robin, self-resetting): at most 64 such kernels of one context may be
+ *     executing at the same time, and one captured graph must not be replayed concurrently with
+ *     itself.
  *   - data faults that would need a sync to report (an id outside [0,E)) are counted on the
  *     device (scalars[UEP_SC_N_INVALID]) and the slot is skipped (S14).
  *   - all DEVICE pointers must be 16-byte aligned.
