@@ -718,3 +718,86 @@ def test_random_shapes_fuzz(seed):
             assert_parity(go, oo, ids, gate)
         except Exception as ex:                                  # name the case that failed
             raise AssertionError(f"fuzz case {case}") from ex
+
+
+def _seq_grad(p, m, x):
+    """sequential fp32 sum in instance order (what the kernel must reproduce bit for bit)"""
+    seq = m.copy()
+    for e in range(p.E):
+        for i in range(p.inst_off[e] + 1, p.inst_off[e + 1]):
+            seq[e] = seq[e] + x[p.inst_rank[i], p.inst_phys[i] - p.M]
+    return seq
+
+
+@pytest.mark.parametrize("seed", [0, 1])
+def test_streaming_kernels_odd_sizes_streams_and_replay(seed):
+    """pack / grad_reduce hand their tiles out from self-resetting counters: tensor sizes that are
+    not a multiple of the tile (down to 16 B), up to 8 tensors, launches in flight on three streams
+    of one context at once, and graph replays must all stay byte-exact / bit-exact."""
+    import random
+    rng = random.Random(seed)
+    T, k, E, R, n_slot = 16384, 4, 64, 16, 2
+    um = synth.stress_u_min(T * k, R)
+    ctx = binding.Context(T, k, E, R, n_slot, um, gate_dtype=binding.GATE_NONE)
+    plans, oplans = [], []
+    for i in range(3):
+        ids = synth.zipf_topk_ids(T, k, E, 1.2 + 0.4 * i, 10 * seed + i)
+        ws, plan = ctx.new_workspace(), ctx.new_plan()
+        count = torch.zeros(E, dtype=torch.int32, device=DEV)
+        ctx.uep_histogram(ids.to(DEV), count, ws)
+        ctx.uep_plan(count, plan, ws)
+        lam, _ = oracle.histogram(ids.numpy(), E)
+        plans.append(plan)
+        oplans.append(oracle.plan(lam, R, n_slot, um, S_total=T * k))
+        assert oplans[-1].n_replicas > 0
+    sizes = [16, 48, 8192, 16384, 16400, 40000 // 16 * 16, 1 << 20, rng.randrange(1, 9000) * 16]
+    nt = [8, 3, 1]
+    g = torch.Generator().manual_seed(seed)
+    srcs, dsts, sents, mains, slots, dmain, dslot = [], [], [], [], [], [], []
+    for i in range(3):                                       # one tensor set per stream
+        bs = rng.sample(sizes, nt[i])
+        srcs.append([torch.randint(0, 256, (E, b), dtype=torch.uint8, generator=g).to(DEV) for b in bs])
+        sents.append([torch.randint(0, 256, (R, n_slot, b), dtype=torch.uint8, generator=g) for b in bs])
+        dsts.append([s.to(DEV) for s in sents[i]])
+        mains.append([torch.randn((E, b // 4), generator=g) for b in bs])
+        slots.append([torch.randn((R, n_slot, b // 4), generator=g) for b in bs])
+        dmain.append([m.to(DEV) for m in mains[i]])
+        dslot.append([x.to(DEV) for x in slots[i]])
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    torch.cuda.synchronize()
+    for rep in range(3):                                     # pack is idempotent: repeat it
+        for i, st in enumerate(streams):
+            with torch.cuda.stream(st):
+                ctx.uep_pack(plans[i], srcs[i], dsts[i])
+    for i, st in enumerate(streams):
+        with torch.cuda.stream(st):
+            ctx.uep_grad_reduce(plans[i], dmain[i], dslot[i])
+            ctx.uep_grad_reduce(plans[i], dmain[i], dslot[i])   # slots are zero now: adds nothing
+    torch.cuda.synchronize()
+    for i in range(3):
+        p = oplans[i]
+        for s_, d_, sn in zip(srcs[i], dsts[i], sents[i]):
+            ref = sn.numpy().reshape(R, n_slot, -1).copy()
+            oracle.pack(p.slot_expert, np.ascontiguousarray(s_.cpu().numpy()), ref)
+            assert np.array_equal(d_.cpu().numpy(), ref)
+        for m, x, dm, dx in zip(mains[i], slots[i], dmain[i], dslot[i]):
+            assert np.array_equal(dm.cpu().numpy(), _seq_grad(p, m.numpy(), x.numpy()))
+            _, s_ref = oracle.grad_reduce(p, m.numpy(), x.numpy())
+            assert np.array_equal(dx.cpu().numpy(), s_ref)
+    # graph replay: the counters must be rearmed by every launch
+    st = streams[0]
+    for d_, sn in zip(dsts[0], sents[0]):
+        d_.copy_(sn)
+    gr = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(st):
+        with torch.cuda.graph(gr, stream=st):
+            ctx.uep_pack(plans[0], srcs[0], dsts[0])
+            ctx.uep_pack(plans[1], srcs[0], dsts[0])
+        for _ in range(4):
+            gr.replay()
+    torch.cuda.synchronize()
+    for s_, d_, sn in zip(srcs[0], dsts[0], sents[0]):       # plan 0 then plan 1 over the same buffers
+        ref = sn.numpy().reshape(R, n_slot, -1).copy()
+        oracle.pack(oplans[0].slot_expert, np.ascontiguousarray(s_.cpu().numpy()), ref)
+        oracle.pack(oplans[1].slot_expert, np.ascontiguousarray(s_.cpu().numpy()), ref)
+        assert np.array_equal(d_.cpu().numpy(), ref)
