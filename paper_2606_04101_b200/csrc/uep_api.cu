@@ -432,6 +432,9 @@ int uep_shard_finish(const uep_ctx* ctx, int32_t shard, int32_t n_shards, const 
   rc = launch_prefix(c, ws, s, /*local=*/true);
   // lambda_e = totals row of the scanned table; the planner publishes it as expert_count
   int32_t* totals = ws_prefix(c, ws) + (size_t)c->l_chunks * c->E_pad;
+  // (the planner is NOT launched programmatically dependent on prefix_kernel: the lookup behind it
+  // reads the prefix rows in its prologue, before its own griddepcontrol.wait, and an early planner
+  // would let that prologue start while prefix_kernel is still running)
   if (rc == UEP_OK) rc = launch_plan(c, nullptr, *plan, s, /*pdl=*/false, 1, totals, expert_count);
   const size_t gb = c->cfg.gate_dtype == UEP_GATE_BF16 ? 2 : 4;
   if (rc == UEP_OK)
