@@ -57,9 +57,10 @@ struct PlanSmem {
   int order[UEP_MAX_R];        // ranks by l_r desc, id asc
   int roff[UEP_MAX_R + 1];
   int rload[UEP_MAX_R];
-  int s_ell[UEP_MAX_R];        // l_r in visit order
-  int v_off[UEP_MAX_R + 1];    // CSR of the flat visit list: experts of the oi-th visited rank
-  int v_lam[UEP_MAX_E];        // lambda_e in visit order
+  // (padded: the probe reads one entry ahead of the one it is working on)
+  int s_ell[UEP_MAX_R + 1];    // l_r in visit order
+  int v_off[UEP_MAX_R + 2];    // CSR of the flat visit list: experts of the oi-th visited rank
+  int v_lam[UEP_MAX_E + 1];    // lambda_e in visit order
   int v_e[UEP_MAX_E];          // expert ids in visit order
   int dscan[kMaxLog];
   int log_n[2][kPlanMaxNodes]; // accepted transfers of the probe at each tree node (per round parity)
@@ -122,13 +123,21 @@ __device__ __forceinline__ bool probe(const PlanSmem& sm, const int tau, const i
   }
   const int brk = strict ? 1 : u_min;        // a rank is drained when exc < brk (S8)
   int nl = 0;
+  // the visit list is read one entry ahead (next rank's load and list end, next expert's lambda):
+  // the shared-memory latency of those loads is then off the probe's dependent chain
+  int nxt_ell = sm.s_ell[0], nxt_b = sm.v_off[1], b = sm.v_off[0];
   for (int oi = 0; oi < R; ++oi) {                                  // line 8
-    int exc = sm.s_ell[oi] - tau;
+    int exc = nxt_ell - tau;
     if (exc < brk) break;                      // ranks are sorted: every later rank is drained too
-    const int a = sm.v_off[oi], b = sm.v_off[oi + 1];
+    const int a = b;
+    b = nxt_b;
+    nxt_ell = sm.s_ell[oi + 1];
+    nxt_b = sm.v_off[oi + 2];
+    int nxt_cap = sm.v_lam[a];
     bool dead = false;     // no rank can absorb u_min any more: slack only shrinks, so it stays so
     for (int ei = a; ei < b && exc >= u_min; ++ei) {                // line 9
-      int cap = sm.v_lam[ei];                                       // line 10 (S6)
+      int cap = nxt_cap;                                            // line 10 (S6)
+      nxt_cap = sm.v_lam[ei + 1];
       if (cap < u_min) break;                  // sorted by lambda: no later expert can pass line 16
       do {                                                          // line 11
         unsigned kl = key[0];
@@ -164,7 +173,7 @@ __device__ __forceinline__ bool probe(const PlanSmem& sm, const int tau, const i
     if (exc >= brk) { n_log = nl; return false; }
     if (dead) {            // nothing can be moved any more: feasible iff no later rank needs to
       n_log = nl;
-      return (oi + 1 >= R) || (sm.s_ell[oi + 1] - tau < brk);
+      return (oi + 1 >= R) || (nxt_ell - tau < brk);
     }
   }
   n_log = nl;
