@@ -603,8 +603,10 @@ def cpu_inputs(c, idx):
     return ids.numpy(), g
 
 
-def cpu_baseline(c, n_samples=3, pack_frac=16):
-    """The oracle as it stands, single-threaded, on this box's host cores, on a bounded sample."""
+def cpu_baseline(c, n_samples=12, pack_frac=16, reps=32):
+    """The oracle as it stands, single-threaded, on this box's host cores, on a bounded sample
+    (about 10 s of CPU work at the DeepSeek-V3 shape: n_samples instances x reps passes of
+    histogram+plan+remap, and the pack of 1/pack_frac of every expert's bytes)."""
     import numpy as np
     B = sum(e * _DT[dt][1] for _, e, dt in c["state"])
     src = np.zeros((c["E"], max(16, B // pack_frac // 16 * 16)), dtype=np.uint8)
@@ -612,9 +614,10 @@ def cpu_baseline(c, n_samples=3, pack_frac=16):
     acc = {}
     for i in range(n_samples):
         ids, g = cpu_inputs(c, i)
-        t, _ = oracle_step(c, ids, g, pack_frac, src if i == 0 else None)
-        for k, v in t.items():
-            acc.setdefault(k, []).append(v)
+        for r in range(reps):
+            t, _ = oracle_step(c, ids, g, pack_frac, src if (i < 4 and r == 0) else None)
+            for k, v in t.items():
+                acc.setdefault(k, []).append(v)
     st = {k: round(statistics.mean(v) * 1e6, 1) for k, v in acc.items()}
     try:
         model = [l.split(":")[1].strip() for l in open("/proc/cpuinfo") if l.startswith("model name")][0]
@@ -623,9 +626,9 @@ def cpu_baseline(c, n_samples=3, pack_frac=16):
     return {"value": round(st["histogram"] + st["plan"] + st["remap"], 1), "unit": UNIT, "cores": 1,
             "kind": "oracle", "host_cores": os.cpu_count(), "cpu_model": model,
             "stages_us": st,
-            "sample": "%d instances of the workload for histogram+plan+remap (single thread, g++ -O2); "
-                      "pack timed on instance 0 over 1/%d of each expert's bytes and scaled x%d"
-                      % (n_samples, pack_frac, pack_frac)}
+            "sample": "%d instances of the workload x %d passes of histogram+plan+remap (single thread, g++ -O2); "
+                      "pack timed on 4 instances over 1/%d of each expert's bytes and scaled x%d"
+                      % (n_samples, reps, pack_frac, pack_frac)}
 
 
 def run_reference(args):
