@@ -308,21 +308,49 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   t_setup = clock64();
 #endif
 
-  // ---- bisection, `levels` levels per round (S9) ---------------------------------------------
-  // Tree node n (heap index, 1 .. 2^levels - 1) is probed by warp n / csize of CTA n % csize:
-  // with 8 CTAs and 6 levels that is <= 2 probes per scheduler, so every probe runs at the
-  // latency of its own dependent chain instead of queueing for issue slots on one SM.  The
-  // verdicts are written into EVERY CTA's shared memory (DSMEM), one cluster barrier per round,
-  // and every CTA walks the path redundantly (identical state everywhere, no broadcast back).
-  const int n_nodes = 1 << levels;
+  // ---- bisection (S9): per round up to 2^levels - 1 nodes of the SEQUENTIAL bisection tree rooted
+  // at the current [lo, hi) are probed speculatively, then the path the sequential search takes is
+  // walked as far as the verdicts reach.  Slot i of a round is probed by warp i / csize of CTA
+  // i % csize (with 8 CTAs and 6 levels <= 2 probes per scheduler, so every probe runs at the
+  // latency of its own dependent chain); the verdicts are written into EVERY CTA's shared memory
+  // (DSMEM), one cluster barrier per round, every CTA walks the path redundantly.
+  // WHICH nodes are speculated only decides how many rounds are needed, never the result:
+  //   * first round, more than `levels` levels to go: the tree is probed where the path is
+  //     expected — tau* sits at or just above tau_lo whenever the slots suffice to reach beta
+  //     (every probe on the path feasible: the all-left spine).  Nodes: the complete top
+  //     levels-2 levels, the spine below them, and the complete bottom levels-1 levels under
+  //     the spine (every tau* in [lo, lo + 2^(levels-1)) resolves in this ONE round, any other
+  //     still advances by at least levels-2 levels or to where it leaves the spine);
+  //   * otherwise the complete tree of the next `levels` levels.
+  // Nodes are named by their heap index in the tree rooted at [lo, hi) (1 = root, 2n = "n was
+  // feasible", 2n+1 = "n was infeasible"), at any depth.
+  const int n_slots = 1 << levels;
+  const int top_lv = levels - 2, bot_lv = levels - 1;
   int round = 0;
   while (true) {
     const int lo = sm.lo, hi = sm.hi;
     if (lo >= hi) break;                                            // line 4
     const int buf = round & 1;
-    const bool log_round = n_bufs > 1 && hi - lo < n_nodes;         // last round: log every probe
-    const int node = warp * csize + crank;
-    if (node >= 1 && node < n_nodes) {
+    const int depth_left = 32 - __clz(hi - lo);                     // levels on the all-feasible path
+    const int bot_depth = max(depth_left - (bot_lv - 1), top_lv + 1);   // depth of the bottom subtree's root
+    const int n_spine = bot_depth - 1 - top_lv;                     // spine nodes between top and bottom
+    const int first_spine = 1 << top_lv, first_bot = first_spine + n_spine;
+    const bool spine = round == 0 && depth_left > levels && top_lv >= 1 &&
+                       first_bot + (1 << bot_lv) - 1 <= n_slots;
+    // rounds whose probes may include the last feasible one log their accepted transfers
+    const bool log_round = n_bufs > 1 && (spine || hi - lo < n_slots);
+    auto node_of = [&](int slot) -> int {
+      if (slot < 1 || slot >= n_slots) return 0;
+      if (!spine || slot < first_spine) return slot;                // complete (top) levels
+      if (slot < first_bot) return 1 << (top_lv + slot - first_spine);          // depth top_lv+1+k, all-left
+      const int q = slot - first_bot + 1;                           // heap index inside the bottom subtree
+      if (q >= (1 << bot_lv)) return 0;
+      const int jl = 31 - __clz(q);
+      return ((1 << (bot_depth - 1)) << jl) + (q - (1 << jl));
+    };
+    const int slot = warp * csize + crank;
+    const int node = node_of(slot);
+    if (node >= 1) {
       const int depth = 31 - __clz(node);
       int l = lo, h = hi;
       bool valid = true;
@@ -348,23 +376,37 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
         if (lane < csize && round < 8) atomicMax(cluster.map_shared_rank(&sm.tmax[round], lane), (int)(clock64() - tp0));
 #endif
         if (lane < csize) {
-          *cluster.map_shared_rank(&sm.node_feas[buf][node], lane) = f ? 1 : 0;
-          *cluster.map_shared_rank(&sm.log_n[buf][node], lane) = nl;
+          *cluster.map_shared_rank(&sm.node_feas[buf][slot], lane) = f ? 1 : 0;
+          *cluster.map_shared_rank(&sm.log_n[buf][slot], lane) = nl;
         }
       }
     }
     if (csize > 1) cluster.sync(); else __syncthreads();
-    if (tid == 0) {
+    if (warp == 0) {
+      // walk the sequential path; lane i knows the nodes of slots i and i + 32.  A node on the
+      // path has a non-empty interval, so it was probed if it was speculated at all.
+      const int n0 = node_of(lane), n1 = node_of(lane + 32);
       int nd = 1, l = lo, h = hi, np = sm.n_probes, last_feas = -1;
-      while (nd < n_nodes && l < h) {
+      while (l < h) {
+        const unsigned m0 = __ballot_sync(kFull, n0 == nd), m1 = __ballot_sync(kFull, n1 == nd);
+        if ((m0 | m1) == 0u) break;                                 // not speculated: next round starts here
+        const int sl = m0 ? __ffs(m0) - 1 : 31 + __ffs(m1);
         const int mid = (l + h) >> 1;                               // line 5
         ++np;
-        if (sm.node_feas[buf][nd]) { h = mid; last_feas = nd; nd = 2 * nd; }   // lines 21-22
+        if (sm.node_feas[buf][sl]) { h = mid; last_feas = sl; nd = 2 * nd; }    // lines 21-22
         else { l = mid + 1; nd = 2 * nd + 1; }                      // line 24
       }
-      sm.lo = l; sm.hi = h; sm.n_probes = np;
-      // the probe at the final tau (= last feasible one) was logged iff this was a logging round
-      if (log_round && last_feas > 0) { sm.log_buf = last_feas; sm.n_log = sm.log_n[buf][last_feas]; }
+      if (lane == 0) {
+        sm.lo = l; sm.hi = h; sm.n_probes = np;
+        // the log of the last feasible probe on the path (= U~ of the final tau, S10) is usable iff
+        // that probe was logged and no later logging round has reused the buffers
+        if (last_feas > 0) {
+          if (log_round) { sm.log_buf = last_feas; sm.n_log = sm.log_n[buf][last_feas]; }
+          else sm.log_buf = -1;
+        } else if (log_round) {
+          sm.log_buf = -1;
+        }
+      }
     }
     __syncthreads();
     ++round;
