@@ -385,16 +385,44 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (warp == 0) {
       // walk the sequential path; lane i knows the nodes of slots i and i + 32.  A node on the
       // path has a non-empty interval, so it was probed if it was speculated at all.
+      // (verdicts in registers: a step of the walk is two ballots, no shared-memory load)
       const int n0 = node_of(lane), n1 = node_of(lane + 32);
+      const bool f0 = sm.node_feas[buf][lane] != 0, f1 = sm.node_feas[buf][lane + 32] != 0;
       int nd = 1, l = lo, h = hi, np = sm.n_probes, last_feas = -1;
-      while (l < h) {
-        const unsigned m0 = __ballot_sync(kFull, n0 == nd), m1 = __ballot_sync(kFull, n1 == nd);
-        if ((m0 | m1) == 0u) break;                                 // not speculated: next round starts here
-        const int sl = m0 ? __ffs(m0) - 1 : 31 + __ffs(m1);
+      {
+        // the run of feasible verdicts at the head of the path (usually the whole path) in one
+        // step: the all-left nodes are the powers of two; they are speculated at every depth up
+        // to spine_depth, and the first infeasible one ends the run
+        const int spine_depth = spine ? depth_left : min(levels, depth_left);
+        const bool s0 = n0 > 0 && (n0 & (n0 - 1)) == 0, s1 = n1 > 0 && (n1 & (n1 - 1)) == 0;
+        const int d0 = 32 - __clz(n0), d1 = 32 - __clz(n1);          // depth, root = 1
+        int dinf = spine_depth + 1;
+        if (s0 && !f0) dinf = min(dinf, d0);
+        if (s1 && !f1) dinf = min(dinf, d1);
+        dinf = __reduce_min_sync(kFull, dinf);                       // depth of the first infeasible all-left node
+        const int n_left = dinf - 1;                                 // feasible all-left nodes on the path
+        for (int q = 0; q < n_left; ++q) h = (l + h) >> 1;           // lines 5, 21-22, n_left times
+        np += n_left;
+        nd = 1 << n_left;
+        if (n_left > 0) {
+          const unsigned m0 = __ballot_sync(kFull, s0 && d0 == n_left);
+          const unsigned m1 = __ballot_sync(kFull, s1 && d1 == n_left);
+          last_feas = m0 ? __ffs(m0) - 1 : 31 + __ffs(m1);
+        }
+      }
+      while (l < h) {                                                // the rest of the path, node by node
+        const bool p0 = n0 == nd, p1 = n1 == nd;
+        const unsigned m = __ballot_sync(kFull, p0 || p1);
+        if (m == 0u) break;                                         // not speculated: next round starts here
+        const unsigned mf = __ballot_sync(kFull, (p0 && f0) || (p1 && f1));
         const int mid = (l + h) >> 1;                               // line 5
         ++np;
-        if (sm.node_feas[buf][sl]) { h = mid; last_feas = sl; nd = 2 * nd; }    // lines 21-22
-        else { l = mid + 1; nd = 2 * nd + 1; }                      // line 24
+        if (mf) {                                                   // lines 21-22
+          h = mid;
+          const unsigned m0 = __ballot_sync(kFull, p0);
+          last_feas = m0 ? __ffs(m0) - 1 : 31 + __ffs(m);
+          nd = 2 * nd;
+        } else { l = mid + 1; nd = 2 * nd + 1; }                    // line 24
       }
       if (lane == 0) {
         sm.lo = l; sm.hi = h; sm.n_probes = np;
