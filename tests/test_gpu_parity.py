@@ -801,3 +801,37 @@ def test_streaming_kernels_odd_sizes_streams_and_replay(seed):
         oracle.pack(oplans[0].slot_expert, np.ascontiguousarray(s_.cpu().numpy()), ref)
         oracle.pack(oplans[1].slot_expert, np.ascontiguousarray(s_.cpu().numpy()), ref)
         assert np.array_equal(d_.cpu().numpy(), ref)
+
+
+@pytest.mark.parametrize("n_slot,u_min,s,strict", [
+    (1, 1024, 1.0, False),     # tau* ~1000 above tau_lo: the path leaves the all-feasible spine mid-way
+    (2, 8192, 1.0, False),     # coarse floor
+    (2, 1024, 1.0, True),      # Alg. 1 verbatim: feasibility not monotone, tau* far from tau_lo
+    (4, 1, 2.0, True),         # u_min = 1: strict == tolerant, long accept lists
+    (2, 1024, 0.0, False),     # balanced input: few or no probes
+])
+def test_planner_paths_off_the_spine_full_size(n_slot, u_min, s, strict):
+    """The planner's first round speculates along the all-feasible spine of the bisection tree;
+    whatever the path really is, plan and scalars (tau, n_probes on the SEQUENTIAL path, ...) must
+    equal the oracle's.  DeepSeek-V3 shape, several instances each."""
+    T, k, E, R = 262144, 8, 256, 64
+    mode_g = binding.FLOOR_STRICT if strict else binding.FLOOR_TOLERANT
+    mode_o = oracle.FLOOR_STRICT if strict else oracle.FLOOR_TOLERANT
+    ctx = binding.Context(T, k, E, R, n_slot, u_min, floor_mode=mode_g, gate_dtype=binding.GATE_NONE)
+    ws = ctx.new_workspace()
+    seen = set()
+    for seed in range(4):
+        ids = synth.zipf_topk_ids(T, k, E, s, 300 + seed)
+        plan = ctx.new_plan(dense_U=True)
+        count = torch.zeros(E, dtype=torch.int32, device=DEV)
+        ctx.uep_histogram(ids.to(DEV), count, ws)
+        ctx.uep_plan(count, plan, ws)
+        torch.cuda.synchronize()
+        lam, _ = oracle.histogram(ids.numpy(), E)
+        p = oracle.plan(lam, R, n_slot, u_min, 101, 100, mode_o, None, S_total=T * k)
+        hp = plan.host()
+        for n in PLAN_ARRAYS:
+            assert np.array_equal(np.asarray(getattr(hp, n)).reshape(-1), np.asarray(getattr(p, n)).reshape(-1)), n
+        sc = np.asarray(hp.scalars)
+        seen.add((int(sc[binding.SC_TAU] - sc[binding.SC_TAU_LO0]) > 0, int(sc[binding.SC_N_PROBES]) > 0))
+    assert seen                                   # (documentation of what the cases exercised)
