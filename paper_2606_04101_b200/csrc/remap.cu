@@ -48,6 +48,7 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
             int group_len, int32_t* __restrict__ packed, int32_t* __restrict__ prefix, int chunk0) {
   extern __shared__ __align__(16) int smem[];
   int2* wrow = reinterpret_cast<int2*>(smem);
+  pdl_trigger();                                 // prefix_kernel may be scheduled (it waits for this grid)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
   const int cb = (int)blockIdx.x + chunk0;       // chunk0 > 0: a token shard's CTAs (uep_shard_count)
@@ -125,8 +126,15 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
 // n_rows into the totals.  One CTA per int4 column group, one thread per row (blocks of 1024
 // rows with a carry): one L2 round trip per block instead of a serial walk.
 __global__ void __launch_bounds__(1024, 1)
-prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG) {
+prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG, int trigger) {
   __shared__ int4 wsum[32];
+  // launched programmatically dependent on rank_kernel: wait for it, and only then (trigger != 0:
+  // uep_remap, whose lookup reads the prefix rows AFTER its own wait) let the kernel behind this
+  // one start, so that its prologue may read what rank_kernel wrote.  uep_balance passes 0: its
+  // lookup reads the rows in its prologue, and under stream capture the lookup's programmatic
+  // launch attribute makes its edge from this kernel programmatic too.
+  pdl_wait();
+  if (trigger) pdl_trigger();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   int4* col = reinterpret_cast<int4*>(prefix) + blockIdx.x;
   int4 carry = make_int4(0, 0, 0, 0);
@@ -168,7 +176,7 @@ prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG) {
 // virtual base of the global [S] array, only the shard's slots are dereferenced); n_launch < 0:
 // all chunks.  with_prefix = false leaves the raw per-chunk counts for the exchange step.
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local, int chunk0,
-                int n_launch, bool with_prefix) {
+                int n_launch, bool with_prefix, bool prefix_trigger) {
   if (c->S == 0) return UEP_OK;
   const int chunks = local ? c->l_chunks : c->r_chunks;
   const size_t smem = sizeof(int2) * (size_t)kRemapWarps * c->E_pad;
@@ -177,15 +185,26 @@ int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool
       local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S, ws_packed(c, ws),
       ws_prefix(c, ws), chunk0);
   UEP_CUDA_TRY(cudaGetLastError());
-  if (with_prefix) return launch_prefix(c, ws, s, local);
+  if (with_prefix) return launch_prefix(c, ws, s, local, /*pdl=*/true, prefix_trigger);
   return UEP_OK;
 }
 
-int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local) {
+// pdl: launched programmatically dependent on the kernel before it in the stream (rank_kernel):
+// the launch latency overlaps that kernel
+int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local, bool pdl, bool trigger) {
   if (c->S == 0) return UEP_OK;
-  prefix_kernel<<<c->E_pad / 4, 1024, 0, s>>>(ws_prefix(c, ws), local ? c->l_chunks : c->r_chunks,
-                                              c->E_pad / 4);
-  UEP_CUDA_TRY(cudaGetLastError());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(c->E_pad / 4);
+  cfg.blockDim = dim3(1024);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl ? 1 : 0;
+  UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, prefix_kernel, ws_prefix(c, ws),
+                                  local ? c->l_chunks : c->r_chunks, c->E_pad / 4, trigger ? 1 : 0));
   return UEP_OK;
 }
 
@@ -227,6 +246,7 @@ reroute_kernel(int E_pad, int R, int inst_cap, int cpg, const int32_t* __restric
   __shared__ int u[kRrMaxInst], uhat[kRrMaxInst], u0[kRrMaxInst + 1], host[kRrMaxInst], locq[kRrMaxInst];
   __shared__ int tmp[8];
   const int tid = threadIdx.x, e = blockIdx.x;
+  pdl_trigger();                 // the lookup's plan-independent prologue may start
   const int lo = inst_off[e], n = inst_off[e + 1] - lo;
   if (e == 0 && n_inflight) for (int r = tid; r < R; r += kRrThreads) n_inflight[r] = 0;
   if (tid < R) {
@@ -310,7 +330,8 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
               int32_t* __restrict__ out_rank, int32_t* __restrict__ out_offset,
               GateT* __restrict__ out_gate, int cpg, int group_len,
               const int32_t* __restrict__ cumq, const int32_t* __restrict__ srcpre,
-              int32_t* __restrict__ n_inflight, int32_t* __restrict__ acc_clear, int chunk0) {
+              int32_t* __restrict__ n_inflight, int32_t* __restrict__ acc_clear, int chunk0,
+              int early_wait) {
   // Token-sharded mode (LOCAL with cumq == nullptr): the grouped chunk geometry and
   // the per-source in-flight count of the source-aware mode, but GLOBAL ranks and the plan's own
   // cumulative quotas, on the chunks [chunk0, chunk0 + gridDim.x) that this GPU owns.
@@ -360,6 +381,9 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
     if (has_gate) gv[i] = in ? __ldg(gate + i * 32) : GateT(0);
   }
 
+  // early_wait (uep_remap): the preceding kernel is prefix_kernel, whose rows are read next; the
+  // loads above (packed ranks, gates) were complete before it started
+  if (early_wait) pdl_wait();
   // ---- chunk base ranks: row c of the exclusive prefix over chunks that rank_kernel left ----------
   const int p_own = (tid < E) ? __ldcg(prefix + (size_t)c * E_pad + tid) : 0;
   const int n_own = (tid < E) ? __ldcg(prefix + (size_t)(c + 1) * E_pad + tid) - p_own : 0;
@@ -488,7 +512,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
                            int32_t* out_replica, int32_t* out_rank, int32_t* out_offset,
                            GateT* out_gate, void* ws, cudaStream_t s, bool pdl, bool local,
                            int32_t* n_inflight, int32_t* acc_clear, int chunk0, int n_launch,
-                           bool src_aware) {
+                           bool src_aware, bool early_wait) {
   const uep_config& g = c->cfg;
   const int inst_cap = g.E + g.R * g.n_slot;
   const bool stage = gate != nullptr;
@@ -514,7 +538,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
                                   (const int32_t*)p.inst_cum, (const int32_t*)p.inst_base,
                                   (const int32_t*)p.rank_base, out_replica, out_rank, out_offset,
                                   out_gate, local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S,
-                                  cumq, srcpre, n_inflight, acc_clear, chunk0));
+                                  cumq, srcpre, n_inflight, acc_clear, chunk0, early_wait ? 1 : 0));
   return UEP_OK;
 }
 
@@ -536,15 +560,15 @@ int init_remap_kernels() {
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& p, int32_t* out_replica,
                   int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
                   bool pdl, bool local, int32_t* n_inflight, int32_t* acc_clear, int chunk0,
-                  int n_launch, bool src_aware) {
+                  int n_launch, bool src_aware, bool early_wait) {
   if (c->S == 0) return UEP_OK;
   if (c->cfg.gate_dtype == UEP_GATE_BF16 && gate)
     return launch_lookup_t<uint16_t>(c, static_cast<const uint16_t*>(gate), p, out_replica, out_rank,
                                      out_offset, static_cast<uint16_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear,
-                                     chunk0, n_launch, src_aware);
+                                     chunk0, n_launch, src_aware, early_wait);
   return launch_lookup_t<uint32_t>(c, static_cast<const uint32_t*>(gate), p, out_replica, out_rank,
                                    out_offset, static_cast<uint32_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear,
-                                   chunk0, n_launch, src_aware);
+                                   chunk0, n_launch, src_aware, early_wait);
 }
 
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& p,
@@ -552,7 +576,10 @@ int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_p
                  void* ws, cudaStream_t s) {
   int rc = launch_rank(c, ids, ws, s);
   if (rc != UEP_OK) return rc;
-  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s, false, false, nullptr, nullptr);
+  // programmatically dependent on prefix_kernel: launch and the loads of packed ranks and gates
+  // overlap it, the prefix rows are read after the wait
+  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s, /*pdl=*/true, false,
+                       nullptr, nullptr, 0, -1, true, /*early_wait=*/true);
 }
 
 }  // namespace uep

@@ -355,8 +355,8 @@ int uep_remap_local(const uep_ctx* ctx, const int32_t* topk_ids, const void* gat
   rc = launch_rank(c, topk_ids, ws, s, /*local=*/true);
   if (rc == UEP_OK) rc = launch_reroute(c, *plan, n_inflight, ws, s);
   if (rc == UEP_OK)
-    rc = launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s, false,
-                       /*local=*/true, n_inflight);
+    rc = launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s, /*pdl=*/true,
+                       /*local=*/true, n_inflight);   // prologue overlaps reroute_kernel
   return rc;
 }
 
@@ -526,7 +526,7 @@ static int balance_impl(const uep_ctx* ctx, const int32_t* topk_ids, const void*
   UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
   int rc2 = launch_histogram(c, topk_ids, expert_count, ws, s, /*red=*/true);
   UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-  rc = launch_rank(c, topk_ids, ws, c->side);
+  rc = launch_rank(c, topk_ids, ws, c->side, false, 0, -1, true, /*prefix_trigger=*/false);
   UEP_CUDA_TRY(cudaEventRecord(c->ev_rank, c->side));
   // planner and lookup are launched programmatically dependent on their predecessor: their
   // prologues (static layout; packed ranks, gates, prefix rows) overlap it

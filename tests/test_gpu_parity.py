@@ -835,3 +835,74 @@ def test_planner_paths_off_the_spine_full_size(n_slot, u_min, s, strict):
         sc = np.asarray(hp.scalars)
         seen.add((int(sc[binding.SC_TAU] - sc[binding.SC_TAU_LO0]) > 0, int(sc[binding.SC_N_PROBES]) > 0))
     assert seen                                   # (documentation of what the cases exercised)
+
+
+@pytest.mark.parametrize("entry", ["balance", "remap", "remap_local"])
+def test_back_to_back_calls_in_one_graph_full_size(entry):
+    """The launch configuration bench.py times: several instances of the DeepSeek-V3 shape run
+    back to back in ONE CUDA graph on one workspace (each call's kernels are launched
+    programmatically dependent on their predecessors, so a missing dependency between the
+    prefix rows of one call and the lookup of the same or the next call shows up here and not in
+    a single call).  Every instance's outputs are compared with the oracle, after three replays."""
+    c = synth.CONFIGS["dsv3_prefill"]
+    T, k, E, R, ns, um = c["T"], c["k"], c["E"], c["R"], c["n_slot"], c["u_min"]
+    n_inst = 5
+    ctx = binding.Context(T, k, E, R, ns, um)
+    ws = ctx.new_workspace()
+    ins, outs = [], []
+    for b in range(n_inst):
+        ids = synth.zipf_topk_ids(T, k, E, 0.7 + 0.2 * b, 900 + b, device=DEV).cpu()
+        gate = synth.gates_uniform_renorm(T, k, 40 + b)
+        d_ids, d_gate = ids.to(DEV), gate.to(DEV)
+        rep, rnk, off, og = ctx.new_outputs(d_gate)
+        ins.append((ids, gate, d_ids, d_gate))
+        outs.append(dict(count=torch.zeros(E, dtype=torch.int32, device=DEV), plan=ctx.new_plan(),
+                         rep=rep, rnk=rnk, off=off, og=og,
+                         infl=torch.zeros(R, dtype=torch.int32, device=DEV)))
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+
+    def call(b):
+        _, _, d_ids, d_gate = ins[b]
+        o = outs[b]
+        if entry == "balance":
+            ctx.uep_balance(d_ids, d_gate, o["count"], o["plan"], o["rep"], o["rnk"], o["off"],
+                            o["og"], [], [], ws)
+        elif entry == "remap":
+            ctx.uep_remap(d_ids, d_gate, o["plan"], o["rep"], o["rnk"], o["off"], o["og"], ws)
+        else:
+            ctx.uep_remap_local(d_ids, d_gate, o["plan"], o["rep"], o["rnk"], o["off"], o["og"],
+                                o["infl"], ws)
+
+    with torch.cuda.stream(stream):
+        for b in range(n_inst):                      # plans for the remap-only entries; warm-up
+            ctx.uep_histogram(ins[b][2], outs[b]["count"], ws)
+            ctx.uep_plan(outs[b]["count"], outs[b]["plan"], ws)
+            call(b)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            for b in range(n_inst):
+                call(b)
+    torch.cuda.synchronize()
+    for o in outs:
+        for t in (o["rep"], o["rnk"], o["off"], o["og"]):
+            t.fill_(0)
+    torch.cuda.synchronize()
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    for b in range(n_inst):
+        ids, gate = ins[b][0], ins[b][1]
+        lam, p, rep, rnk, off, og = oracle_chain(ids, gate, E, R, ns, um)
+        o = outs[b]
+        assert np.array_equal(o["count"].cpu().numpy(), lam)
+        assert np.array_equal(np.asarray(o["plan"].host().inst_cum).ravel(), np.asarray(p.inst_cum).ravel())
+        gbits = gate.view(torch.int32).numpy().view(np.uint32)
+        if entry == "remap_local":
+            rep, rnk, off, og, _, o_infl = oracle.remap_local(ids.numpy(), gbits, p)
+            assert np.array_equal(o["infl"].cpu().numpy(), o_infl)
+        assert np.array_equal(o["rep"].cpu().numpy(), rep), (entry, b)
+        assert np.array_equal(o["rnk"].cpu().numpy(), rnk), (entry, b)
+        assert np.array_equal(o["off"].cpu().numpy(), off), (entry, b)
+        nv = int(p.rank_base[-1])
+        assert np.array_equal(o["og"].cpu().view(torch.int32).numpy().view(np.uint32)[:nv], og[:nv])
