@@ -4,10 +4,14 @@
 // all of its int4 loads of a round before it touches shared memory (kHistVecs x 16 B in flight
 // per thread, 64 KB per SM), then counts into a WARP-PRIVATE shared-memory row (pitch E_pad+1
 // so the same expert in different rows falls into different banks): no contention between
-// warps on a hot expert, only the intra-warp multiplicity.  The CTA's row of the chunk table
-// (raw counts, used only by this kernel's own reduction) is written once.  The last
-// CTA to finish (ticket) sums the table's columns with one round of independent int4 L2 loads
-// and emits expert_count.  Integer adds only: bit-identical run to run.
+// warps on a hot expert, only the intra-warp multiplicity.  Every CTA adds its column sums to an
+// accumulator in the workspace (zero between calls) with fire-and-forget reductions — integer
+// adds, order-free, bit-identical run to run — and exits.  The accumulator is consumed by the
+// kernel behind it in the stream, launched programmatically dependent: the planner inside
+// uep_balance (it publishes expert_count), publish_kernel in the standalone uep_histogram (one
+// CTA: accumulator -> expert_count, accumulator cleared).  An earlier design elected the last CTA
+// by a ticket and summed a table of per-CTA rows there: fence + ticket + that CTA's serial pass
+// cost 4.8 of the kernel's 9.4 us at the DeepSeek-V3 shape.
 #include "uep_internal.cuh"
 
 namespace uep {
@@ -26,30 +30,23 @@ __device__ __forceinline__ void count_one(int* row, int e, int E) {
   if ((unsigned)e < (unsigned)E) atomicAdd(&row[e], 1);
 }
 
-// dynamic shared memory (ints): priv[kHistWarps][E_pad+1] | part[kColPartInts] | tot[E_pad]
+// dynamic shared memory (ints): priv[kHistWarps][E_pad+1]
 __host__ __device__ inline size_t hist_smem_ints(int E_pad) {
-  return (size_t)kHistWarps * (E_pad + 1) + kColPartInts + E_pad;
+  return (size_t)kHistWarps * (E_pad + 1);
 }
 
-// RED = false: the CTA's row goes to the chunk table, the last CTA (ticket) sums the columns into
-// expert_count.  RED = true (uep_balance): the ticket, the fence and the last CTA's serial pass cost
-// 4.8 of the kernel's 9.4 us at the DeepSeek-V3 shape, so every CTA instead adds its counts to an
-// accumulator in the workspace with fire-and-forget reductions (integer adds: order-free) and
-// exits; the planner reads the accumulator, publishes expert_count and clears it.
-template <bool RED>
+// TABLE: also leave the CTA's raw counts in row c of the chunk table (uep_histogram's by-product,
+// SURVEY 8(a1); uep_balance does not need it)
+template <bool TABLE>
 __global__ void __launch_bounds__(kHistThreads, 1)
 hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len,
-            int n_chunks, int32_t* __restrict__ table, unsigned* __restrict__ ticket,
-            int32_t* __restrict__ expert_count) {
+            int32_t* __restrict__ table, int32_t* __restrict__ acc) {
   extern __shared__ __align__(16) int hsm[];
   const int pitch = E_pad + 1;
   int* priv = hsm;
-  int* part = hsm + ((kHistWarps * pitch + 3) & ~3);
-  int* tot = part + kColPartInts;
-  __shared__ unsigned s_last;
   const int tid = threadIdx.x, warp = tid >> 5;
   const int c = blockIdx.x;
-  pdl_trigger();     // uep_balance launches the planner behind this kernel with its prologue overlapped
+  pdl_trigger();     // the kernel behind this one (planner / publish_kernel) may start its prologue
 
   const long long begin = (long long)c * chunk_len;
   const int len = (int)min((long long)chunk_len, (long long)S - begin);   // > 0 by construction
@@ -85,28 +82,24 @@ hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
   if (tid < (len & 3)) count_one(row, ids[begin + (n_vec << 2) + tid], E);   // ragged tail
   __syncthreads();
 
-  int32_t* grow = table + (size_t)c * E_pad;
   for (int e = tid; e < E_pad; e += kHistThreads) {
     int s = 0;
 #pragma unroll 8
     for (int w = 0; w < kHistWarps; ++w) s += priv[w * pitch + e];
-    if (RED) { if (s != 0 && e < E) atomicAdd(expert_count + e, s); }   // expert_count = the accumulator
-    else grow[e] = s;
+    if (s != 0 && e < E) atomicAdd(acc + e, s);          // result unused: a fire-and-forget RED
+    if (TABLE) table[(size_t)c * E_pad + e] = s;
   }
-  if (RED) return;
-  __syncthreads();                   // the CTA's row is written (barrier orders it before thread 0's fence)
-  if (tid == 0) {
-    __threadfence();                 // cumulative: makes the whole row visible before the ticket
-    s_last = (atomicAdd(ticket, 1u) == (unsigned)(n_chunks - 1));
-  }
-  __syncthreads();
-  if (!s_last) return;
-  __threadfence();
+}
 
-  // Last CTA: column totals -> expert_count.
-  column_sums(table, n_chunks, E_pad, part, tot);
-  for (int e = tid; e < E; e += kHistThreads) expert_count[e] = tot[e];
-  if (tid == 0) *ticket = 0u;        // self-reset: the next launch (graph replay) starts clean
+// uep_histogram's second kernel, one CTA, launched programmatically dependent on hist_kernel (its
+// launch overlaps it): accumulator -> expert_count, accumulator cleared for the next call.
+__global__ void __launch_bounds__(UEP_MAX_E)
+publish_kernel(int E, int32_t* __restrict__ acc, int32_t* __restrict__ expert_count) {
+  pdl_wait();                        // hist_kernel complete, its reductions performed
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    expert_count[e] = __ldcg(acc + e);
+    acc[e] = 0;
+  }
 }
 
 // S == 0: nothing to read; zero the counts and the single table row.
@@ -125,22 +118,34 @@ int init_hist_kernels() {
   return UEP_OK;
 }
 
+// red = true (uep_balance): only the accumulator is left, for the planner.
 int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s,
                      bool red) {
   if (c->S == 0) {
     if (!red) hist_empty_kernel<<<1, 256, 0, s>>>(c->cfg.E, c->E_pad, ws_table(ws), count);
-  } else {
-    const size_t smem = sizeof(int) * (hist_smem_ints(c->E_pad) + 4);
-    if (red)
-      hist_kernel<true><<<c->n_chunks, kHistThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
-                                                                c->chunk_len, c->n_chunks, ws_table(ws),
-                                                                ws_ticket(ws), ws_acc(ws));
-    else
-      hist_kernel<false><<<c->n_chunks, kHistThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
-                                                                 c->chunk_len, c->n_chunks, ws_table(ws),
-                                                                 ws_ticket(ws), count);
+    UEP_CUDA_TRY(cudaGetLastError());
+    return UEP_OK;
   }
+  const size_t smem = sizeof(int) * (hist_smem_ints(c->E_pad) + 4);
+  if (red) {
+    hist_kernel<false><<<c->n_chunks, kHistThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
+                                                               c->chunk_len, ws_table(ws), ws_acc(ws));
+    UEP_CUDA_TRY(cudaGetLastError());
+    return UEP_OK;
+  }
+  hist_kernel<true><<<c->n_chunks, kHistThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
+                                                            c->chunk_len, ws_table(ws), ws_acc(ws));
   UEP_CUDA_TRY(cudaGetLastError());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(1);
+  cfg.blockDim = dim3(c->E_pad < 32 ? 32 : c->E_pad);
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, publish_kernel, c->cfg.E, ws_acc(ws), count));
   return UEP_OK;
 }
 

@@ -308,16 +308,16 @@ int launch_reroute(const Ctx* c, const uep_plan_out& plan, int32_t* n_inflight, 
 
 // ------------------------------------------------------------------------------------------------
 // lookup_kernel.  dynamic shared memory layout (ints):
-//   rec[E_pad] (int4) | base0[E_pad] | elb[E_pad] | s_off[E_pad+4] | rbase[(R+7)&~3]
-//   | i_cum | i_dbase | i_gbase | i_rank (icap each) | wtot[36]
-//   | (STAGE) sg[kMaxChunk] gates + sd[kMaxChunk] ints
+//   rec[E_pad] (int4) | base0[E_pad] | s_off[E_pad+4] | rbase[(R+7)&~3]
+//   | i_cum | i_base | i_rank (icap each) | wtot[36]
+//   | (STAGE) stg[kMaxChunk] (int2 {gate bits, out_gate index})
 // ------------------------------------------------------------------------------------------------
-__host__ __device__ inline size_t lookup_smem_bytes(int E_pad, int R, int inst_cap, bool stage,
-                                                    int gate_bytes) {
-  const size_t fixed = 4 * (size_t)E_pad + 2 * (size_t)E_pad + (E_pad + 4) + ((R + 7) & ~3) +
-                       4 * (size_t)((inst_cap + 3) & ~3) + 36;
-  const size_t scratch = stage ? (size_t)kMaxChunk * (gate_bytes + sizeof(int)) : 0;
-  return sizeof(int) * fixed + scratch;
+__host__ __device__ inline size_t lookup_smem_ints(int E_pad, int R, int inst_cap) {
+  return 4 * (size_t)E_pad + (size_t)E_pad + (E_pad + 4) + ((R + 7) & ~3) +
+         3 * (size_t)((inst_cap + 3) & ~3) + 36;           // a multiple of 4: stg is 16-B aligned
+}
+__host__ __device__ inline size_t lookup_smem_bytes(int E_pad, int R, int inst_cap, bool stage) {
+  return sizeof(int) * lookup_smem_ints(E_pad, R, inst_cap) + (stage ? sizeof(int2) * (size_t)kMaxChunk : 0);
 }
 
 template <typename GateT, bool STAGE, bool LOCAL>
@@ -343,17 +343,14 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   extern __shared__ __align__(16) int smem[];
   int4* rec = reinterpret_cast<int4*>(smem);     // [E_pad] fast-path record per expert
   int* base0 = reinterpret_cast<int*>(rec + E_pad);   // [E_pad] global rank of the chunk's first slot of e
-  int* elb = base0 + E_pad;                      // [E_pad] staging position of chunk rank jl is elb[e] + jl
-  int* s_off = elb + E_pad;                      // [E+1]
-  int* rbase = s_off + (E_pad + 4);              // [R+1]
+  int* s_off = base0 + E_pad;                    // [E_pad+4] CSR of instances
+  int* rbase = s_off + E_pad + 4;                // [(R+7)&~3] rank_base
   const int icap = (inst_cap + 3) & ~3;
-  int* i_cum = rbase + ((R + 7) & ~3);           // inclusive cumulative quota
-  int* i_dbase = i_cum + icap;                   // inst_base - cum_prev
-  int* i_gbase = i_dbase + icap;                 // rank_base[rank] + i_dbase
-  int* i_rank = i_gbase + icap;
+  int* i_cum = rbase + ((R + 7) & ~3);           // cumulative quotas (row of the source rank when local)
+  int* i_base = i_cum + icap;                    // inst_base (+ srcpre when local)
+  int* i_rank = i_base + icap;
   int* wtot = i_rank + icap;                     // [32] warp totals, [32] = chunk total
-  GateT* sg = reinterpret_cast<GateT*>(wtot + 36);    // staged gates, (expert, rank) order
-  int* sd = reinterpret_cast<int*>(sg + kMaxChunk);   // their out_gate index
+  int2* stg = reinterpret_cast<int2*>(wtot + 36);     // staged {gate bits, out_gate index}, (expert, rank) order
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int c = LOCAL ? (int)blockIdx.x + chunk0 : (int)blockIdx.x;
@@ -404,40 +401,29 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   for (int e = tid; e <= E; e += kRemapThreads) s_off[e] = g_inst_off[e];
   for (int r = tid; r <= R; r += kRemapThreads) rbase[r] = g_rank_base[r];
   for (int p = tid; p < inst_cap; p += kRemapThreads) {
-    const int cum = local ? __ldcg(cumq + (size_t)grp * inst_cap + p) : g_inst_cum[p];
-    i_cum[p] = cum;
+    i_cum[p] = local ? __ldcg(cumq + (size_t)grp * inst_cap + p) : g_inst_cum[p];
     i_rank[p] = g_inst_rank[p];
-    i_gbase[p] = g_inst_base[p] + (local ? __ldcg(srcpre + (size_t)grp * inst_cap + p) : 0);   // raw base for now
-    if (p + 1 < inst_cap) i_dbase[p + 1] = cum;  // cum_prev of the next entry
-    if (p == 0) i_dbase[0] = 0;
+    i_base[p] = g_inst_base[p] + (local ? __ldcg(srcpre + (size_t)grp * inst_cap + p) : 0);
   }
   __syncthreads();
-  if (tid < E) {
-    base0[tid] = b0_own;
-    i_dbase[s_off[tid]] = 0;                     // first instance of an expert: cum_prev = 0
-  }
+  // rec[e] (E <= kRemapThreads: one thread per expert), in chunk-rank space: {cum - base0,
+  // dbase + base0, gbase + base0, staging base << 19 | replica << 8 | rank} of the instance
+  // holding the chunk's first slot of e, where dbase = inst_base - cum_prev (offset = dbase + j)
+  // and gbase = rank_base[rank] + dbase (out_gate index = gbase + j)
   {
     int pre = 0;
     for (int w = 0; w < warp; ++w) pre += wtot[w];
-    if (tid < E) elb[tid] = pre + el_inc - n_own;
+    if (tid < E) {
+      const int lo = s_off[tid], last = s_off[tid + 1] - 1, b0 = b0_own;
+      int p = lo;
+      while (p < last && i_cum[p] <= b0) ++p;
+      const int rk = i_rank[p];
+      const int d = i_base[p] - (p > lo ? i_cum[p - 1] : 0) + b0;
+      base0[tid] = b0;
+      rec[tid] = make_int4(i_cum[p] - b0, d, rbase[rk] + d,
+                           (int)(((unsigned)(pre + el_inc - n_own) << 19) | (unsigned)((p - lo) << 8) | (unsigned)rk));
+    }
     if (tid == kRemapThreads - 1) wtot[32] = pre + el_inc;          // valid slots in this chunk
-  }
-  __syncthreads();
-  const int n_inst = s_off[E];
-  for (int p = tid; p < n_inst; p += kRemapThreads) {
-    const int d = i_gbase[p] - i_dbase[p];
-    i_dbase[p] = d;
-    i_gbase[p] = rbase[i_rank[p]] + d;
-  }
-  __syncthreads();
-  // rec[e], in chunk-rank space: {cum - base0, dbase + base0, gbase + base0,
-  // staging base << 19 | replica << 8 | rank} of the instance holding the chunk's first slot of e
-  for (int e = tid; e < E; e += kRemapThreads) {
-    const int lo = s_off[e], last = s_off[e + 1] - 1, b0 = base0[e];
-    int p = lo;
-    while (p < last && i_cum[p] <= b0) ++p;
-    rec[e] = make_int4(i_cum[p] - b0, i_dbase[p] + b0, i_gbase[p] + b0,
-                       (int)(((unsigned)elb[e] << 19) | (unsigned)((p - lo) << 8) | (unsigned)i_rank[p]));
   }
   __syncthreads();
 
@@ -470,14 +456,14 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
               int p = s_off[e] + rep + 1;
               const int last = s_off[e + 1] - 1;         // cum[last] = lambda_e > j when ws matches plan
               while (p < last && i_cum[p] <= j) ++p;
-              db = i_dbase[p] + b0; gb = i_gbase[p] + b0; rep = p - s_off[e]; rk = i_rank[p];
+              rk = i_rank[p];
+              db = i_base[p] - i_cum[p - 1] + b0;          // p > s_off[e]: cum_prev is the entry before
+              gb = rbase[rk] + db; rep = p - s_off[e];
             }
             of = db + jl;
             if (has_gate) {
               if (STAGE) {
-                const int lp = (int)(rw >> 19) + jl;
-                sg[lp] = gv[i];
-                sd[lp] = gb + jl;
+                stg[(int)(rw >> 19) + jl] = make_int2((int)gv[i], gb + jl);
               } else {
                 out_gate[gb + jl] = gv[i];
               }
@@ -502,7 +488,10 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
 #pragma unroll
     for (int i = 0; i < kRemapItems; ++i) {
       const int lp = i * kRemapThreads + tid;
-      if (lp < n_valid) out_gate[sd[lp]] = sg[lp];
+      if (lp < n_valid) {
+        const int2 v = stg[lp];
+        out_gate[v.y] = (GateT)v.x;
+      }
     }
   }
 }
@@ -516,7 +505,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
   const uep_config& g = c->cfg;
   const int inst_cap = g.E + g.R * g.n_slot;
   const bool stage = gate != nullptr;
-  const size_t smem = lookup_smem_bytes(c->E_pad, g.R, inst_cap, stage, sizeof(GateT));
+  const size_t smem = lookup_smem_bytes(c->E_pad, g.R, inst_cap, stage);
   auto k = local ? (stage ? lookup_kernel<GateT, true, true> : lookup_kernel<GateT, false, true>)
                  : (stage ? lookup_kernel<GateT, true, false> : lookup_kernel<GateT, false, false>);
   cudaLaunchConfig_t cfg = {};
@@ -544,7 +533,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
 
 int init_remap_kernels() {
   const int rank_bytes = (int)(sizeof(int2) * (size_t)kRemapWarps * UEP_MAX_E);
-  const int bytes = (int)lookup_smem_bytes(UEP_MAX_E, UEP_MAX_R, UEP_MAX_E + UEP_MAX_R * UEP_MAX_NSLOT, true, 4);
+  const int bytes = (int)lookup_smem_bytes(UEP_MAX_E, UEP_MAX_R, UEP_MAX_E + UEP_MAX_R * UEP_MAX_NSLOT, true);
   UEP_CUDA_TRY(cudaFuncSetAttribute(rank_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rank_bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));

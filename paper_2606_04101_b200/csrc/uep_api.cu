@@ -202,7 +202,7 @@ size_t uep_workspace_bytes(const uep_ctx* ctx) {
 int uep_workspace_init(const uep_ctx* ctx, void* ws, void* stream) {
   const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
   if (!c || !ws || !aligned16(ws)) return UEP_ERR_INVALID_ARG;
-  // tickets, and row 0 of the remap prefix table (it stays zero: the scan starts at row 1)
+  // the accumulator, and row 0 of the remap prefix table (it stays zero: the scan starts at row 1)
   UEP_CUDA_TRY(cudaMemsetAsync(ws, 0, kWsHeaderBytes, static_cast<cudaStream_t>(stream)));
   UEP_CUDA_TRY(cudaMemsetAsync(ws_prefix(c, ws), 0, ws_prefix_bytes(c), static_cast<cudaStream_t>(stream)));
   return UEP_OK;

@@ -12,8 +12,7 @@
 
 namespace uep {
 
-constexpr int kWsHeaderBytes = 256 + 4 * UEP_MAX_E;   // [0] ticket of the histogram's last-CTA reduction;
-                                                     // from byte 256: acc[E] of uep_balance's histogram (zero between calls)
+constexpr int kWsHeaderBytes = 256 + 4 * UEP_MAX_E;   // from byte 256: acc[E], the histogram's accumulator (zero between calls)
 constexpr int kHistThreads = 1024;
 constexpr int kRemapThreads = 512;
 constexpr int kRemapWarps = kRemapThreads / 32;
@@ -68,9 +67,9 @@ struct PackArgs {
 
 int set_cuda_error(cudaError_t e);
 
-// red = true (uep_balance): no ticket, no last-CTA pass; every CTA adds its counts to ws_acc(ws)
-// with fire-and-forget reductions and the planner (launch_plan with from_acc) reads them there,
-// publishes expert_count and zeroes the accumulator again.
+// every CTA adds its counts to ws_acc(ws) with fire-and-forget reductions.  red = true
+// (uep_balance): the planner (launch_plan with acc) reads them there and publishes expert_count,
+// the lookup zeroes the accumulator again.  red = false: publish_kernel does both.
 int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s,
                      bool red = false);
 int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
@@ -104,11 +103,6 @@ int init_reduce_kernels();
 
 int init_hist_kernels();
 
-// ---- column sums of the chunk table (device) ---------------------------------------------------
-// out[e] = sum_{r < n_rows} table[r][e] for e < E_pad.  Whole CTA (1024 threads) must call it.
-// int4 loads, every thread's loads independent (one L2 round trip), partials in `part`
-// (kColPartInts ints of shared memory), result in `out` (shared).  Ends with a __syncthreads().
-constexpr int kColPartInts = 4096;
 #ifdef __CUDACC__
 // Programmatic dependent launch (sm_90+).  pdl_trigger: the next kernel in the stream, if it was
 // launched with programmatic stream serialization, may start now (its prologue overlaps this
@@ -116,37 +110,11 @@ constexpr int kColPartInts = 4096;
 // a no-op when the kernel was launched normally.
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-
-__device__ __forceinline__ void column_sums(const int32_t* __restrict__ table, int n_rows, int E_pad,
-                                            int* part, int* out) {
-  const int tid = threadIdx.x;
-  const int CG = E_pad >> 2;                                // int4 column groups per row
-  const int NRG = min(32, (int)blockDim.x / CG);            // row groups; NRG*E_pad <= kColPartInts
-  const int cg = tid % CG, rg = tid / CG;
-  if (rg < NRG) {
-    int4 acc = make_int4(0, 0, 0, 0);
-    const int4* col = reinterpret_cast<const int4*>(table) + cg;
-#pragma unroll 10
-    for (int r = rg; r < n_rows; r += NRG) {
-      const int4 v = __ldcg(col + (size_t)r * CG);
-      acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
-    }
-    reinterpret_cast<int4*>(part)[rg * CG + cg] = acc;
-  }
-  __syncthreads();
-  for (int e = tid; e < E_pad; e += blockDim.x) {
-    int s = 0;
-    for (int g = 0; g < NRG; ++g) s += part[g * E_pad + e];
-    out[e] = s;
-  }
-  __syncthreads();
-}
 #endif
 
 inline int32_t* ws_table(void* ws) {
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes);
 }
-inline unsigned* ws_ticket(void* ws) { return reinterpret_cast<unsigned*>(ws); }
 inline int32_t* ws_acc(void* ws) { return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + 256); }
 inline size_t ws_table_bytes(const Ctx* c) {
   return (sizeof(int32_t) * (size_t)c->n_chunks * c->E_pad + 255) & ~(size_t)255;
