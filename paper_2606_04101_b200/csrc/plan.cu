@@ -24,6 +24,7 @@
 //     probe at the final tau is run (deterministic, so it reproduces that probe).
 #include <algorithm>
 #include <cstdlib>
+#include <cstdio>
 #include <cooperative_groups.h>
 #include "uep_internal.cuh"
 
@@ -31,11 +32,18 @@ namespace uep {
 
 namespace cg = cooperative_groups;
 
+#ifdef UEP_PLAN_TIMING     // developer probe: cycle stamps at the barriers of setup and emit, printed by the emitting CTA
+#define UEP_STAMP(i) do { if (tid == 0) stamps[i] = clock64(); } while (0)
+#else
+#define UEP_STAMP(i)
+#endif
+
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kMaxLog = UEP_MAX_R * UEP_MAX_NSLOT;      // 1024 accepted transfers at most
 constexpr int kPlanWarps = kPlanThreads / 32;
 constexpr int kLogPer = kMaxLog / kPlanThreads;        // log entries handled per thread when emitting
 static_assert(kLogPer * kPlanThreads == kMaxLog && UEP_MAX_E <= kPlanThreads && UEP_MAX_R < kPlanThreads, "plan emit");
+static_assert(kPlanThreads == 512, "rank order: threads per rank derived from 2^9");
 // CTAs (SMs) sharing one solve, so that the 63 probes of a round spread over many schedulers:
 // 8 CTAs = two probes per scheduler.  Measured on B200 (DSV3 shape): 4 / 8 / 16 CTAs give
 // 22.9 / 20.6 / 20.4 us of bisection, i.e. from 8 up the probes are bound by the latency of their
@@ -67,6 +75,7 @@ struct PlanSmem {
   int node_feas[2][kPlanMaxNodes];   // probe verdict per tree node, written by its owner to every CTA
   int pc[kPcSmem];
   int warp_tmp[32];
+  unsigned long long scan_tmp[32];
   int feas[32];
   int lo, hi, n_probes, n_log, log_buf;
 #ifdef UEP_PLAN_TIMING
@@ -95,6 +104,32 @@ __device__ __forceinline__ int block_incl_scan(int v, int* tmp) {
   if (w == 0) {
     int t = tmp[lane];
     t = warp_incl_scan(t, lane);
+    tmp[lane] = t;
+  }
+  __syncthreads();
+  if (w > 0) s += tmp[w - 1];
+  return s;
+}
+
+// The same for a 64-bit value (two packed 32-bit sums).  tmp: 32 x 8 bytes of smem.
+__device__ __forceinline__ unsigned long long block_incl_scan64(unsigned long long v, unsigned long long* tmp) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  unsigned long long s = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned long long y = __shfl_up_sync(kFull, s, o);
+    if (lane >= o) s += y;
+  }
+  __syncthreads();
+  if (lane == 31) tmp[w] = s;
+  __syncthreads();
+  if (w == 0) {
+    unsigned long long t = (lane < kPlanWarps) ? tmp[lane] : 0ull;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned long long y = __shfl_up_sync(kFull, t, o);
+      if (lane >= o) t += y;
+    }
     tmp[lane] = t;
   }
   __syncthreads();
@@ -205,8 +240,12 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   const bool strict = strict_i != 0;
 #ifdef UEP_PLAN_TIMING
   long long t_start = clock64(), t_setup = 0, t_bisect = 0, t_final = 0;
+  long long stamps[24] = {};
 #endif
 
+  // touch both ends of the parameter block now: the emit phase reads the plan's pointers on the
+  // critical path, and a cold constant-cache line there costs several hundred cycles
+  if (out.slot_expert == nullptr || out.scalars == nullptr || count_out == reinterpret_cast<int32_t*>(1)) return;
   // ---- stage inputs ---------------------------------------------------------------------
   pdl_trigger();                   // the lookup kernel may start its plan-independent prologue
   if (tid < E) {                   // static layout first: it does not depend on the histogram
@@ -216,8 +255,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   }
   if (tid <= R) sm.roff[tid] = g_roff[tid];
   pdl_wait();                      // the histogram (preceding kernel) is complete
+  UEP_STAMP(0);
   if (tid < E) sm.lam[tid] = acc ? __ldcg(acc + tid) : expert_count[tid];
   __syncthreads();
+  UEP_STAMP(1);
   // line 2: l_r
   if (tid < R) {
     int s = 0;
@@ -225,6 +266,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     sm.ell[tid] = s;
   }
   __syncthreads();
+  UEP_STAMP(2);
   // sum and max of l_r (R <= 256 -> first 8 warps)
   {
     int v = (tid < R) ? sm.ell[tid] : 0;
@@ -233,34 +275,53 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (lane == 0) { sm.warp_tmp[warp] = sum; sm.feas[warp] = mx; }
   }
   __syncthreads();
-  if (tid == 0) {
-    long long sv = 0;
-    int mx = 0;
-    for (int w = 0; w < kPlanWarps; ++w) { sv += sm.warp_tmp[w]; mx = max(mx, sm.feas[w]); }
-    sm.s_valid = sv;
-    sm.max_ell = mx;
-    // line 3 (S3): tau_lo = floor(beta * ceil(mean)), tau_hi = max l_r
-    const long long mean_ceil = (sv + R - 1) / R;
-    const long long tl = mean_ceil * beta_num / beta_den;
-    sm.lo = (int)min(tl, (long long)0x7fffffff);
-    sm.hi = mx;
-    sm.n_probes = 0;
-    sm.n_log = 0;
+  UEP_STAMP(3);
+  if (warp == kPlanWarps - 1) {    // (the last warp has no expert to order below when E < kPlanThreads)
+    // per-warp partials -> totals with two warp reductions (S < 2^31: 32-bit sums are exact)
+    const int ps = (lane < kPlanWarps) ? sm.warp_tmp[lane] : 0;
+    const int pm = (lane < kPlanWarps) ? sm.feas[lane] : 0;
+    const unsigned sv = (unsigned)__reduce_add_sync(kFull, ps);
+    const int mx = __reduce_max_sync(kFull, pm);
+    if (lane == 0) {
+      sm.s_valid = (long long)sv;
+      sm.max_ell = mx;
+      // line 3 (S3): tau_lo = floor(beta * ceil(mean)), tau_hi = max l_r.  32-bit divisions where the
+      // operands fit (a 64-bit division is a ~300-cycle subroutine on this dependent path)
+      const unsigned mean_ceil = (sv + (unsigned)R - 1u) / (unsigned)R;
+      const unsigned long long prod = (unsigned long long)mean_ceil * (unsigned long long)beta_num;
+      const unsigned long long tl = (prod >> 32) == 0ull ? (unsigned long long)((unsigned)prod / (unsigned)beta_den)
+                                                         : prod / (unsigned long long)beta_den;
+      sm.lo = (int)min(tl, (unsigned long long)0x7fffffff);
+      sm.hi = mx;
+      sm.n_probes = 0;
+      sm.n_log = 0;
+    }
   }
 #ifdef UEP_PLAN_TIMING
   const long long t_s1 = clock64();
 #endif
-  // rank order: position = number of ranks that come before (l desc, id asc); a warp per rank
-  for (int r = warp; r < R; r += kPlanWarps) {
-    const int lr = sm.ell[r];
+  // rank order: position = number of ranks that come before (l desc, id asc).  gsz threads per
+  // rank (a power of two, all of the CTA's threads when R allows), each counting over a strided
+  // part of the ranks with independent loads, then a shuffle reduction inside the group.  (A warp
+  // per rank with a warp reduction each cost 500 cycles per rank, four ranks per warp in a row.)
+  {
+    const int gsh = min(5, 9 - (32 - __clz(R - 1)));           // kPlanThreads = 2^9 >= R << gsh
+    const int gsz = 1 << gsh, r = tid >> gsh, sub = tid & (gsz - 1);
     int cnt = 0;
-    for (int q = lane; q < R; q += 32) {
-      const int lq = sm.ell[q];
-      cnt += (lq > lr || (lq == lr && q < r)) ? 1 : 0;
+    UEP_STAMP(21);
+    if (r < R) {
+      const int lr = sm.ell[r];
+#pragma unroll 4
+      for (int q = sub; q < R; q += gsz) {
+        const int lq = sm.ell[q];
+        cnt += (lq > lr || (lq == lr && q < r)) ? 1 : 0;
+      }
     }
-    cnt = __reduce_add_sync(kFull, cnt);
-    if (lane == 0) sm.order[cnt] = r;
+    UEP_STAMP(22);
+    for (int o = gsz >> 1; o > 0; o >>= 1) cnt += __shfl_xor_sync(kFull, cnt, o);
+    if (r < R && sub == 0) sm.order[cnt] = r;
   }
+  UEP_STAMP(17);
   if (tid < E) {
     // per-rank expert order: lambda desc, id asc; a thread per expert counts the experts of its
     // home rank that come before it; positions into u_main (temp)
@@ -275,12 +336,15 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     }
     sm.u_main[e] = a + cnt;
   }
+  UEP_STAMP(18);
   __syncthreads();
+  UEP_STAMP(4);
 #ifdef UEP_PLAN_TIMING
   const long long t_s2 = clock64();
 #endif
   if (tid < E) sm.elist[sm.u_main[tid]] = tid;
   __syncthreads();
+  UEP_STAMP(5);
   // flat visit list: ranks in visit order, each with its experts in visit order (S5)
   {
     const int r = (tid < R) ? sm.order[tid] : 0;
@@ -304,6 +368,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   }
   __syncthreads();
   const int tau_lo0 = sm.lo, tau_hi0 = sm.hi;
+  UEP_STAMP(6);
 #ifdef UEP_PLAN_TIMING
   t_setup = clock64();
 #endif
@@ -440,6 +505,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     ++round;
   }
   const int tau = sm.hi;
+  UEP_STAMP(8);
 #ifdef UEP_PLAN_TIMING
   t_bisect = clock64();
 #endif
@@ -451,9 +517,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   const int log_node = sm.log_buf;
   const int owner = log_node < 0 ? 0 : log_node % csize;
   if (crank != owner) return;
+  UEP_STAMP(19);
   if (acc && tid < E) count_out[tid] = sm.lam[tid];
   uep_plan_out o = out;            // this instance's arrays (offset only here: the probes above
-  {                                // must not carry eleven pointers in registers)
+  if (batch_b != 0) {              // must not carry eleven pointers in registers)
     const size_t bb = (size_t)batch_b;
     const int n_inst_cap = E + R * n_slot;
     o.slot_expert += bb * max(1, R * n_slot);
@@ -476,6 +543,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (lane == 0) sm.n_log = nl;
   }
   const int4* lg = logs + (size_t)log_buf * log_cap;
+  UEP_STAMP(20);
   if (tid < E) { sm.u_main[tid] = sm.lam[tid]; sm.n_rep[tid] = 0; sm.first[tid] = 0x7fffffff; }
   const int RP = R * P;
   const bool pc_in_smem = RP <= kPcSmem;
@@ -484,6 +552,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   for (int i = tid; i < R * n_slot; i += kPlanThreads) o.slot_expert[i] = -1;
   if (o.U) for (int i = tid; i < E * R; i += kPlanThreads) o.U[i] = 0;
   __syncthreads();
+  UEP_STAMP(9);
   const int n_log = sm.n_log;
 #ifdef UEP_PLAN_TIMING
   t_final = clock64();
@@ -501,20 +570,24 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     }
   }
   __syncthreads();
+  UEP_STAMP(10);
   {
-    const int v = (tid < E) ? (1 + sm.n_rep[tid]) : 0;
-    const int inc = block_incl_scan(v, sm.warp_tmp);
-    if (tid < E) sm.inst_off[tid] = inc - v;
-    if (tid == E - 1) sm.inst_off[E] = inc;
-    __syncthreads();
-    int d[kLogPer], dsum = 0;                   // inclusive scan of delta over the log, kLogPer per thread
+    // one block scan for both prefix sums: instances per expert (high word; <= E + R * n_slot) and
+    // delta over the log, kLogPer entries per thread (low word; <= S < 2^24, so it never carries)
+    int d[kLogPer], dsum = 0;
 #pragma unroll
     for (int j = 0; j < kLogPer; ++j) {
       const int l = tid * kLogPer + j;
       d[j] = (l < n_log) ? lg[l].w : 0;
       dsum += d[j];
     }
-    int run = block_incl_scan(dsum, sm.warp_tmp) - dsum;
+    const int v = (tid < E) ? (1 + sm.n_rep[tid]) : 0;
+    const unsigned long long both =
+        block_incl_scan64(((unsigned long long)v << 32) | (unsigned long long)(unsigned)dsum, sm.scan_tmp);
+    const int inc = (int)(both >> 32);
+    if (tid < E) sm.inst_off[tid] = inc - v;
+    if (tid == E - 1) sm.inst_off[E] = inc;
+    int run = (int)(unsigned)both - dsum;
 #pragma unroll
     for (int j = 0; j < kLogPer; ++j) {
       const int l = tid * kLogPer + j;
@@ -523,6 +596,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     }
   }
   __syncthreads();
+  UEP_STAMP(11);
   for (int i = tid; i <= E; i += kPlanThreads) o.inst_off[i] = sm.inst_off[i];
   int fan = 0;
   if (tid < E) {
@@ -558,6 +632,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     int mf = __reduce_max_sync(kFull, fan);
     int ng = __reduce_add_sync(kFull, (fan > 1) ? 1 : 0);
     __syncthreads();                                                // pc complete
+  UEP_STAMP(12);
     if (lane == 0) { sm.feas[warp] = mf; sm.warp_tmp[warp] = ng; }
   }
   // receive layout (S13): per rank exclusive prefix over its P physical slots
@@ -572,6 +647,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     o.rank_load[tid] = load;
   }
   __syncthreads();
+  UEP_STAMP(13);
   // inst_base: offset of each instance's first token in its rank's receive buffer (S13)
   {
     const int* pb = pc_in_smem ? pc : o.phys_base;      // bases (global ones are CTA-visible now)
@@ -588,6 +664,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   int max_fan = 0, n_groups = 0;
   if (tid == 0) for (int w = 0; w < kPlanWarps; ++w) { max_fan = max(max_fan, sm.feas[w]); n_groups += sm.warp_tmp[w]; }
   __syncthreads();
+  UEP_STAMP(14);
   {
     const int inc = block_incl_scan(load, sm.warp_tmp);
     if (tid < R) o.rank_base[tid] = inc - load;
@@ -596,6 +673,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     __syncthreads();
     if (lane == 0) sm.feas[warp] = mx;
     __syncthreads();
+  UEP_STAMP(15);
   }
   if (tid == 0) {
     int max_load = 0;
@@ -618,6 +696,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     o.scalars[13] = (int)(t_bisect - t_setup);
     o.scalars[14] = (int)(t_final - t_bisect);
     o.scalars[15] = (int)(clock64() - t_final);
+    stamps[16] = clock64();
+    printf("plan stamps (cycles since start):");
+    for (int i = 0; i < 23; ++i) printf(" %d:%lld", i, stamps[i] ? stamps[i] - t_start : 0ll);
+    printf("\n");
 #endif
   }
 }
@@ -639,15 +721,26 @@ static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out&
   cfg.blockDim = dim3(kPlanThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = s;
-  cudaLaunchAttribute attr[2];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = cluster;
-  attr[0].val.clusterDim.y = 1;
-  attr[0].val.clusterDim.z = 1;
-  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[1].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchAttribute attr[3];
+  int na = 0;
+  attr[na].id = cudaLaunchAttributeClusterDimension;
+  attr[na].val.clusterDim.x = cluster;
+  attr[na].val.clusterDim.y = 1;
+  attr[na].val.clusterDim.z = 1;
+  ++na;
+  if (pdl) {
+    attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
+  }
+  // the planner is the critical path: when SMs free up its CTAs go before pending CTAs of the
+  // kernels running beside it (uep_balance: the second wave of rank_kernel)
+  // (measured, DeepSeek-V3 shape: chain 34.0 -> 32.2 us)
+  attr[na].id = cudaLaunchAttributePriority;
+  attr[na].val.priority = c->prio_high;
+  ++na;
   cfg.attrs = attr;
-  cfg.numAttrs = pdl ? 2 : 1;
+  cfg.numAttrs = na;
   UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, plan_kernel<RPL>, count, (const int32_t*)c->d_home,
                                   (const int32_t*)c->d_main_phys, (const int32_t*)c->d_roff,
                                   (const int32_t*)c->d_rexp, plan, g.E, g.R, g.n_slot, c->M, c->P,

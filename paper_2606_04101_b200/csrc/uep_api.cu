@@ -162,7 +162,13 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   UEP_TRY_OR_FAIL(cudaMemcpy(c->d_main_phys, main_phys.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
   UEP_TRY_OR_FAIL(cudaMemcpy(c->d_roff, roff.data(), sizeof(int32_t) * (R + 1), cudaMemcpyHostToDevice));
   UEP_TRY_OR_FAIL(cudaMemcpy(c->d_rexp, rexp.data(), sizeof(int32_t) * E, cudaMemcpyHostToDevice));
-  UEP_TRY_OR_FAIL(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+  {
+    int least = 0, greatest = 0;
+    UEP_TRY_OR_FAIL(cudaDeviceGetStreamPriorityRange(&least, &greatest));
+    c->prio_high = greatest;
+    // side stream (rank + prefix, pack) at the lowest priority: the critical path runs on the caller's stream
+    UEP_TRY_OR_FAIL(cudaStreamCreateWithPriority(&c->side, cudaStreamNonBlocking, least));
+  }
   UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
   UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
   UEP_TRY_OR_FAIL(cudaEventCreateWithFlags(&c->ev_rank, cudaEventDisableTiming));

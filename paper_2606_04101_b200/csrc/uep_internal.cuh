@@ -40,6 +40,7 @@ struct Ctx {
   int sm_count;
   int pack_ctas;
   int plan_cluster;       // CTAs per plan solve (thread-block cluster size)
+  int prio_high;          // greatest stream priority of the device (launch priority of the planner)
   // static layout, device
   int32_t* d_home;        // [E]   h(e)
   int32_t* d_main_phys;   // [E]   index of e among E_{h(e)} ascending
