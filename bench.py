@@ -460,7 +460,7 @@ def run_uep(args):
     # DRAM traffic per launch from the committed ncu --set full capture (dsv3_prefill only; that
     # capture is not re-taken here: a number printed under a profiler is never a bench value)
     traffic = {}
-    tpath = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r01_final_traffic.csv")
+    tpath = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "r01c_traffic.csv")
     if args.workload == "dsv3_prefill" and args.state_scale == 1.0 and os.path.exists(tpath):
         with open(tpath) as f:
             for line in f.read().splitlines()[1:]:

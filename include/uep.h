@@ -142,7 +142,9 @@ int uep_plan_bytes(const uep_ctx* ctx, uep_plan_sizes* out);      /* out: HOST *
 /* lambda_e = #{slots s : topk_ids[s] == e} (Alg. 1 line 2).
  *   topk_ids      DEVICE int32 [T,k] row-major (slot s = i*k + kk)
  *   expert_count  DEVICE int32 [E], overwritten
- *   ws            DEVICE workspace; afterwards holds the chunk count table for uep_remap    */
+ *   ws            DEVICE workspace (initialised); scratch: an accumulator that the call leaves
+ *                 zero again, and the per-CTA count rows.  Two kernels, the second one launched
+ *                 programmatically dependent on the first; asynchronous, capturable.          */
 int uep_histogram(const uep_ctx* ctx, const int32_t* topk_ids, int32_t* expert_count, void* ws,
                   void* stream);
 

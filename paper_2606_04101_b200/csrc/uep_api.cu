@@ -528,7 +528,8 @@ static int balance_impl(const uep_ctx* ctx, const int32_t* topk_ids, const void*
   // so the rank kernel does not depend on it): its CTAs take the SMs first, the rank CTAs fill in
   // as they retire and run beside the plan.  Measured on B200 (DSV3 shape, whole chain):
   // rank launched first 58.9 us, histogram first 54.5 us, rank made dependent on the histogram
-  // 62.5 us (its CTAs then race the plan's cluster for SMs).
+  // 62.5 us (its CTAs then race the plan's cluster for SMs).  Re-measured with the planner
+  // launched at high priority (chain 32.2 us): rank made dependent on the histogram 32.7 us.
   UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
   int rc2 = launch_histogram(c, topk_ids, expert_count, ws, s, /*red=*/true);
   UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
