@@ -215,8 +215,10 @@ __device__ __forceinline__ bool probe(const PlanSmem& sm, const int tau, const i
   return true;
 }
 
-template <int RPL>
-__global__ void __launch_bounds__(kPlanThreads, 1)
+// LOWREG (uep_plan_batched): two CTAs per SM at 64 registers — a single solve is slower that way
+// (16.5 against 15.4 us), many solves at once are faster (1.13 against 1.52 us per layer for 32)
+template <int RPL, bool LOWREG>
+__global__ void __launch_bounds__(kPlanThreads, LOWREG ? 2 : 1)
 plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict__ g_home,
             const int32_t* __restrict__ g_main_phys, const int32_t* __restrict__ g_roff,
             const int32_t* __restrict__ g_rexp, uep_plan_out out, int E, int R, int n_slot, int M,
@@ -246,6 +248,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   // touch both ends of the parameter block now: the emit phase reads the plan's pointers on the
   // critical path, and a cold constant-cache line there costs several hundred cycles
   if (out.slot_expert == nullptr || out.scalars == nullptr || count_out == reinterpret_cast<int32_t*>(1)) return;
+  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc, 2);
   // ---- stage inputs ---------------------------------------------------------------------
   pdl_trigger();                   // the lookup kernel may start its plan-independent prologue
   if (tid < E) {                   // static layout first: it does not depend on the histogram
@@ -255,6 +258,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   }
   if (tid <= R) sm.roff[tid] = g_roff[tid];
   pdl_wait();                      // the histogram (preceding kernel) is complete
+  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc, 3);
   UEP_STAMP(0);
   if (tid < E) sm.lam[tid] = acc ? __ldcg(acc + tid) : expert_count[tid];
   __syncthreads();
@@ -505,6 +509,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     ++round;
   }
   const int tau = sm.hi;
+  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc, 4);
   UEP_STAMP(8);
 #ifdef UEP_PLAN_TIMING
   t_bisect = clock64();
@@ -688,6 +693,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     o.scalars[UEP_SC_TAU_HI0] = tau_hi0;
     o.scalars[UEP_SC_N_GROUPS] = n_groups;
     for (int i = UEP_SC_N_GROUPS + 1; i < UEP_N_SCALARS; ++i) o.scalars[i] = 0;
+    UEP_TL_SET(acc, 5);
 #ifdef UEP_PLAN_TIMING   // developer probe: cycles of setup / bisection / final probe / emit
     o.scalars[9] = sm.tmax[0];
     o.scalars[10] = sm.tmax[1];
@@ -741,7 +747,8 @@ static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out&
   ++na;
   cfg.attrs = attr;
   cfg.numAttrs = na;
-  UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, plan_kernel<RPL>, count, (const int32_t*)c->d_home,
+  auto kern = n_inst > 1 ? plan_kernel<RPL, true> : plan_kernel<RPL, false>;
+  UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, count, (const int32_t*)c->d_home,
                                   (const int32_t*)c->d_main_phys, (const int32_t*)c->d_roff,
                                   (const int32_t*)c->d_rexp, plan, g.E, g.R, g.n_slot, c->M, c->P,
                                   g.u_min, g.beta_num, g.beta_den,
@@ -763,8 +770,10 @@ int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cu
 template <int RPL>
 static int init_plan_one(int& max16) {
   const int bytes = (int)(sizeof(PlanSmem) + 16 + kLogBudget);
-  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL, false>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(16);
   cfg.blockDim = dim3(kPlanThreads);
@@ -777,7 +786,7 @@ static int init_plan_one(int& max16) {
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   int n = 0;
-  if (cudaOccupancyMaxActiveClusters(&n, plan_kernel<RPL>, &cfg) != cudaSuccess) { cudaGetLastError(); n = 0; }
+  if (cudaOccupancyMaxActiveClusters(&n, plan_kernel<RPL, false>, &cfg) != cudaSuccess) { cudaGetLastError(); n = 0; }
   max16 = std::min(max16, n);
   return UEP_OK;
 }

@@ -358,6 +358,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   int2* stg = reinterpret_cast<int2*>(wtot + 36);     // staged {gate bits, out_gate index}, (expert, rank) order
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (blockIdx.x == 0 && threadIdx.x == 0) UEP_TL_SET(acc_clear, 6);
   const int c = LOCAL ? (int)blockIdx.x + chunk0 : (int)blockIdx.x;
   const bool local = LOCAL && cumq != nullptr;   // ranks local to (source rank, expert)
   const int grp = LOCAL ? c / cpg : 0, sub = LOCAL ? c % cpg : c;
@@ -402,6 +403,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   pdl_wait();
   // uep_balance: the planner (now complete) has consumed the histogram's accumulator; clear it for
   // the next call
+  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 7);
   if (acc_clear && c == 0) for (int e = tid; e < E; e += kRemapThreads) acc_clear[e] = 0;
   for (int e = tid; e <= E; e += kRemapThreads) s_off[e] = g_inst_off[e];
   for (int r = tid; r <= R; r += kRemapThreads) rbase[r] = g_rank_base[r];
@@ -499,6 +501,10 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
       }
     }
   }
+#ifdef UEP_TIMELINE
+  __syncthreads();
+  if (tid == 0) UEP_TL_MAX(acc_clear, 8);
+#endif
 }
 
 template <typename GateT>

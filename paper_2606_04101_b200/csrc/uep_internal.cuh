@@ -110,6 +110,23 @@ int init_hist_kernels();
 // kernel).  pdl_wait: block until the preceding kernel has completed and its writes are visible;
 // a no-op when the kernel was launched normally.
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+// Developer probe (-DUEP_TIMELINE): kernels of uep_balance stamp %globaltimer into the 256 reserved
+// bytes at the head of the workspace (32 slots; `acc` points just behind them).  Slots: 0 hist CTA 0
+// start, 1 hist end (max over CTAs), 2 plan CTA 0 start, 3 plan after the wait, 4 plan bisection
+// done, 5 plan end, 6 lookup CTA 0 start, 7 lookup CTA 0 after the wait, 8 lookup end (max over
+// CTAs), 9 the previous call's lookup end.
+#ifdef UEP_TIMELINE
+__device__ __forceinline__ unsigned long long tl_now() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t;
+}
+#define UEP_TL_SET(acc, i) do { if (acc) reinterpret_cast<unsigned long long*>(const_cast<int32_t*>(acc))[(i) - 32] = tl_now(); } while (0)
+#define UEP_TL_MAX(acc, i) do { if (acc) atomicMax(reinterpret_cast<unsigned long long*>(const_cast<int32_t*>(acc)) + ((i) - 32), tl_now()); } while (0)
+#else
+#define UEP_TL_SET(acc, i)
+#define UEP_TL_MAX(acc, i)
+#endif
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 #endif
 
