@@ -230,7 +230,8 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   const int csize = (int)cluster.num_blocks(), crank = (int)cluster.block_rank();
   // batched solve (uep_plan_batched): cluster b solves instance b; every array of instance b
   // starts b * (its element count) after instance 0's
-  const int batch_b = (int)blockIdx.x / csize;
+  const int csh = 31 - __clz(csize);                 // the cluster size is a power of two (init_plan_kernels)
+  const int batch_b = (int)blockIdx.x >> csh;
   expert_count += (size_t)batch_b * E;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   PlanSmem& sm = *reinterpret_cast<PlanSmem*>(smem_raw);
@@ -366,6 +367,16 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       }
     }
     if (tid == 0) sm.log_buf = -1;
+    // emit state, cleared here (off the path between the last probe and the plan's first store;
+    // no probe touches it): per-expert replica counts, first log entry, staged phys_count, and by
+    // CTA 0 the slot map in global memory (the emitting CTA writes it after a cluster barrier, or
+    // is CTA 0 itself when no round runs)
+    if (tid < E) { sm.u_main[tid] = sm.lam[tid]; sm.n_rep[tid] = 0; sm.first[tid] = 0x7fffffff; }
+    if (R * P <= kPcSmem) for (int i = tid; i < R * P; i += kPlanThreads) sm.pc[i] = 0;
+    if (crank == 0) {
+      int32_t* se = out.slot_expert + (size_t)batch_b * max(1, R * n_slot);
+      for (int i = tid; i < R * n_slot; i += kPlanThreads) se[i] = -1;
+    }
 #ifdef UEP_PLAN_TIMING
     if (tid < 8) sm.tmax[tid] = 0;
 #endif
@@ -520,7 +531,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   // last round did not log it (the final tau was found in an earlier round, or the log buffers do
   // not fit), CTA 0 runs one logged probe at the final tau.
   const int log_node = sm.log_buf;
-  const int owner = log_node < 0 ? 0 : log_node % csize;
+  const int owner = log_node < 0 ? 0 : (log_node & (csize - 1));
   if (crank != owner) return;
   UEP_STAMP(19);
   if (acc && tid < E) count_out[tid] = sm.lam[tid];
@@ -541,7 +552,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     o.scalars += bb * UEP_N_SCALARS;
     if (o.U) o.U += bb * E * R;
   }
-  const int log_buf = log_node < 0 ? 0 : 1 + log_node / csize;
+  const int log_buf = log_node < 0 ? 0 : 1 + (log_node >> csh);
   if (warp == 0 && sm.n_probes > 0 && log_node < 0) {
     int nl;
     probe<RPL, true>(sm, tau, R, n_slot, u_min, strict, lane, logs, nl);
@@ -549,12 +560,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   }
   const int4* lg = logs + (size_t)log_buf * log_cap;
   UEP_STAMP(20);
-  if (tid < E) { sm.u_main[tid] = sm.lam[tid]; sm.n_rep[tid] = 0; sm.first[tid] = 0x7fffffff; }
   const int RP = R * P;
   const bool pc_in_smem = RP <= kPcSmem;
   int* pc = pc_in_smem ? sm.pc : o.phys_count;
-  for (int i = tid; i < RP; i += kPlanThreads) pc[i] = 0;
-  for (int i = tid; i < R * n_slot; i += kPlanThreads) o.slot_expert[i] = -1;
+  if (!pc_in_smem) for (int i = tid; i < RP; i += kPlanThreads) pc[i] = 0;
   if (o.U) for (int i = tid; i < E * R; i += kPlanThreads) o.U[i] = 0;
   __syncthreads();
   UEP_STAMP(9);
