@@ -400,6 +400,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   if (lane == 31) wtot[warp] = el_inc;
   // ---- everything above is independent of the plan: under programmatic dependent launch it
   // overlaps the planner (uep_balance); now wait for it and stage the plan (coalesced, in L2) ------
+  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 10);
   pdl_wait();
   // uep_balance: the planner (now complete) has consumed the histogram's accumulator; clear it for
   // the next call

@@ -115,7 +115,8 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   // launch geometry.  Histogram: one CTA per chunk, one chunk per SM (whole 128-slot lines).
   // Remap (rank + lookup kernels): chunks of whole 512-slot steps, <= kMaxChunk slots (one
   // register-resident round), about two chunks per SM so that co-resident CTAs overlap their
-  // load / rank / store phases.
+  // load / rank / store phases.  (Measured: 274 chunks of 7680 slots, so that every lookup CTA is
+  // resident beside the planner's 8 SMs, gives a chain of 32.8 us against 32.0 us with 293 x 7168.)
   {
     long long per = (S + c->sm_count - 1) / c->sm_count;
     per = std::max<long long>(per, kMinChunk);
