@@ -359,6 +359,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (blockIdx.x == 0 && threadIdx.x == 0) UEP_TL_SET(acc_clear, 6);
+  if (threadIdx.x == 0) UEP_TL_MAX(acc_clear, 15);     // latest CTA start
   const int c = LOCAL ? (int)blockIdx.x + chunk0 : (int)blockIdx.x;
   const bool local = LOCAL && cumq != nullptr;   // ranks local to (source rank, expert)
   const int grp = LOCAL ? c / cpg : 0, sub = LOCAL ? c % cpg : c;
@@ -405,6 +406,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   // uep_balance: the planner (now complete) has consumed the histogram's accumulator; clear it for
   // the next call
   if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 7);
+  if (tid == 0) UEP_TL_MAX(acc_clear, 18);
   if (acc_clear && c == 0) for (int e = tid; e < E; e += kRemapThreads) acc_clear[e] = 0;
   for (int e = tid; e <= E; e += kRemapThreads) s_off[e] = g_inst_off[e];
   for (int r = tid; r <= R; r += kRemapThreads) rbase[r] = g_rank_base[r];
@@ -435,6 +437,8 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   }
   __syncthreads();
 
+  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 11);
+  if (tid == 0) UEP_TL_MAX(acc_clear, 16);
   int n_fly = 0;
   // two slots at a time: their records are loaded before any of them stores to shared memory
   // (the compiler cannot prove that the staging stores do not alias the records)
@@ -485,6 +489,9 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
       }
     }
   }
+  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 12);
+  if (tid == 0) UEP_TL_MAX(acc_clear, 17);
+  if (tid == kRemapThreads - 1) UEP_TL_MAX(acc_clear, 19);
   if (LOCAL && n_inflight) {                             // tokens of source rank grp that leave it
     n_fly = __reduce_add_sync(kFullMask, n_fly);
     if (lane == 0 && n_fly) atomicAdd(n_inflight + grp, n_fly);
@@ -505,6 +512,8 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
 #ifdef UEP_TIMELINE
   __syncthreads();
   if (tid == 0) UEP_TL_MAX(acc_clear, 8);
+  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 13);
+  if (blockIdx.x == gridDim.x - 1 && tid == 0) UEP_TL_SET(acc_clear, 14);
 #endif
 }
 

@@ -123,7 +123,10 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
     per = (per + 127) / 128 * 128;
     c->chunk_len = (int)per;
     c->n_chunks = (int)std::max<long long>(1, (S + per - 1) / per);
-    long long rper = (S + 2 * c->sm_count - 1) / (2 * c->sm_count);
+    int reserve = 0;                                      // SMs left out of the remap grid's sizing
+    if (const char* v = getenv("UEP_REMAP_SM_RESERVE")) reserve = atoi(v);   // developer sweeps only
+    const int r_sms = std::max(1, c->sm_count - std::max(0, reserve));
+    long long rper = (S + 2 * r_sms - 1) / (2 * r_sms);
     rper = std::max<long long>(rper, kMinChunk);
     rper = (rper + kRemapThreads - 1) / kRemapThreads * kRemapThreads;
     rper = std::min<long long>(rper, kMaxChunk);
