@@ -906,3 +906,47 @@ def test_back_to_back_calls_in_one_graph_full_size(entry):
         assert np.array_equal(o["off"].cpu().numpy(), off), (entry, b)
         nv = int(p.rank_base[-1])
         assert np.array_equal(o["og"].cpu().view(torch.int32).numpy().view(np.uint32)[:nv], og[:nv])
+
+
+def test_histogram_accumulator_stays_clean_between_calls():
+    """uep_histogram and uep_balance share the workspace's accumulator: each must leave it zero
+    (publish_kernel / the lookup clear it).  Many calls of both kinds on ONE workspace, back to back
+    in one CUDA graph and replayed, with different inputs and an invalid id: every count exact."""
+    T, k, E, R, ns, um = 30001, 8, 200, 25, 2, 64
+    ctx = binding.Context(T, k, E, R, ns, um)
+    ws, plan = ctx.new_workspace(), ctx.new_plan()
+    n = 6
+    ids = [synth.zipf_topk_ids(T, k, E, 0.5 + 0.3 * b, 70 + b) for b in range(n)]
+    ids[2][5, 1] = E + 3                                   # skipped, not counted (S14)
+    d_ids = [x.to(DEV) for x in ids]
+    counts = [torch.full((E,), -1, dtype=torch.int32, device=DEV) for _ in range(n)]
+    rep, rnk, off, _ = ctx.new_outputs(None)
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+
+    def run_all():
+        for b in range(n):
+            if b % 3 == 2:
+                ctx.uep_balance(d_ids[b], None, counts[b], plan, rep, rnk, off, None, [], [], ws)
+            else:
+                ctx.uep_histogram(d_ids[b], counts[b], ws)
+
+    with torch.cuda.stream(stream):
+        run_all()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            run_all()
+    torch.cuda.synchronize()
+    for _ in range(3):
+        for c in counts:
+            c.fill_(-1)
+        graph.replay()
+        torch.cuda.synchronize()
+        for b in range(n):
+            lam, bad = oracle.histogram(ids[b].numpy(), E)
+            assert np.array_equal(counts[b].cpu().numpy(), lam), b
+            assert bad == (1 if b == 2 else 0)
+    # the chunk table (by-product of uep_histogram): its rows sum to the counts
+    ctx.uep_histogram(d_ids[0], counts[0], ws)
+    torch.cuda.synchronize()
+    assert int(counts[0].sum()) == T * k
