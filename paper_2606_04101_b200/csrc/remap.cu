@@ -13,8 +13,8 @@
 //   lookup_kernel (plan-DEPENDENT) global rank = chunk base (the chunk's row of the exclusive
 //                 prefix over chunks, left by prefix_kernel) + rank in chunk; cumulative-quota
 //                 lookup; writes (replica, rank, offset) and the gates in dispatch order.  Under
-//                 programmatic dependent launch everything before its griddepcontrol.wait (packed
-//                 ranks, gates, prefix rows) overlaps the planner.
+//                 programmatic dependent launch everything before its griddepcontrol.wait (the
+//                 loads of packed ranks and gates) overlaps the planner.
 //
 // The source-aware variant (uep_remap_local, SolveReroute of Alg. 1 lines 26-36) reuses the same
 // kernels on chunks that never straddle a source rank's block of tokens, with reroute_kernel
@@ -131,15 +131,13 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
 // n_rows into the totals.  One CTA per int4 column group, one thread per row (blocks of 1024
 // rows with a carry): one L2 round trip per block instead of a serial walk.
 __global__ void __launch_bounds__(1024, 1)
-prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG, int trigger) {
+prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG) {
   __shared__ int4 wsum[32];
-  // launched programmatically dependent on rank_kernel: wait for it, and only then (trigger != 0:
-  // uep_remap, whose lookup reads the prefix rows AFTER its own wait) let the kernel behind this
-  // one start, so that its prologue may read what rank_kernel wrote.  uep_balance passes 0: its
-  // lookup reads the rows in its prologue, and under stream capture the lookup's programmatic
-  // launch attribute makes its edge from this kernel programmatic too.
+  // launched programmatically dependent on rank_kernel: wait for it, and only then let the kernel
+  // behind this one (the lookup) start: its prologue reads what rank_kernel wrote, and it reads this
+  // kernel's rows only after its own wait
   pdl_wait();
-  if (trigger) pdl_trigger();
+  pdl_trigger();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   int4* col = reinterpret_cast<int4*>(prefix) + blockIdx.x;
   int4 carry = make_int4(0, 0, 0, 0);
@@ -181,7 +179,7 @@ prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG, int trigger) {
 // virtual base of the global [S] array, only the shard's slots are dereferenced); n_launch < 0:
 // all chunks.  with_prefix = false leaves the raw per-chunk counts for the exchange step.
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local, int chunk0,
-                int n_launch, bool with_prefix, bool prefix_trigger) {
+                int n_launch, bool with_prefix) {
   if (c->S == 0) return UEP_OK;
   const int chunks = local ? c->l_chunks : c->r_chunks;
   const size_t smem = sizeof(int2) * (size_t)kRemapWarps * c->E_pad;
@@ -190,13 +188,13 @@ int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool
       local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S, ws_packed(c, ws),
       ws_prefix(c, ws), chunk0);
   UEP_CUDA_TRY(cudaGetLastError());
-  if (with_prefix) return launch_prefix(c, ws, s, local, /*pdl=*/true, prefix_trigger);
+  if (with_prefix) return launch_prefix(c, ws, s, local, /*pdl=*/true);
   return UEP_OK;
 }
 
 // pdl: launched programmatically dependent on the kernel before it in the stream (rank_kernel):
 // the launch latency overlaps that kernel
-int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local, bool pdl, bool trigger) {
+int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local, bool pdl) {
   if (c->S == 0) return UEP_OK;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(c->E_pad / 4);
@@ -209,7 +207,7 @@ int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local, bool pdl, 
   cfg.attrs = attr;
   cfg.numAttrs = pdl ? 1 : 0;
   UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, prefix_kernel, ws_prefix(c, ws),
-                                  local ? c->l_chunks : c->r_chunks, c->E_pad / 4, trigger ? 1 : 0));
+                                  local ? c->l_chunks : c->r_chunks, c->E_pad / 4));
   return UEP_OK;
 }
 
@@ -335,8 +333,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
               int32_t* __restrict__ out_rank, int32_t* __restrict__ out_offset,
               GateT* __restrict__ out_gate, int cpg, int group_len,
               const int32_t* __restrict__ cumq, const int32_t* __restrict__ srcpre,
-              int32_t* __restrict__ n_inflight, int32_t* __restrict__ acc_clear, int chunk0,
-              int early_wait) {
+              int32_t* __restrict__ n_inflight, int32_t* __restrict__ acc_clear, int chunk0) {
   // Token-sharded mode (LOCAL with cumq == nullptr): the grouped chunk geometry and
   // the per-source in-flight count of the source-aware mode, but GLOBAL ranks and the plan's own
   // cumulative quotas, on the chunks [chunk0, chunk0 + gridDim.x) that this GPU owns.
@@ -385,28 +382,24 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
     if (has_gate) gv[i] = in ? __ldg(gate + i * 32) : GateT(0);
   }
 
-  // early_wait (uep_remap): the preceding kernel is prefix_kernel, whose rows are read next; the
-  // loads above (packed ranks, gates) were complete before it started
-  if (early_wait) pdl_wait();
-  // ---- chunk base ranks: row c of the exclusive prefix over chunks that rank_kernel left ----------
+  // ---- everything above is independent of the plan and of prefix_kernel (the packed ranks were
+  // complete before prefix_kernel started): under programmatic dependent launch it overlaps the
+  // planner (uep_balance) or prefix_kernel (uep_remap); now wait for them ------------------------
+  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 10);
+  pdl_wait();
+  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 7);
+  if (tid == 0) UEP_TL_MAX(acc_clear, 18);
+  // ---- chunk base ranks: row c of the exclusive prefix over chunks that prefix_kernel left.  Read
+  // AFTER the wait, in the same L2 round trip as the plan below: under stream capture the lookup's
+  // programmatic attribute makes its edge from prefix_kernel programmatic too, and only the wait
+  // guarantees that kernel's writes are visible.  (Reading the rows in the prologue was 0.3 us
+  // faster and never observed stale; reading them early and verifying after the wait measured the
+  // same as this.) ---------------------------------------------------------------------------------
   const int p_own = (tid < E) ? __ldcg(prefix + (size_t)c * E_pad + tid) : 0;
   const int n_own = (tid < E) ? __ldcg(prefix + (size_t)(c + 1) * E_pad + tid) - p_own : 0;
   const int b0_own = (local && tid < E) ? p_own - __ldcg(prefix + (size_t)grp * cpg * E_pad + tid) : p_own;
-  int el_inc = n_own;                            // inclusive scan of n_own over experts
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int y = __shfl_up_sync(kFullMask, el_inc, o);
-    if (lane >= o) el_inc += y;
-  }
-  if (lane == 31) wtot[warp] = el_inc;
-  // ---- everything above is independent of the plan: under programmatic dependent launch it
-  // overlaps the planner (uep_balance); now wait for it and stage the plan (coalesced, in L2) ------
-  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 10);
-  pdl_wait();
   // uep_balance: the planner (now complete) has consumed the histogram's accumulator; clear it for
   // the next call
-  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 7);
-  if (tid == 0) UEP_TL_MAX(acc_clear, 18);
   if (acc_clear && c == 0) for (int e = tid; e < E; e += kRemapThreads) acc_clear[e] = 0;
   for (int e = tid; e <= E; e += kRemapThreads) s_off[e] = g_inst_off[e];
   for (int r = tid; r <= R; r += kRemapThreads) rbase[r] = g_rank_base[r];
@@ -415,6 +408,13 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
     i_rank[p] = g_inst_rank[p];
     i_base[p] = g_inst_base[p] + (local ? __ldcg(srcpre + (size_t)grp * inst_cap + p) : 0);
   }
+  int el_inc = n_own;                            // inclusive scan of n_own over experts
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int y = __shfl_up_sync(kFullMask, el_inc, o);
+    if (lane >= o) el_inc += y;
+  }
+  if (lane == 31) wtot[warp] = el_inc;
   __syncthreads();
   // rec[e] (E <= kRemapThreads: one thread per expert), in chunk-rank space: {cum - base0,
   // dbase + base0, gbase + base0, staging base << 19 | replica << 8 | rank} of the instance
@@ -522,7 +522,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
                            int32_t* out_replica, int32_t* out_rank, int32_t* out_offset,
                            GateT* out_gate, void* ws, cudaStream_t s, bool pdl, bool local,
                            int32_t* n_inflight, int32_t* acc_clear, int chunk0, int n_launch,
-                           bool src_aware, bool early_wait) {
+                           bool src_aware) {
   const uep_config& g = c->cfg;
   const int inst_cap = g.E + g.R * g.n_slot;
   const bool stage = gate != nullptr;
@@ -548,7 +548,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
                                   (const int32_t*)p.inst_cum, (const int32_t*)p.inst_base,
                                   (const int32_t*)p.rank_base, out_replica, out_rank, out_offset,
                                   out_gate, local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S,
-                                  cumq, srcpre, n_inflight, acc_clear, chunk0, early_wait ? 1 : 0));
+                                  cumq, srcpre, n_inflight, acc_clear, chunk0));
   return UEP_OK;
 }
 
@@ -570,15 +570,15 @@ int init_remap_kernels() {
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& p, int32_t* out_replica,
                   int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
                   bool pdl, bool local, int32_t* n_inflight, int32_t* acc_clear, int chunk0,
-                  int n_launch, bool src_aware, bool early_wait) {
+                  int n_launch, bool src_aware) {
   if (c->S == 0) return UEP_OK;
   if (c->cfg.gate_dtype == UEP_GATE_BF16 && gate)
     return launch_lookup_t<uint16_t>(c, static_cast<const uint16_t*>(gate), p, out_replica, out_rank,
                                      out_offset, static_cast<uint16_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear,
-                                     chunk0, n_launch, src_aware, early_wait);
+                                     chunk0, n_launch, src_aware);
   return launch_lookup_t<uint32_t>(c, static_cast<const uint32_t*>(gate), p, out_replica, out_rank,
                                    out_offset, static_cast<uint32_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear,
-                                   chunk0, n_launch, src_aware, early_wait);
+                                   chunk0, n_launch, src_aware);
 }
 
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& p,
@@ -588,8 +588,7 @@ int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_p
   if (rc != UEP_OK) return rc;
   // programmatically dependent on prefix_kernel: launch and the loads of packed ranks and gates
   // overlap it, the prefix rows are read after the wait
-  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s, /*pdl=*/true, false,
-                       nullptr, nullptr, 0, -1, true, /*early_wait=*/true);
+  return launch_lookup(c, gate, p, out_replica, out_rank, out_offset, out_gate, ws, s, /*pdl=*/true);
 }
 
 }  // namespace uep

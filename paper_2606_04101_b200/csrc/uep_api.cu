@@ -442,10 +442,9 @@ int uep_shard_finish(const uep_ctx* ctx, int32_t shard, int32_t n_shards, const 
   rc = launch_prefix(c, ws, s, /*local=*/true);
   // lambda_e = totals row of the scanned table; the planner publishes it as expert_count
   int32_t* totals = ws_prefix(c, ws) + (size_t)c->l_chunks * c->E_pad;
-  // (the planner is NOT launched programmatically dependent on prefix_kernel: the lookup behind it
-  // reads the prefix rows in its prologue, before its own griddepcontrol.wait, and an early planner
-  // would let that prologue start while prefix_kernel is still running)
-  if (rc == UEP_OK) rc = launch_plan(c, nullptr, *plan, s, /*pdl=*/false, 1, totals, expert_count);
+  // planner and lookup programmatically dependent on their predecessors (the lookup reads the prefix
+  // rows after its wait, i.e. after the planner, which itself waited for prefix_kernel)
+  if (rc == UEP_OK) rc = launch_plan(c, nullptr, *plan, s, /*pdl=*/true, 1, totals, expert_count);
   const size_t gb = c->cfg.gate_dtype == UEP_GATE_BF16 ? 2 : 4;
   if (rc == UEP_OK)
     rc = launch_lookup(c, virtual_base(gate_local, g.slot0, gb), *plan,
@@ -537,7 +536,7 @@ static int balance_impl(const uep_ctx* ctx, const int32_t* topk_ids, const void*
   UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
   int rc2 = launch_histogram(c, topk_ids, expert_count, ws, s, /*red=*/true);
   UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-  rc = launch_rank(c, topk_ids, ws, c->side, false, 0, -1, true, /*prefix_trigger=*/false);
+  rc = launch_rank(c, topk_ids, ws, c->side);
   UEP_CUDA_TRY(cudaEventRecord(c->ev_rank, c->side));
   // planner and lookup are launched programmatically dependent on their predecessor: their
   // prologues (static layout; packed ranks, gates, prefix rows) overlap it

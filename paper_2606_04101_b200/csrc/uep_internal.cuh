@@ -78,14 +78,13 @@ int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cu
 // uep_remap = launch_rank (plan-independent: stable rank of every slot inside its chunk, packed
 // with the expert id into the workspace) + launch_lookup (plan-dependent: cumulative-quota lookup).
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local = false,
-                int chunk0 = 0, int n_launch = -1, bool with_prefix = true, bool prefix_trigger = true);
-int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local, bool pdl = false, bool trigger = false);
+                int chunk0 = 0, int n_launch = -1, bool with_prefix = true);
+int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local, bool pdl = false);
 int launch_reroute(const Ctx* c, const uep_plan_out& plan, int32_t* n_inflight, void* ws, cudaStream_t s);
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& plan, int32_t* out_replica,
                   int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
                   bool pdl = false, bool local = false, int32_t* n_inflight = nullptr,
-                  int32_t* acc_clear = nullptr, int chunk0 = 0, int n_launch = -1, bool src_aware = true,
-                  bool early_wait = false);
+                  int32_t* acc_clear = nullptr, int chunk0 = 0, int n_launch = -1, bool src_aware = true);
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& plan,
                  int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
                  void* ws, cudaStream_t s);
