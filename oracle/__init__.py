@@ -8,7 +8,9 @@ The arithmetic of O-1..O-4 lives in ``uep_oracle.cpp`` (plain single-threaded C+
 from reference/PAPER.md Algorithm 1 and §5.2); this module compiles it with g++ and marshals
 numpy arrays through ctypes.  The backward-path definitions O-5 (gradient reduction, fp64) and
 O-6 (inverse remap) are a few lines of numpy each, below; their pins are in
-tests/test_oracle_pins.py::test_grad_reduce_and_inverse_remap_pins.
+tests/test_oracle_pins.py::test_grad_reduce_and_inverse_remap_pins.  O-7 (relay trees) and O-8a
+(the source-wise split Q of SolveReroute) are plain Python loops below; O-8b (the per-token
+source-aware assignment) is the per-slot loop uep_oracle_remap_local in uep_oracle.cpp.
 """
 from __future__ import annotations
 
@@ -49,7 +51,7 @@ def _load():
     if _lib is None:
         _lib = ctypes.CDLL(build())
         for name in ("uep_oracle_histogram", "uep_oracle_layout", "uep_oracle_plan",
-                     "uep_oracle_remap", "uep_oracle_pack"):
+                     "uep_oracle_remap", "uep_oracle_remap_local", "uep_oracle_pack"):
             getattr(_lib, name).restype = ctypes.c_int
     return _lib
 
@@ -330,41 +332,42 @@ def remap_local(ids: np.ndarray, gate: np.ndarray | None, pl: Plan):
     cumulative over q[r,e,.] in instance order.  Receive order inside an instance (the paper leaves
     it to the dispatch library; reading S25): by source rank ascending, then local order, so
     offset = inst_base + sum_{r'<r} q[r',e,i] + (j - cumulative before i).
-    Returns (replica, rank, offset, out_gate, q_list, n_inflight[R])."""
+
+    The split Q is O-8a (reroute_split, above) on Lambda[r,e] counted here slot by slot; the
+    assignment itself is the plain per-slot loop uep_oracle_remap_local in uep_oracle.cpp (next to
+    O-3, same shape).  Returns (replica, rank, offset, out_gate, q_list, n_inflight[R])."""
     ids32 = _i32(ids)
     T, k = ids32.shape
     E, R = pl.E, pl.R
     flat = ids32.reshape(-1)
     S = flat.size
-    src = np.repeat(source_rank(T, R), k)
+    src = np.repeat(source_rank(T, R), k)                    # S1: source rank of every slot
     valid = (flat >= 0) & (flat < E)
-    Lam = np.zeros((R, E), dtype=np.int64)
+    Lam = np.zeros((R, E), dtype=np.int64)                   # lambda_{r,e}: a plain count
     np.add.at(Lam, (src[valid], flat[valid]), 1)
     qs = reroute_split(Lam, pl)
-    rep = np.full(S, -1, np.int32); rnk = np.full(S, -1, np.int32); off = np.full(S, -1, np.int32)
-    inst_base = np.asarray(pl.phys_base).reshape(R, -1)
-    order = np.argsort(np.where(valid, src.astype(np.int64) * E + flat, np.int64(R) * E), kind="stable")
-    keys = (src.astype(np.int64) * E + flat)[order]
-    nv = int(valid.sum())
-    bounds = np.flatnonzero(np.diff(np.concatenate([[-1], keys[:nv]]))).tolist() + [nv]
-    for a, b in zip(bounds[:-1], bounds[1:]):
-        r, e = divmod(int(keys[a]), E)
-        lo = int(pl.inst_off[e])
-        q = qs[e]
-        cum = np.cumsum(q[r])
-        j = np.arange(b - a)
-        i = np.searchsorted(cum, j, side="right")
-        before = np.concatenate([[0], cum])[i]
-        srcpre = q[:r].sum(axis=0)
-        sl = order[a:b]
-        rep[sl] = i
-        rnk[sl] = pl.inst_rank[lo + i]
-        off[sl] = inst_base[pl.inst_rank[lo + i], pl.inst_phys[lo + i]] + srcpre[i] + (j - before)
-    out_gate = None
+    cap = int(np.asarray(pl.inst_rank).size)
+    q = np.zeros((R, cap), dtype=np.int64)                   # q[r][CSR entry]
+    for e in range(E):
+        lo, hi = int(pl.inst_off[e]), int(pl.inst_off[e + 1])
+        q[:, lo:hi] = qs[e]
+    rep, rnk, off = (np.empty(S, dtype=np.int32) for _ in range(3))
+    infl = np.zeros(R, dtype=np.int32)
     if gate is not None:
-        g = np.ascontiguousarray(gate).reshape(-1)
-        out_gate = np.zeros(S, dtype=g.dtype)
-        out_gate[pl.rank_base[rnk[valid]] + off[valid]] = g[valid]
-    n_inflight = np.bincount(src[valid & (rnk != src)], minlength=R).astype(np.int32)
+        gate = np.ascontiguousarray(gate).reshape(-1)
+        assert gate.size == S and gate.itemsize in (2, 4)
+        out_gate = np.zeros(S, dtype=gate.dtype)
+        gbytes = gate.itemsize
+    else:
+        out_gate, gbytes = None, 0
+    P = int(np.asarray(pl.phys_base).reshape(R, -1).shape[1])
+    rc = _load().uep_oracle_remap_local(
+        _p(flat), _p(gate), ctypes.c_int32(gbytes), ctypes.c_int64(T), ctypes.c_int32(k),
+        ctypes.c_int32(E), ctypes.c_int32(R), ctypes.c_int32(P), ctypes.c_int32(cap),
+        _p(_i32(pl.inst_off)), _p(_i32(pl.inst_rank)), _p(_i32(pl.inst_phys)), _p(q),
+        _p(np.ascontiguousarray(pl.phys_base, dtype=np.int32).reshape(-1)), _p(_i32(pl.rank_base)),
+        _p(rep), _p(rnk), _p(off), _p(out_gate), _p(infl))
+    if rc != 0:
+        raise ValueError(f"uep_oracle_remap_local rc={rc}")
     shp = ids32.shape
-    return rep.reshape(shp), rnk.reshape(shp), off.reshape(shp), out_gate, qs, n_inflight
+    return rep.reshape(shp), rnk.reshape(shp), off.reshape(shp), out_gate, qs, infl

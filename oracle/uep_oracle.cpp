@@ -14,6 +14,9 @@
 //                   cumulative quota covers j (upper-bound lookup)
 //   O-4 pack      : §4.2 forward weight distribution main -> replica slot,
 //                   on one GPU = a byte copy per (rank, redundant slot, tensor)
+//   O-8b remap_local : §5.2 "Token Assignment" per (source rank, expert) pair
+//                   over the source-wise split Q of Alg. 1 lines 26-36 (Q itself, O-8a, is
+//                   computed by oracle/__init__.py::reroute_split and passed in)
 //
 // The planner is a heuristic (bisection over a greedy probe), so O-2 follows Algorithm 1
 // step by step in the paper's order and notation; no blocking, fusion, early exit or
@@ -21,8 +24,9 @@
 // Readings of points the paper leaves open are the ones listed in DESIGN.md §3
 // (S1..S23); each is marked at the line that applies it.
 //
-// Pins (tests/test_oracle_*.py, all `-m "not gpu"`): hand-worked examples A and B
-// (tests/golden/), the all-slots-to-one-expert closed form, the paper's constraints as
+// Pins (tests/test_oracle_*.py, all `-m "not gpu"`): hand-worked examples A and B and the
+// per-token example of the source-aware assignment (tests/golden/), the
+// all-slots-to-one-expert closed form, the paper's constraints as
 // invariants, numpy bincount / stable argsort, strict==tolerant at u_min=1, identity
 // cases, and an exhaustive optimum bound on the tiny config.  No function here is
 // "parity unpinned"; the reading S3 (rounding of tau_lo) is unpinned BY THE PAPER and is
@@ -296,6 +300,56 @@ int uep_oracle_remap(const int32_t* ids, const void* gate, int32_t gate_bytes, i
     out_replica[s] = i; out_rank[s] = rank; out_offset[s] = (int32_t)off;
     if (gsrc && gdst)
       std::memcpy(gdst + (rank_base[rank] + off) * gate_bytes, gsrc + s * gate_bytes, gate_bytes);
+  }
+  return 0;
+}
+
+// ---- O-8b -----------------------------------------------------------------------------
+// Source-aware token assignment (§5.2 "Token Assignment"): "the j-th local token
+// of pair (r, e) is sent to the first physical instance whose cumulative quota covers j", the
+// cumulative quotas being those of the source-wise split q[r,e,.] (Alg. 1 lines 26-36, computed
+// by the caller: O-8a) in instance order.  Written as O-3 is: one pass over the slots in flat
+// order, one counter per (source rank, expert) pair.
+//   src(s)    = floor(i*R/T) for token i = s / k                                    (S1)
+//   j         = #{s' < s : src(s') == src(s), ids[s'] == ids[s]}      (local stable rank)
+//   instance  = first i with q[r][lo+0] + .. + q[r][lo+i] > j
+//   offset    = phys_base[rank][phys] + sum_{r' < r} q[r'][lo+i] + (j - cumulative before i)
+//               (S25: inside an instance tokens arrive by source rank, then local order)
+// q: [R][inst_cap] int64, q[r][p] = q_{r,e,t} for CSR entry p of the plan (instance of e on t).
+// n_inflight[r] (may be NULL) = slots of source rank r whose destination rank is not r.
+int uep_oracle_remap_local(const int32_t* ids, const void* gate, int32_t gate_bytes, int64_t T,
+                           int32_t k, int32_t E, int32_t R, int32_t P, int32_t inst_cap,
+                           const int32_t* inst_off, const int32_t* inst_rank,
+                           const int32_t* inst_phys, const int64_t* q,
+                           const int32_t* phys_base, const int32_t* rank_base,
+                           int32_t* out_replica, int32_t* out_rank, int32_t* out_offset,
+                           void* out_gate, int32_t* n_inflight) {
+  std::vector<int64_t> seen((size_t)R * E, 0);
+  const unsigned char* gsrc = (const unsigned char*)gate;
+  unsigned char* gdst = (unsigned char*)out_gate;
+  if (n_inflight) for (int r = 0; r < R; ++r) n_inflight[r] = 0;
+  for (int64_t s = 0; s < T * k; ++s) {
+    const int32_t e = ids[s];
+    if (e < 0 || e >= E) { out_replica[s] = out_rank[s] = out_offset[s] = -1; continue; }
+    const int r = (int)(((s / k) * R) / T);                   // source rank of the token (S1)
+    const int64_t j = seen[(size_t)r * E + e]++;              // j-th local token of pair (r, e)
+    const int lo = inst_off[e], n = inst_off[e + 1] - inst_off[e];
+    int i = 0;
+    int64_t cum = 0, before = 0;
+    for (; i < n; ++i) {                                      // first instance whose cumulative
+      before = cum;                                           // quota of THIS source covers j
+      cum += q[(size_t)r * inst_cap + lo + i];
+      if (cum > j) break;
+    }
+    if (i >= n) return -2;                                    // split does not cover the demand
+    int64_t from_lower = 0;                                   // tokens of lower source ranks come first
+    for (int rr = 0; rr < r; ++rr) from_lower += q[(size_t)rr * inst_cap + lo + i];
+    const int rank = inst_rank[lo + i], phys = inst_phys[lo + i];
+    const int64_t off = phys_base[rank * P + phys] + from_lower + (j - before);
+    out_replica[s] = i; out_rank[s] = rank; out_offset[s] = (int32_t)off;
+    if (gsrc && gdst)
+      std::memcpy(gdst + (rank_base[rank] + off) * gate_bytes, gsrc + s * gate_bytes, gate_bytes);
+    if (n_inflight && rank != r) n_inflight[r] += 1;
   }
   return 0;
 }

@@ -61,6 +61,10 @@ def test_worked_examples(name):
         assert got == transfers
         assert p.inst_cum[p.inst_off[0]:p.inst_off[1]].tolist() == \
             [int(x) for x in g["cum_e0"].split()]
+        # S13: local physical slot of every instance (main: index among E_h(e); replica: M + slot)
+        assert p.M == int(g["M"])
+        assert p.inst_phys[:p.inst_off[-1]].tolist() == [int(x) for x in g["inst_phys"].split()]
+        assert p.main_phys.tolist() == [p.inst_phys[p.inst_off[e]] for e in range(p.E)]
         ck.check_plan(lam, p, int(g["u_min"]), bn, bd, fm)
 
 
@@ -376,6 +380,44 @@ def test_relay_plan_pins():
         assert (parent[p.inst_off[-1]:] == -1).all()
 
 
+@pytest.mark.parametrize("name", ["example_local_A.txt", "example_local_B.txt"])
+def test_local_remap_worked_examples_per_token(name):
+    """O-8a + O-8b against hand-worked per-token literals (tests/golden/README.md): the split Q,
+    and (replica, rank, offset) of EVERY slot, including a source that spills to a remote replica
+    and two sources landing in one instance (reading S25 fixes their order), invalid ids, the gate
+    placement and the in-flight counts."""
+    import types
+    g = _read_golden(name)
+    ints = lambda key: [int(x) for x in g[key].split()]
+    E, R, T, k = int(g["E"]), int(g["R"]), int(g["T"]), int(g["k"])
+    P = len(ints("phys_base")) // R
+    pl = types.SimpleNamespace(
+        E=E, R=R, n_slot=int(g["n_slot"]), inst_off=np.array(ints("inst_off"), np.int32),
+        inst_rank=np.array(ints("inst_rank"), np.int32), inst_phys=np.array(ints("inst_phys"), np.int32),
+        inst_cum=np.array(ints("inst_cum"), np.int32),
+        phys_base=np.array(ints("phys_base"), np.int32).reshape(R, P),
+        rank_base=np.array(ints("rank_base"), np.int32))
+    ids = np.array(ints("ids"), np.int32).reshape(T, k)
+    Lam = np.array(ints("Lambda")).reshape(R, E)
+    qs = oracle.reroute_split(Lam, pl)
+    for e in range(E):
+        assert qs[e].reshape(-1).tolist() == ints(f"q_e{e}"), e
+    gate = (np.arange(T * k, dtype=np.uint32) * np.uint32(2654435761) + np.uint32(7)).reshape(T, k)
+    rep, rnk, off, og, qs2, infl = oracle.remap_local(ids, gate, pl)
+    assert rep.reshape(-1).tolist() == ints("replica")
+    assert rnk.reshape(-1).tolist() == ints("rank")
+    assert off.reshape(-1).tolist() == ints("offset")
+    assert infl.tolist() == ints("n_inflight")
+    assert all(np.array_equal(a, b) for a, b in zip(qs, qs2))       # Lambda counted from the ids
+    want = np.zeros(T * k, np.uint32)                                # gates land at rank_base + offset
+    for s, (t, o) in enumerate(zip(ints("rank"), ints("offset"))):
+        if t >= 0:
+            want[ints("rank_base")[t] + o] = gate.reshape(-1)[s]
+    assert np.array_equal(og, want)
+    v = ck.remap_local_vectorised(ids, pl, qs)                       # the sort-based cross-check agrees
+    assert all(np.array_equal(a, b) for a, b in zip(v, (rep, rnk, off)))
+
+
 def test_reroute_split_and_local_remap_pins():
     """O-8 against what the paper fixes: the hand-worked split below; both marginals of Q (Table 1,
     PAPER.md:133-135: sum_t q = lambda_{r,e}, sum_r q = u_{e,t}); local quota consumed first
@@ -419,6 +461,8 @@ def test_reroute_split_and_local_remap_pins():
                 b0 = p.phys_base[t, p.inst_phys[lo + i]]
                 assert (rnk.reshape(-1)[m] == t).all()
                 assert np.array_equal(np.sort(off.reshape(-1)[m]), b0 + np.arange(u[i]))
+        v = ck.remap_local_vectorised(ids, p, qs)                  # sort-based cross-check of the loop
+        assert all(np.array_equal(a, b) for a, b in zip(v, (rep, rnk, off)))
         g_rep, g_rnk, g_off, _ = oracle.remap(ids, None, p)
         assert infl.sum() == (rnk.reshape(-1) != src).sum()
         assert infl.sum() <= (g_rnk.reshape(-1) != src).sum()

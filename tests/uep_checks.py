@@ -152,3 +152,36 @@ def check_pack(slot_expert, src, dst, sentinel_dst):
             e = X[t, k]
             ref = s[e] if e >= 0 else s0[t, k]
             assert np.array_equal(d[t, k].view(np.uint8), ref.view(np.uint8)), (t, k, e)
+
+
+def remap_local_vectorised(ids, pl, qs):
+    """Cross-check of the oracle's per-slot loop O-8b (oracle.remap_local): the same assignment
+    computed the way a fast implementation would (stable argsort over (source rank, expert),
+    searchsorted per group).  qs = oracle.reroute_split's list.  Returns (replica, rank, offset)."""
+    ids32 = np.ascontiguousarray(ids, dtype=np.int32)
+    T, k = ids32.shape
+    E, R = pl.E, pl.R
+    flat = ids32.reshape(-1)
+    S = flat.size
+    src = np.repeat((np.arange(T, dtype=np.int64) * R // max(T, 1)), k)
+    valid = (flat >= 0) & (flat < E)
+    rep = np.full(S, -1, np.int32); rnk = np.full(S, -1, np.int32); off = np.full(S, -1, np.int32)
+    inst_base = np.asarray(pl.phys_base).reshape(R, -1)
+    order = np.argsort(np.where(valid, src * E + flat, np.int64(R) * E), kind="stable")
+    keys = (src * E + flat)[order]
+    nv = int(valid.sum())
+    bounds = np.flatnonzero(np.diff(np.concatenate([[-1], keys[:nv]]))).tolist() + [nv]
+    for a, b in zip(bounds[:-1], bounds[1:]):
+        r, e = divmod(int(keys[a]), E)
+        lo = int(pl.inst_off[e])
+        q = qs[e]
+        cum = np.cumsum(q[r])
+        j = np.arange(b - a)
+        i = np.searchsorted(cum, j, side="right")
+        before = np.concatenate([[0], cum])[i]
+        srcpre = q[:r].sum(axis=0)
+        sl = order[a:b]
+        rep[sl] = i
+        rnk[sl] = pl.inst_rank[lo + i]
+        off[sl] = inst_base[pl.inst_rank[lo + i], pl.inst_phys[lo + i]] + srcpre[i] + (j - before)
+    return rep.reshape(ids32.shape), rnk.reshape(ids32.shape), off.reshape(ids32.shape)
