@@ -71,10 +71,16 @@ enum { UEP_SC_TAU = 0,           /* final threshold tau (Alg. 1: tau_hi on exit)
        UEP_SC_N_GROUPS = 8,      /* number of experts with at least one replica                  */
        UEP_N_SCALARS = 16 };
 
-typedef struct uep_ctx uep_ctx;  /* opaque; immutable after uep_create */
+/* Opaque.  Shapes, launch geometry and the static layout are immutable after uep_create.  The
+ * context also owns a little MUTABLE launch state: the internal side stream and three events that
+ * uep_balance forks and joins on, a round-robin index into the work-counter pool of uep_pack /
+ * uep_grad_reduce, and a launch counter (uep_launch_count) — see the threading rules above. */
+typedef struct uep_ctx uep_ctx;
 
 typedef struct uep_config {
-  int32_t T, k;                  /* tokens and top-k; S = T*k < 2^24 slots                       */
+  int32_t T, k;                  /* tokens and top-k; S = T*k < 2^24 slots (S20: the
+                                    planner packs a rank's slack into 24 bits of its arg-max key;
+                                    the BASELINE configs reach 2^22)                              */
   int32_t E, R, n_slot;          /* 1<=E<=512, 1<=R<=256, 0<=n_slot<=4                            */
   int32_t u_min;                 /* quota floor u_min >= 1 (paper: 1024)           */
   int32_t beta_num, beta_den;    /* balancing target beta as a rational (paper: 101/100)         */
@@ -134,7 +140,10 @@ void uep_destroy(uep_ctx* ctx);
 /* Bytes of DEVICE workspace one in-flight call needs (scratch of the histogram's chunk table,
  * and of the remap: per-chunk expert counts, their exclusive prefix over chunks and one packed
  * int32 {expert, rank inside chunk} per slot, ~4 bytes per slot in total).
- * uep_workspace_init must be called once (async on `stream`) before first use. */
+ * uep_workspace_init must be called once (async on `stream`) before first use: it zeroes the
+ * histogram's accumulator and the first row of the remap's prefix table, which every call then
+ * leaves zero again.  (A departure from the header SURVEY.md §8(b) proposed, which had no such
+ * call: the alternative is a memset node in every uep_balance.) */
 size_t uep_workspace_bytes(const uep_ctx* ctx);
 int uep_workspace_init(const uep_ctx* ctx, void* ws, void* stream);
 int uep_plan_bytes(const uep_ctx* ctx, uep_plan_sizes* out);      /* out: HOST */
@@ -274,7 +283,9 @@ int uep_remap_inverse(const uep_ctx* ctx, const int32_t* out_rank, const int32_t
  * events on a side stream: uep_remap_rank runs beside histogram + plan (it does not depend on
  * them), and pack runs beside uep_remap_lookup, overlapping the reroute with the weight
  * distribution as in Eq. 1, max(T_reroute, T_w_distr).  Capturable.
- * n_tensors may be 0. */
+ * n_tensors may be 0.  If a launch fails part-way (UEP_ERR_CUDA / UEP_ERR_UNSUPPORTED from a
+ * stage), the side stream is joined back into `stream` before returning, so an enclosing stream
+ * capture stays valid, and the workspace's accumulator is cleared: the workspace can be reused. */
 int uep_balance(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
                 int32_t* expert_count, const uep_plan_out* plan, int32_t* out_replica,
                 int32_t* out_rank, int32_t* out_offset, void* out_gate, int32_t n_tensors,
@@ -291,6 +302,10 @@ int uep_balance_host(const uep_ctx* ctx, const int32_t* topk_ids_host, const voi
                      int32_t* out_rank_host, int32_t* out_offset_host, void* out_gate_host,
                      int32_t* scalars_host, int32_t n_tensors, const void* const* src,
                      const size_t* bytes_per_expert, void* const* dst, void* ws, void* stream);
+
+/* Number of kernels launched through this context so far (host-side count, all entry points).
+ * The bench reports the difference over its timed region as gpu_launches. */
+unsigned long long uep_launch_count(const uep_ctx* ctx);
 
 const char* uep_strerror(int code);
 const char* uep_last_cuda_error(void);   /* text of the last CUDA error seen on this thread */

@@ -27,7 +27,8 @@ EXPORTS = ["uep_create", "uep_destroy", "uep_workspace_bytes", "uep_workspace_in
            "uep_remap_rank", "uep_shard_count", "uep_shard_rows", "uep_shard_finish",
            "uep_remap_lookup", "uep_remap_inverse", "uep_relay_plan", "uep_pack", "uep_grad_reduce",
            "uep_balance",
-           "uep_balance_host", "uep_strerror", "uep_last_cuda_error", "uep_get_launch_info"]
+           "uep_balance_host", "uep_strerror", "uep_last_cuda_error", "uep_get_launch_info",
+           "uep_launch_count"]
 
 
 class UepError(RuntimeError):
@@ -78,6 +79,7 @@ def lib():
         L.uep_strerror.restype = ctypes.c_char_p
         L.uep_last_cuda_error.restype = ctypes.c_char_p
         L.uep_destroy.restype = None
+        L.uep_launch_count.restype = ctypes.c_ulonglong
         _lib = L
     return _lib
 
@@ -177,6 +179,10 @@ class Context:
             self.close()
         except Exception:
             pass
+
+    def uep_launch_count(self) -> int:
+        """Kernels launched through this context so far (host-side count kept by the library)."""
+        return int(lib().uep_launch_count(self._h))
 
     # ---- allocation helpers (PyTorch = device memory only) ------------------------------
     def workspace_bytes(self) -> int:

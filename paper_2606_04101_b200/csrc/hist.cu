@@ -47,12 +47,6 @@ hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
   const int tid = threadIdx.x, warp = tid >> 5;
   const int c = blockIdx.x;
   pdl_trigger();     // the kernel behind this one (planner / publish_kernel) may start its prologue
-#ifdef UEP_TIMELINE
-  if (c == 0 && tid == 0) {
-    reinterpret_cast<unsigned long long*>(acc)[9 - 32] = reinterpret_cast<unsigned long long*>(acc)[8 - 32];
-    UEP_TL_SET(acc, 0);
-  }
-#endif
 
   const long long begin = (long long)c * chunk_len;
   const int len = (int)min((long long)chunk_len, (long long)S - begin);   // > 0 by construction
@@ -95,10 +89,6 @@ hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
     if (s != 0 && e < E) atomicAdd(acc + e, s);          // result unused: a fire-and-forget RED
     if (TABLE) table[(size_t)c * E_pad + e] = s;
   }
-#ifdef UEP_TIMELINE
-  __syncthreads();
-  if (tid == 0) UEP_TL_MAX(acc, 1);
-#endif
 }
 
 // uep_histogram's second kernel, one CTA, launched programmatically dependent on hist_kernel (its
@@ -134,6 +124,7 @@ int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws,
   if (c->S == 0) {
     if (!red) hist_empty_kernel<<<1, 256, 0, s>>>(c->cfg.E, c->E_pad, ws_table(ws), count);
     UEP_CUDA_TRY(cudaGetLastError());
+    if (!red) count_launch(c);
     return UEP_OK;
   }
   const size_t smem = sizeof(int) * (hist_smem_ints(c->E_pad) + 4);
@@ -144,6 +135,7 @@ int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws,
     hist_kernel<false><<<c->n_chunks, kHistThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
                                                                c->chunk_len, ws_table(ws), ws_acc(ws));
     UEP_CUDA_TRY(cudaGetLastError());
+    count_launch(c);
     return UEP_OK;
   }
   hist_kernel<true><<<c->n_chunks, kHistThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad,
@@ -159,6 +151,7 @@ int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws,
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, publish_kernel, c->cfg.E, ws_acc(ws), count));
+  count_launch(c, 2);
   return UEP_OK;
 }
 

@@ -20,47 +20,6 @@ constexpr int kPackThreads = 32;
 constexpr int kPackPending = 1;          // store groups allowed in flight when a stage is reused
 constexpr int kPackAhead = kPackStages - 1 - kPackPending;   // loads issued ahead of the stores
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
-               : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_LOOP:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE;\n"
-      "bra WAIT_LOOP;\n"
-      "DONE:\n"
-      "}\n" ::"r"(smem_u32(bar)), "r"(parity)
-      : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-          smem_u32(dst_smem)),
-      "l"(src), "r"(bytes), "r"(smem_u32(bar))
-      : "memory");
-}
-__device__ __forceinline__ void bulk_s2g(void* dst, const void* src_smem, uint32_t bytes) {
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst),
-               "r"(smem_u32(src_smem)), "r"(bytes)
-               : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void bulk_wait_read() {
-  asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
-}
-__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-
 // A unit = one source tile and its destinations.  Units are numbered expert-major over the
 // replicated experts only: u = (index of e among replicated experts) * TPE + (tile index over the
 // expert's tensors in order), TPE = sum_j ceil(B_j / kPackTile).
@@ -100,8 +59,8 @@ pack_kernel(PackArgs a, int E, int n_slot, int M, const int32_t* __restrict__ in
   __syncwarp();
   if (lane != 0) return;                                // one elected thread drives the TMA engine
   for (int s = 0; s < kPackStages; ++s) mbar_init(&full[s], 1);
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  mbar_fence_init();
+  fence_proxy_async();
 
   unsigned tiles_of[UEP_MAX_TENSORS];
   unsigned tpe = 0;
@@ -168,7 +127,7 @@ pack_kernel(PackArgs a, int E, int n_slot, int M, const int32_t* __restrict__ in
     }
     const int st = (int)(n_stored % kPackStages);
     mbar_wait(&full[st], (uint32_t)((n_stored / kPackStages) & 1));
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    fence_proxy_async();
     const Unit u = ring[st];
     const int lo = inst_off[u.e], hi = inst_off[u.e + 1];
     const unsigned long long B = a.bytes[u.j];
@@ -203,6 +162,7 @@ int launch_pack(const Ctx* c, const uep_plan_out& plan, const PackArgs& a, cudaS
   pack_kernel<<<c->pack_ctas, kPackThreads, kPackStages * kPackTile, s>>>(
       a, c->cfg.E, c->cfg.n_slot, c->M, plan.inst_off, plan.inst_rank, plan.inst_phys, next_counter(c));
   UEP_CUDA_TRY(cudaGetLastError());
+  count_launch(c);
   return UEP_OK;
 }
 

@@ -32,12 +32,6 @@ namespace uep {
 
 namespace cg = cooperative_groups;
 
-#ifdef UEP_PLAN_TIMING     // developer probe: cycle stamps at the barriers of setup and emit, printed by the emitting CTA
-#define UEP_STAMP(i) do { if (tid == 0) stamps[i] = clock64(); } while (0)
-#else
-#define UEP_STAMP(i)
-#endif
-
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kMaxLog = UEP_MAX_R * UEP_MAX_NSLOT;      // 1024 accepted transfers at most
 constexpr int kPlanWarps = kPlanThreads / 32;
@@ -78,9 +72,6 @@ struct PlanSmem {
   unsigned long long scan_tmp[32];
   int feas[32];
   int lo, hi, n_probes, n_log, log_buf;
-#ifdef UEP_PLAN_TIMING
-  int tmax[8];
-#endif
   long long s_valid;
   int max_ell;
 };
@@ -241,15 +232,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   int4* logs = reinterpret_cast<int4*>(smem_raw + ((sizeof(PlanSmem) + 15) & ~(size_t)15));
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool strict = strict_i != 0;
-#ifdef UEP_PLAN_TIMING
-  long long t_start = clock64(), t_setup = 0, t_bisect = 0, t_final = 0;
-  long long stamps[24] = {};
-#endif
 
   // touch both ends of the parameter block now: the emit phase reads the plan's pointers on the
   // critical path, and a cold constant-cache line there costs several hundred cycles
   if (out.slot_expert == nullptr || out.scalars == nullptr || count_out == reinterpret_cast<int32_t*>(1)) return;
-  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc, 2);
   // ---- stage inputs ---------------------------------------------------------------------
   pdl_trigger();                   // the lookup kernel may start its plan-independent prologue
   if (tid < E) {                   // static layout first: it does not depend on the histogram
@@ -259,11 +245,8 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   }
   if (tid <= R) sm.roff[tid] = g_roff[tid];
   pdl_wait();                      // the histogram (preceding kernel) is complete
-  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc, 3);
-  UEP_STAMP(0);
   if (tid < E) sm.lam[tid] = acc ? __ldcg(acc + tid) : expert_count[tid];
   __syncthreads();
-  UEP_STAMP(1);
   // line 2: l_r
   if (tid < R) {
     int s = 0;
@@ -271,7 +254,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     sm.ell[tid] = s;
   }
   __syncthreads();
-  UEP_STAMP(2);
   // sum and max of l_r (R <= 256 -> first 8 warps)
   {
     int v = (tid < R) ? sm.ell[tid] : 0;
@@ -280,7 +262,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (lane == 0) { sm.warp_tmp[warp] = sum; sm.feas[warp] = mx; }
   }
   __syncthreads();
-  UEP_STAMP(3);
   if (warp == kPlanWarps - 1) {    // (the last warp has no expert to order below when E < kPlanThreads)
     // per-warp partials -> totals with two warp reductions (S < 2^31: 32-bit sums are exact)
     const int ps = (lane < kPlanWarps) ? sm.warp_tmp[lane] : 0;
@@ -302,9 +283,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       sm.n_log = 0;
     }
   }
-#ifdef UEP_PLAN_TIMING
-  const long long t_s1 = clock64();
-#endif
   // rank order: position = number of ranks that come before (l desc, id asc).  gsz threads per
   // rank (a power of two, all of the CTA's threads when R allows), each counting over a strided
   // part of the ranks with independent loads, then a shuffle reduction inside the group.  (A warp
@@ -313,7 +291,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     const int gsh = min(5, 9 - (32 - __clz(R - 1)));           // kPlanThreads = 2^9 >= R << gsh
     const int gsz = 1 << gsh, r = tid >> gsh, sub = tid & (gsz - 1);
     int cnt = 0;
-    UEP_STAMP(21);
     if (r < R) {
       const int lr = sm.ell[r];
 #pragma unroll 4
@@ -322,11 +299,9 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
         cnt += (lq > lr || (lq == lr && q < r)) ? 1 : 0;
       }
     }
-    UEP_STAMP(22);
     for (int o = gsz >> 1; o > 0; o >>= 1) cnt += __shfl_xor_sync(kFull, cnt, o);
     if (r < R && sub == 0) sm.order[cnt] = r;
   }
-  UEP_STAMP(17);
   if (tid < E) {
     // per-rank expert order: lambda desc, id asc; a thread per expert counts the experts of its
     // home rank that come before it; positions into u_main (temp)
@@ -341,15 +316,9 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     }
     sm.u_main[e] = a + cnt;
   }
-  UEP_STAMP(18);
   __syncthreads();
-  UEP_STAMP(4);
-#ifdef UEP_PLAN_TIMING
-  const long long t_s2 = clock64();
-#endif
   if (tid < E) sm.elist[sm.u_main[tid]] = tid;
   __syncthreads();
-  UEP_STAMP(5);
   // flat visit list: ranks in visit order, each with its experts in visit order (S5)
   {
     const int r = (tid < R) ? sm.order[tid] : 0;
@@ -367,6 +336,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       }
     }
     if (tid == 0) sm.log_buf = -1;
+    if (tid < 2 * kPlanMaxNodes) (&sm.node_feas[0][0])[tid] = 0;    // an unprobed slot never reads as a verdict
     // emit state, cleared here (off the path between the last probe and the plan's first store;
     // no probe touches it): per-expert replica counts, first log entry, staged phys_count, and by
     // CTA 0 the slot map in global memory (the emitting CTA writes it after a cluster barrier, or
@@ -377,16 +347,9 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       int32_t* se = out.slot_expert + (size_t)batch_b * max(1, R * n_slot);
       for (int i = tid; i < R * n_slot; i += kPlanThreads) se[i] = -1;
     }
-#ifdef UEP_PLAN_TIMING
-    if (tid < 8) sm.tmax[tid] = 0;
-#endif
   }
   __syncthreads();
   const int tau_lo0 = sm.lo, tau_hi0 = sm.hi;
-  UEP_STAMP(6);
-#ifdef UEP_PLAN_TIMING
-  t_setup = clock64();
-#endif
 
   // ---- bisection (S9): per round up to 2^levels - 1 nodes of the SEQUENTIAL bisection tree rooted
   // at the current [lo, hi) are probed speculatively, then the path the sequential search takes is
@@ -443,18 +406,12 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       if (valid) {
         int nl = 0;
         bool f;
-#ifdef UEP_PLAN_TIMING
-        const long long tp0 = clock64();
-#endif
         if (log_round) {
           f = probe<RPL, true>(sm, (l + h) >> 1, R, n_slot, u_min, strict, lane,
                                logs + (size_t)(1 + warp) * log_cap, nl);
         } else {
           f = probe<RPL, false>(sm, (l + h) >> 1, R, n_slot, u_min, strict, lane, nullptr, nl);
         }
-#ifdef UEP_PLAN_TIMING
-        if (lane < csize && round < 8) atomicMax(cluster.map_shared_rank(&sm.tmax[round], lane), (int)(clock64() - tp0));
-#endif
         if (lane < csize) {
           *cluster.map_shared_rank(&sm.node_feas[buf][slot], lane) = f ? 1 : 0;
           *cluster.map_shared_rank(&sm.log_n[buf][slot], lane) = nl;
@@ -520,11 +477,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     ++round;
   }
   const int tau = sm.hi;
-  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc, 4);
-  UEP_STAMP(8);
-#ifdef UEP_PLAN_TIMING
-  t_bisect = clock64();
-#endif
 
   // ---- materialise (S10).  The CTA holding the log of the final tau's probe emits the plan; the
   // others are done (nothing touches their shared memory after the last cluster barrier).  If the
@@ -533,7 +485,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   const int log_node = sm.log_buf;
   const int owner = log_node < 0 ? 0 : (log_node & (csize - 1));
   if (crank != owner) return;
-  UEP_STAMP(19);
   if (acc && tid < E) count_out[tid] = sm.lam[tid];
   uep_plan_out o = out;            // this instance's arrays (offset only here: the probes above
   if (batch_b != 0) {              // must not carry eleven pointers in registers)
@@ -559,18 +510,13 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (lane == 0) sm.n_log = nl;
   }
   const int4* lg = logs + (size_t)log_buf * log_cap;
-  UEP_STAMP(20);
   const int RP = R * P;
   const bool pc_in_smem = RP <= kPcSmem;
   int* pc = pc_in_smem ? sm.pc : o.phys_count;
   if (!pc_in_smem) for (int i = tid; i < RP; i += kPlanThreads) pc[i] = 0;
   if (o.U) for (int i = tid; i < E * R; i += kPlanThreads) o.U[i] = 0;
   __syncthreads();
-  UEP_STAMP(9);
   const int n_log = sm.n_log;
-#ifdef UEP_PLAN_TIMING
-  t_final = clock64();
-#endif
 
   // ---- emit (line 22 "materialize U~ into X" + cumulative reroute metadata, §5.2) ---------
 #pragma unroll
@@ -584,7 +530,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     }
   }
   __syncthreads();
-  UEP_STAMP(10);
   {
     // one block scan for both prefix sums: instances per expert (high word; <= E + R * n_slot) and
     // delta over the log, kLogPer entries per thread (low word; <= S < 2^24, so it never carries)
@@ -610,7 +555,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     }
   }
   __syncthreads();
-  UEP_STAMP(11);
   for (int i = tid; i <= E; i += kPlanThreads) o.inst_off[i] = sm.inst_off[i];
   int fan = 0;
   if (tid < E) {
@@ -646,7 +590,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     int mf = __reduce_max_sync(kFull, fan);
     int ng = __reduce_add_sync(kFull, (fan > 1) ? 1 : 0);
     __syncthreads();                                                // pc complete
-  UEP_STAMP(12);
     if (lane == 0) { sm.feas[warp] = mf; sm.warp_tmp[warp] = ng; }
   }
   // receive layout (S13): per rank exclusive prefix over its P physical slots
@@ -661,7 +604,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     o.rank_load[tid] = load;
   }
   __syncthreads();
-  UEP_STAMP(13);
   // inst_base: offset of each instance's first token in its rank's receive buffer (S13)
   {
     const int* pb = pc_in_smem ? pc : o.phys_base;      // bases (global ones are CTA-visible now)
@@ -678,7 +620,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   int max_fan = 0, n_groups = 0;
   if (tid == 0) for (int w = 0; w < kPlanWarps; ++w) { max_fan = max(max_fan, sm.feas[w]); n_groups += sm.warp_tmp[w]; }
   __syncthreads();
-  UEP_STAMP(14);
   {
     const int inc = block_incl_scan(load, sm.warp_tmp);
     if (tid < R) o.rank_base[tid] = inc - load;
@@ -687,7 +628,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     __syncthreads();
     if (lane == 0) sm.feas[warp] = mx;
     __syncthreads();
-  UEP_STAMP(15);
   }
   if (tid == 0) {
     int max_load = 0;
@@ -702,20 +642,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     o.scalars[UEP_SC_TAU_HI0] = tau_hi0;
     o.scalars[UEP_SC_N_GROUPS] = n_groups;
     for (int i = UEP_SC_N_GROUPS + 1; i < UEP_N_SCALARS; ++i) o.scalars[i] = 0;
-    UEP_TL_SET(acc, 5);
-#ifdef UEP_PLAN_TIMING   // developer probe: cycles of setup / bisection / final probe / emit
-    o.scalars[9] = sm.tmax[0];
-    o.scalars[10] = sm.tmax[1];
-    o.scalars[11] = sm.tmax[2];
-    o.scalars[12] = (int)(t_setup - t_start);
-    o.scalars[13] = (int)(t_bisect - t_setup);
-    o.scalars[14] = (int)(t_final - t_bisect);
-    o.scalars[15] = (int)(clock64() - t_final);
-    stamps[16] = clock64();
-    printf("plan stamps (cycles since start):");
-    for (int i = 0; i < 23; ++i) printf(" %d:%lld", i, stamps[i] ? stamps[i] - t_start : 0ll);
-    printf("\n");
-#endif
   }
 }
 
@@ -763,6 +689,7 @@ static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out&
                                   g.u_min, g.beta_num, g.beta_den,
                                   g.floor_mode == UEP_FLOOR_STRICT ? 1 : 0, c->S, n_bufs, log_cap,
                                   levels, acc, count_out));
+  count_launch(c);
   return UEP_OK;
 }
 
@@ -806,11 +733,11 @@ int init_plan_kernels(Ctx* c) {
   if (rc == UEP_OK) rc = init_plan_one<2>(max16);
   if (rc == UEP_OK) rc = init_plan_one<4>(max16);
   if (rc == UEP_OK) rc = init_plan_one<8>(max16);
+  // 8 CTAs x 8 probing warps cover the 64 tree slots of a round (launch_plan_t: levels = 6); the
+  // path walk relies on every speculated slot having an owner, so the size is not configurable
   c->plan_cluster = 8;
-  if (const char* e = getenv("UEP_PLAN_CLUSTER")) {        // developer override: 1, 2, 4, 8 or 16
-    const int v = atoi(e);
-    if (v == 1 || v == 2 || v == 4 || v == 8 || (v == 16 && max16 >= 1)) c->plan_cluster = v;
-  }
+  static_assert(8 * 8 >= kPlanMaxNodes, "every tree slot of a round needs a probing warp");
+  (void)max16;
   return rc;
 }
 

@@ -36,36 +36,6 @@ struct RedArgs {
   int n_tensors;
 };
 
-__device__ __forceinline__ uint32_t red_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void red_mbar_init(uint64_t* bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(red_smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void red_mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(red_smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void red_mbar_arrive(uint64_t* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(red_smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void red_mbar_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "RED_WAIT:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra RED_DONE;\n"
-      "bra RED_WAIT;\n"
-      "RED_DONE:\n"
-      "}\n" ::"r"(red_smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void red_bulk_g2s(void* dst_smem, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                   red_smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(red_smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void red_bulk_s2g(void* dst, const void* src_smem, uint32_t bytes) {
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(red_smem_u32(src_smem)),
-               "r"(bytes) : "memory");
-}
-
 // A unit = one tile of the main buffer and the same tile of every replica slot: 1 + f ring
 // stages.  Units are numbered expert-major over the replicated experts (as in pack.cu) and handed
 // out DYNAMICALLY in batches of kRedBatch from a self-resetting counter in global memory (a
@@ -96,10 +66,10 @@ grad_reduce_kernel(RedArgs a, int E, int n_slot, int M, const int32_t* __restric
   for (int i = tid; i < kRedTile / 16; i += kRedThreads)
     reinterpret_cast<float4*>(zero)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
   if (tid == 0) {
-    for (int s = 0; s < kRedStages; ++s) { red_mbar_init(&full[s], 1); red_mbar_init(&empty[s], kRedConsumers); }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    for (int s = 0; s < kRedStages; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], kRedConsumers); }
+    mbar_fence_init();
   }
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");       // zero tile visible to bulk stores
+  fence_proxy_async();                                               // zero tile visible to bulk stores
   __syncthreads();
   auto slot_of = [&](int p) { return __ldg(inst_rank + p) * n_slot + (__ldg(inst_phys + p) - M); };
 
@@ -126,13 +96,13 @@ grad_reduce_kernel(RedArgs a, int E, int n_slot, int M, const int32_t* __restric
     unsigned long long n = 0, unit = 0;                              // ring position, unit counter
     auto acquire = [&]() {                                           // stage n % kRedStages is free again
       const int st = (int)(n % kRedStages);
-      if (n >= kRedStages) red_mbar_wait(&empty[st], (uint32_t)(((n / kRedStages) - 1) & 1));
+      if (n >= kRedStages) mbar_wait(&empty[st], (uint32_t)(((n / kRedStages) - 1) & 1));
       return st;
     };
     auto load = [&](const unsigned char* src, uint32_t bytes) {
       const int st = acquire();
-      red_mbar_expect_tx(&full[st], bytes);
-      red_bulk_g2s(ring + (size_t)st * kRedTile, src, bytes, &full[st]);
+      mbar_expect_tx(&full[st], bytes);
+      bulk_g2s(ring + (size_t)st * kRedTile, src, bytes, &full[st]);
       ++n;
     };
     unsigned nxt = atomicAdd(ctr, kRedBatch);
@@ -169,7 +139,7 @@ grad_reduce_kernel(RedArgs a, int E, int n_slot, int M, const int32_t* __restric
     {                                                                // end marker: an empty stage
       const int st = acquire();
       units[unit % kRedUnitRing].f = -1;
-      red_mbar_arrive(&full[st]);
+      mbar_arrive(&full[st]);
     }
     __threadfence();                                                 // every request has returned
     if (atomicAdd(ctr + 1, 1u) == gridDim.x - 1) {                   // last CTA rearms the counters
@@ -186,7 +156,7 @@ grad_reduce_kernel(RedArgs a, int E, int n_slot, int M, const int32_t* __restric
   while (true) {
     {                                                    // the unit's first stage also publishes its descriptor
       const int st = (int)(n % kRedStages);
-      red_mbar_wait(&full[st], (uint32_t)((n / kRedStages) & 1));
+      mbar_wait(&full[st], (uint32_t)((n / kRedStages) & 1));
     }
     const RedUnit d = units[unit % kRedUnitRing];
     if (d.f < 0) break;
@@ -197,7 +167,7 @@ grad_reduce_kernel(RedArgs a, int E, int n_slot, int M, const int32_t* __restric
     float4 acc[kRedVec];
     for (int q = 0; q <= f; ++q) {                       // instance order: main, replica 1, 2, ...
       const int st = (int)(n % kRedStages);
-      if (q) red_mbar_wait(&full[st], (uint32_t)((n / kRedStages) & 1));
+      if (q) mbar_wait(&full[st], (uint32_t)((n / kRedStages) & 1));
       const float4* t = reinterpret_cast<const float4*>(ring + (size_t)st * kRedTile);
 #pragma unroll
       for (int v = 0; v < kRedVec; ++v) {
@@ -206,7 +176,7 @@ grad_reduce_kernel(RedArgs a, int E, int n_slot, int M, const int32_t* __restric
         if (q == 0) acc[v] = x;
         else { acc[v].x += x.x; acc[v].y += x.y; acc[v].z += x.z; acc[v].w += x.w; }
       }
-      red_mbar_arrive(&empty[st]);                       // this thread is done with the stage
+      mbar_arrive(&empty[st]);                       // this thread is done with the stage
       ++n;
     }
     // (A) the elected thread has waited until the stores of unit-2 finished reading outbuf[unit&1]
@@ -217,20 +187,20 @@ grad_reduce_kernel(RedArgs a, int E, int n_slot, int M, const int32_t* __restric
       const int i = v * kRedConsumers + ct;
       if (i < n4) ob[i] = acc[v];
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    fence_proxy_async();
     asm volatile("bar.sync 1, %0;" ::"n"(kRedConsumers) : "memory");      // (B) tile complete in shared memory
     if (ct == 0) {
       const unsigned long long B = a.bytes[j];
-      red_bulk_s2g(reinterpret_cast<unsigned char*>(a.main_grad[j]) + (unsigned long long)e * B + off, ob, bytes);
+      bulk_s2g(reinterpret_cast<unsigned char*>(a.main_grad[j]) + (unsigned long long)e * B + off, ob, bytes);
       for (int q = 1; q <= f; ++q)                       // cleared in place
-        red_bulk_s2g(reinterpret_cast<unsigned char*>(a.slot_grad[j]) + (unsigned long long)slot_of(lo + q) * B + off,
+        bulk_s2g(reinterpret_cast<unsigned char*>(a.slot_grad[j]) + (unsigned long long)slot_of(lo + q) * B + off,
                      zero, bytes);
-      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-      asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");  // unit-1's stores have read their smem
+      bulk_commit();
+      bulk_wait_read<1>();                               // unit-1's stores have read their smem
     }
     ++unit;
   }
-  if (ct == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+  if (ct == 0) bulk_wait_all();
 }
 
 __global__ void __launch_bounds__(256)
@@ -267,6 +237,7 @@ int launch_grad_reduce(const Ctx* c, const uep_plan_out& plan, int n_tensors, vo
                                                             plan.inst_off, plan.inst_rank,
                                                             plan.inst_phys, next_counter(c));
   UEP_CUDA_TRY(cudaGetLastError());
+  count_launch(c);
   return UEP_OK;
 }
 
@@ -276,6 +247,7 @@ int launch_inverse(const Ctx* c, const int32_t* out_rank, const int32_t* out_off
   inverse_kernel<<<(c->S + 255) / 256, 256, 0, s>>>(out_rank, out_offset, plan.rank_base, c->S,
                                                    c->cfg.R, out_src);
   UEP_CUDA_TRY(cudaGetLastError());
+  count_launch(c);
   return UEP_OK;
 }
 

@@ -93,6 +93,7 @@ int launch_relay(const Ctx* c, const uep_plan_out& plan, int32_t* parent, int32_
   relay_kernel<<<1, 32, 0, s>>>(c->cfg.E, c->cfg.R, c->cfg.E + c->cfg.R * c->cfg.n_slot, plan.inst_off,
                                 plan.inst_rank, c->d_home, parent, send_volume);
   UEP_CUDA_TRY(cudaGetLastError());
+  count_launch(c);
   return UEP_OK;
 }
 

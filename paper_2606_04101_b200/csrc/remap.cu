@@ -188,6 +188,7 @@ int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool
       local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S, ws_packed(c, ws),
       ws_prefix(c, ws), chunk0);
   UEP_CUDA_TRY(cudaGetLastError());
+  count_launch(c);
   if (with_prefix) return launch_prefix(c, ws, s, local, /*pdl=*/true);
   return UEP_OK;
 }
@@ -208,6 +209,7 @@ int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local, bool pdl) 
   cfg.numAttrs = pdl ? 1 : 0;
   UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, prefix_kernel, ws_prefix(c, ws),
                                   local ? c->l_chunks : c->r_chunks, c->E_pad / 4));
+  count_launch(c);
   return UEP_OK;
 }
 
@@ -306,6 +308,7 @@ int launch_reroute(const Ctx* c, const uep_plan_out& plan, int32_t* n_inflight, 
                                                 plan.inst_off, plan.inst_rank, plan.inst_cum, cumq,
                                                 cumq + (size_t)c->cfg.R * inst_cap, n_inflight);
   UEP_CUDA_TRY(cudaGetLastError());
+  count_launch(c);
   return UEP_OK;
 }
 
@@ -355,8 +358,6 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   int2* stg = reinterpret_cast<int2*>(wtot + 36);     // staged {gate bits, out_gate index}, (expert, rank) order
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (blockIdx.x == 0 && threadIdx.x == 0) UEP_TL_SET(acc_clear, 6);
-  if (threadIdx.x == 0) UEP_TL_MAX(acc_clear, 15);     // latest CTA start
   const int c = LOCAL ? (int)blockIdx.x + chunk0 : (int)blockIdx.x;
   const bool local = LOCAL && cumq != nullptr;   // ranks local to (source rank, expert)
   const int grp = LOCAL ? c / cpg : 0, sub = LOCAL ? c % cpg : c;
@@ -385,10 +386,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   // ---- everything above is independent of the plan and of prefix_kernel (the packed ranks were
   // complete before prefix_kernel started): under programmatic dependent launch it overlaps the
   // planner (uep_balance) or prefix_kernel (uep_remap); now wait for them ------------------------
-  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 10);
   pdl_wait();
-  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 7);
-  if (tid == 0) UEP_TL_MAX(acc_clear, 18);
   // ---- chunk base ranks: row c of the exclusive prefix over chunks that prefix_kernel left.  Read
   // AFTER the wait, in the same L2 round trip as the plan below: under stream capture the lookup's
   // programmatic attribute makes its edge from prefix_kernel programmatic too, and only the wait
@@ -437,8 +435,6 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   }
   __syncthreads();
 
-  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 11);
-  if (tid == 0) UEP_TL_MAX(acc_clear, 16);
   int n_fly = 0;
   // two slots at a time: their records are loaded before any of them stores to shared memory
   // (the compiler cannot prove that the staging stores do not alias the records)
@@ -489,9 +485,6 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
       }
     }
   }
-  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 12);
-  if (tid == 0) UEP_TL_MAX(acc_clear, 17);
-  if (tid == kRemapThreads - 1) UEP_TL_MAX(acc_clear, 19);
   if (LOCAL && n_inflight) {                             // tokens of source rank grp that leave it
     n_fly = __reduce_add_sync(kFullMask, n_fly);
     if (lane == 0 && n_fly) atomicAdd(n_inflight + grp, n_fly);
@@ -509,12 +502,6 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
       }
     }
   }
-#ifdef UEP_TIMELINE
-  __syncthreads();
-  if (tid == 0) UEP_TL_MAX(acc_clear, 8);
-  if (blockIdx.x == 0 && tid == 0) UEP_TL_SET(acc_clear, 13);
-  if (blockIdx.x == gridDim.x - 1 && tid == 0) UEP_TL_SET(acc_clear, 14);
-#endif
 }
 
 template <typename GateT>
@@ -549,6 +536,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
                                   (const int32_t*)p.rank_base, out_replica, out_rank, out_offset,
                                   out_gate, local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S,
                                   cumq, srcpre, n_inflight, acc_clear, chunk0));
+  count_launch(c);
   return UEP_OK;
 }
 

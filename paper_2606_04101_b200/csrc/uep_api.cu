@@ -123,9 +123,7 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
     per = (per + 127) / 128 * 128;
     c->chunk_len = (int)per;
     c->n_chunks = (int)std::max<long long>(1, (S + per - 1) / per);
-    int reserve = 0;                                      // SMs left out of the remap grid's sizing
-    if (const char* v = getenv("UEP_REMAP_SM_RESERVE")) reserve = atoi(v);   // developer sweeps only
-    const int r_sms = std::max(1, c->sm_count - std::max(0, reserve));
+    const int r_sms = std::max(1, c->sm_count);
     long long rper = (S + 2 * r_sms - 1) / (2 * r_sms);
     rper = std::max<long long>(rper, kMinChunk);
     rper = (rper + kRemapThreads - 1) / kRemapThreads * kRemapThreads;
@@ -148,10 +146,6 @@ int uep_create(const uep_config* cfg, uep_ctx** out) {
   // pack / grad_reduce grid: one persistent streaming CTA per SM; the tiles are handed out
   // dynamically (profiles/r01_pack_grid.md: a static split is bound by the slowest SM)
   c->pack_ctas = c->sm_count;
-  if (const char* v = getenv("UEP_PACK_CTAS")) {        // developer sweeps only
-    const int n = atoi(v);
-    if (n >= 1 && n <= 16 * c->sm_count) c->pack_ctas = n;
-  }
 
   auto fail = [&](int rc) { uep_destroy(reinterpret_cast<uep_ctx*>(c)); return rc; };
   cudaError_t e;
@@ -250,6 +244,11 @@ int uep_get_launch_info(const uep_ctx* ctx, uep_launch_info* out) {
   out->r_chunk_len = c->r_chunk_len;
   out->plan_cluster = c->plan_cluster;
   return UEP_OK;
+}
+
+unsigned long long uep_launch_count(const uep_ctx* ctx) {
+  const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
+  return c ? __atomic_load_n(&const_cast<Ctx*>(c)->n_launches, __ATOMIC_RELAXED) : 0ull;
 }
 
 int uep_histogram(const uep_ctx* ctx, const int32_t* topk_ids, int32_t* expert_count, void* ws,
@@ -533,28 +532,45 @@ static int balance_impl(const uep_ctx* ctx, const int32_t* topk_ids, const void*
   // rank launched first 58.9 us, histogram first 54.5 us, rank made dependent on the histogram
   // 62.5 us (its CTAs then race the plan's cluster for SMs).  Re-measured with the planner
   // launched at high priority (chain 32.2 us): rank made dependent on the histogram 32.7 us.
-  UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
-  int rc2 = launch_histogram(c, topk_ids, expert_count, ws, s, /*red=*/true);
-  UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-  rc = launch_rank(c, topk_ids, ws, c->side);
-  UEP_CUDA_TRY(cudaEventRecord(c->ev_rank, c->side));
+  // From the first event record on, every failure goes through `fail`: the side stream is joined
+  // back into `stream` (a capture stays valid and ends with no un-joined fork) and the histogram's
+  // accumulator, which only a completed chain leaves zero, is cleared.
+  cudaError_t ce = cudaSuccess;
+  bool forked = false;
+  rc = UEP_OK;
+#define UEP_BAL_TRY(expr) do { if (rc == UEP_OK && ce == cudaSuccess) ce = (expr); } while (0)
+#define UEP_BAL_RC(expr) do { if (rc == UEP_OK && ce == cudaSuccess) rc = (expr); } while (0)
+  UEP_BAL_TRY(cudaEventRecord(c->ev_fork, s));
+  UEP_BAL_RC(launch_histogram(c, topk_ids, expert_count, ws, s, /*red=*/true));
+  UEP_BAL_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+  forked = (rc == UEP_OK && ce == cudaSuccess);
+  UEP_BAL_RC(launch_rank(c, topk_ids, ws, c->side));
+  UEP_BAL_TRY(cudaEventRecord(c->ev_rank, c->side));
   // planner and lookup are launched programmatically dependent on their predecessor: their
-  // prologues (static layout; packed ranks, gates, prefix rows) overlap it
-  if (rc2 == UEP_OK) rc2 = launch_plan(c, expert_count, *plan, s, /*pdl=*/true, 1, ws_acc(ws), expert_count);
+  // prologues (static layout; packed ranks, gates) overlap it
+  UEP_BAL_RC(launch_plan(c, expert_count, *plan, s, /*pdl=*/true, 1, ws_acc(ws), expert_count));
   const bool do_pack = n_tensors > 0 && c->cfg.n_slot > 0;
-  if (do_pack && rc2 == UEP_OK) {   // pack depends only on the plan and overlaps the lookup (Eq. 1)
-    UEP_CUDA_TRY(cudaEventRecord(c->ev_fork, s));
-    UEP_CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-    int rc3 = launch_pack(c, *plan, a, c->side);
-    if (rc == UEP_OK) rc = rc3;
+  if (do_pack) {   // pack depends only on the plan and overlaps the lookup (Eq. 1)
+    UEP_BAL_TRY(cudaEventRecord(c->ev_fork, s));
+    UEP_BAL_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+    UEP_BAL_RC(launch_pack(c, *plan, a, c->side));
   }
-  UEP_CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
-  UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_rank, 0));          // join the rank kernel
-  if (rc == UEP_OK && rc2 == UEP_OK)
-    rc2 = launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s, /*pdl=*/true,
-                        false, nullptr, ws_acc(ws));
-  if (join_pack) UEP_CUDA_TRY(cudaStreamWaitEvent(s, c->ev_join, 0));   // join the side stream (pack)
-  return rc != UEP_OK ? rc : rc2;
+  UEP_BAL_TRY(cudaEventRecord(c->ev_join, c->side));
+  UEP_BAL_TRY(cudaStreamWaitEvent(s, c->ev_rank, 0));          // join the rank kernel
+  UEP_BAL_RC(launch_lookup(c, gate, *plan, out_replica, out_rank, out_offset, out_gate, ws, s, /*pdl=*/true,
+                           false, nullptr, ws_acc(ws)));
+  if (join_pack) UEP_BAL_TRY(cudaStreamWaitEvent(s, c->ev_join, 0));   // join the side stream (pack)
+#undef UEP_BAL_TRY
+#undef UEP_BAL_RC
+  if (rc == UEP_OK && ce == cudaSuccess) return UEP_OK;
+  // ---- failure: join whatever was forked, leave the workspace reusable -----------------------------
+  if (ce != cudaSuccess) rc = set_cuda_error(ce);
+  if (forked) {
+    if (cudaEventRecord(c->ev_join, c->side) == cudaSuccess) cudaStreamWaitEvent(s, c->ev_join, 0);
+  }
+  cudaMemsetAsync(ws_acc(ws), 0, sizeof(int32_t) * UEP_MAX_E, s);    // a half-run chain may have left counts there
+  cudaGetLastError();
+  return rc;
 }
 
 extern "C" {

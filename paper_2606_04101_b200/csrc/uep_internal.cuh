@@ -51,6 +51,7 @@ struct Ctx {
   // robin, so up to kCtrSlots such kernels of one context may be in flight at a time
   unsigned* d_ctr;
   unsigned ctr_next;      // host, advanced atomically
+  unsigned long long n_launches;   // host, advanced atomically: kernels launched through this context
   // fork/join for uep_balance
   cudaStream_t side;
   cudaEvent_t ev_fork, ev_join, ev_rank;
@@ -58,6 +59,10 @@ struct Ctx {
 
 constexpr int kCtrSlots = 64;
 unsigned* next_counter(const Ctx* c);     // the next {unit, done} counter pair (thread-safe)
+// every launch_* below reports its kernel launches here (uep_launch_count; the bench's gpu_launches)
+inline void count_launch(const Ctx* c, int n = 1) {
+  __atomic_fetch_add(&const_cast<Ctx*>(c)->n_launches, (unsigned long long)n, __ATOMIC_RELAXED);
+}
 
 struct PackArgs {
   const unsigned char* src[UEP_MAX_TENSORS];
@@ -109,24 +114,47 @@ int init_hist_kernels();
 // kernel).  pdl_wait: block until the preceding kernel has completed and its writes are visible;
 // a no-op when the kernel was launched normally.
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-// Developer probe (-DUEP_TIMELINE): kernels of uep_balance stamp %globaltimer into the 256 reserved
-// bytes at the head of the workspace (32 slots; `acc` points just behind them).  Slots: 0 hist CTA 0
-// start, 1 hist end (max over CTAs), 2 plan CTA 0 start, 3 plan after the wait, 4 plan bisection
-// done, 5 plan end, 6 lookup CTA 0 start, 7 lookup CTA 0 after the wait, 8 lookup end (max over
-// CTAs), 9 the previous call's lookup end.
-#ifdef UEP_TIMELINE
-__device__ __forceinline__ unsigned long long tl_now() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-  return t;
-}
-#define UEP_TL_SET(acc, i) do { if (acc) reinterpret_cast<unsigned long long*>(const_cast<int32_t*>(acc))[(i) - 32] = tl_now(); } while (0)
-#define UEP_TL_MAX(acc, i) do { if (acc) atomicMax(reinterpret_cast<unsigned long long*>(const_cast<int32_t*>(acc)) + ((i) - 32), tl_now()); } while (0)
-#else
-#define UEP_TL_SET(acc, i)
-#define UEP_TL_MAX(acc, i)
-#endif
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// ---- mbarrier + bulk-copy (TMA engine, 1-D cp.async.bulk) wrappers shared by the streaming kernels
+// (pack.cu, reduce.cu) and the histogram's chunk staging (hist.cu) ---------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "MBAR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra MBAR_DONE;\n"
+      "bra MBAR_WAIT;\n"
+      "MBAR_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// global -> shared, completion counted in bytes on an mbarrier
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// shared -> global, tracked by the thread's bulk async-group
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src_smem)),
+               "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 #endif
 
 inline int32_t* ws_table(void* ws) {

@@ -215,7 +215,7 @@ def test_multi_tensor_pack_training_state():
     assert_parity(g, o, ids, None, states)
 
 
-@pytest.mark.parametrize("name,s", [("glm_air", 0.6), ("glm_air", 1.4), ("dsv3_prefill", 1.0)])
+@pytest.mark.parametrize("name,s", [("glm_air", 0.6), ("glm_air", 1.0), ("glm_air", 1.4), ("dsv3_prefill", 1.0)])
 def test_full_size_configs_bit_exact(name, s):
     """BASELINE configs 1 and 2 at full size, in the launch configuration bench.py times
     (uep_balance): every integer output against the oracle, element by element."""
@@ -950,3 +950,158 @@ def test_histogram_accumulator_stays_clean_between_calls():
     ctx.uep_histogram(d_ids[0], counts[0], ws)
     torch.cuda.synchronize()
     assert int(counts[0].sum()) == T * k
+
+
+def _fullsize_plan(ctx, c, seed, zipf_s=1.0):
+    """ids of one full-size instance on the device, and the ORACLE's plan for them."""
+    ids = synth.zipf_topk_ids(c["T"], c["k"], c["E"], zipf_s, seed, device=DEV)
+    lam, _ = oracle.histogram(ids.cpu().numpy(), c["E"])
+    p = oracle.plan(lam, c["R"], c["n_slot"], c["u_min"], S_total=c["T"] * c["k"])
+    assert p.n_replicas > 8
+    return ids, lam, p
+
+
+def test_pack_at_the_benchmarked_byte_size():
+    """uep_pack at the size bench.py times (dsv3_prefill: 88 080 384 B per expert, 22.5 GB of source,
+    11.3 GB of slot buffers: byte offsets beyond 4 GiB, 5376 tiles per expert), once through
+    uep_balance (the timed launch configuration) and once through uep_pack on another plan.  Compared
+    on the device, slot by slot (BASELINE.md §5 allows the chunk-wise compare): every destination
+    slot equals the source expert that the ORACLE's slot_expert names, byte for byte, and every empty
+    slot still holds the sentinel ("remains empty"; weight distribution PAPER.md:162)."""
+    c = synth.CONFIGS["dsv3_prefill"]
+    T, k, E, R, ns, um = c["T"], c["k"], c["E"], c["R"], c["n_slot"], c["u_min"]
+    elems = c["state"][0][1]
+    assert elems * 2 == 88080384
+    ctx = binding.Context(T, k, E, R, ns, um)
+    ws, plan = ctx.new_workspace(), ctx.new_plan()
+    src = synth.expert_state(E, elems, 7, dtype=torch.bfloat16, device=DEV)
+    assert src.numel() * 2 > (1 << 34)                              # > 16 GiB: 64-bit offsets matter
+    dst = torch.empty((R, ns, elems), dtype=torch.bfloat16, device=DEV)
+    SENT = 0x5A5B
+    for seed, through_balance in ((4242, True), (4243, False)):
+        ids, lam, p = _fullsize_plan(ctx, c, seed)
+        dst.view(torch.int16).fill_(SENT)
+        count = torch.zeros(E, dtype=torch.int32, device=DEV)
+        gate = synth.gates_uniform_renorm(T, k, 6, device=DEV)
+        rep, rnk, off, og = ctx.new_outputs(gate)
+        if through_balance:
+            ctx.uep_balance(ids, gate, count, plan, rep, rnk, off, og, [src], [dst], ws)
+        else:
+            ctx.uep_histogram(ids, count, ws)
+            ctx.uep_plan(count, plan, ws)
+            ctx.uep_pack(plan, [src], [dst])
+        torch.cuda.synchronize()
+        assert np.array_equal(plan.host().slot_expert, p.slot_expert)
+        n_used = 0
+        for t in range(R):
+            for q in range(ns):
+                e = int(p.slot_expert[t, q])
+                if e >= 0:
+                    n_used += 1
+                    assert torch.equal(dst[t, q].view(torch.int16), src[e].view(torch.int16)), (t, q, e)
+                else:
+                    assert bool((dst[t, q].view(torch.int16) == SENT).all()), (t, q)
+        assert n_used == p.n_replicas
+
+
+def test_grad_reduce_at_the_benchmarked_byte_size():
+    """uep_grad_reduce over fp32 [E, 7168 x 2048] main gradients (15 GB) and [R, n_slot, 7168 x 2048]
+    slot gradients (7.5 GB) — the size bench.py times.  On the device, expert by
+    expert as the ORACLE's plan names them: main = the sequential fp32 sum in instance order (bit for
+    bit), used slots zero, empty slots and unreplicated experts untouched; and on 4096 sampled
+    columns the fp64 oracle O-5 within n_terms x 2^-24 x sum|terms|."""
+    c = synth.CONFIGS["dsv3_prefill"]
+    T, k, E, R, ns, um = c["T"], c["k"], c["E"], c["R"], c["n_slot"], c["u_min"]
+    B = 7168 * 2048
+    ctx = binding.Context(T, k, E, R, ns, um, gate_dtype=binding.GATE_NONE)
+    ws, plan = ctx.new_workspace(), ctx.new_plan()
+    ids, lam, p = _fullsize_plan(ctx, c, 99)
+    count = torch.zeros(E, dtype=torch.int32, device=DEV)
+    ctx.uep_histogram(ids, count, ws)
+    ctx.uep_plan(count, plan, ws)
+    main0 = synth.expert_state(E, B, 21, dtype=torch.float32, device=DEV, std=1.0)
+    slot0 = synth.expert_state(R * ns, B, 22, dtype=torch.float32, device=DEV, std=1.0).view(R, ns, B)
+    main, slot = main0.clone(), slot0.clone()
+    ctx.uep_grad_reduce(plan, [main], [slot])
+    torch.cuda.synchronize()
+    assert np.array_equal(plan.host().inst_rank, p.inst_rank)
+    used = np.zeros((R, ns), dtype=bool)
+    for e in range(E):
+        exp = main0[e]
+        lo, hi = int(p.inst_off[e]), int(p.inst_off[e + 1])
+        for i in range(lo + 1, hi):                                   # instance order (S11)
+            t, q = int(p.inst_rank[i]), int(p.inst_phys[i]) - p.M
+            exp = exp + slot0[t, q]
+            used[t, q] = True
+        assert torch.equal(main[e], exp), e
+    assert used.sum() == p.n_replicas and np.array_equal(used, p.slot_expert >= 0)
+    for t in range(R):
+        for q in range(ns):
+            if used[t, q]:
+                assert not bool(slot[t, q].any()), (t, q)             # cleared in place
+            else:
+                assert torch.equal(slot[t, q], slot0[t, q]), (t, q)   # empty slots untouched
+    # fp64 oracle on sampled columns (incl. the first and last element of the tensor)
+    g = torch.Generator().manual_seed(1)
+    cols = torch.cat([torch.tensor([0, B - 1]), torch.randint(0, B, (4094,), generator=g)]).to(DEV)
+    m_s, s_s = main0[:, cols].cpu().numpy(), slot0[:, :, cols].cpu().numpy()
+    m64, s_ref = oracle.grad_reduce(p, m_s, s_s)
+    got = main[:, cols].cpu().numpy()
+    mag, nterm = np.abs(m_s).astype(np.float64), np.ones(E)
+    for t in range(R):
+        for q in range(ns):
+            e = int(p.slot_expert[t, q])
+            if e >= 0:
+                mag[e] += np.abs(s_s[t, q]); nterm[e] += 1
+    assert (np.abs(got - m64) <= (nterm[:, None] * 2.0 ** -24) * mag + 1e-30).all()
+    assert np.array_equal(slot[:, :, cols].cpu().numpy(), s_ref)
+
+
+def test_balance_failure_mid_chain_leaves_stream_and_workspace_usable():
+    """A stage that fails to launch part-way through uep_balance (here: uep_pack refuses a tensor
+    with more tiles than its unit counter can index, after histogram, rank and plan were enqueued)
+    must still join the internal side stream back into the caller's stream — inside a stream capture
+    too, which has to end cleanly — and must leave the workspace's accumulator clean, so that the
+    next call on the same workspace publishes exact counts."""
+    import ctypes
+    T, k, E, R, ns, um = 16384, 4, 64, 16, 2, 64
+    ctx = binding.Context(T, k, E, R, ns, um, gate_dtype=binding.GATE_NONE)
+    ws, plan = ctx.new_workspace(), ctx.new_plan()
+    ids = synth.zipf_topk_ids(T, k, E, 1.3, 3)
+    d_ids = ids.to(DEV)
+    count = torch.zeros(E, dtype=torch.int32, device=DEV)
+    rep, rnk, off, _ = ctx.new_outputs(None)
+    src = torch.zeros((E, 16), dtype=torch.uint8, device=DEV)
+    dst = torch.zeros((R, ns, 16), dtype=torch.uint8, device=DEV)
+    L = binding.lib()
+
+    def bad_call(stream):
+        srcs = (ctypes.c_void_p * 1)(src.data_ptr())
+        dsts = (ctypes.c_void_p * 1)(dst.data_ptr())
+        bpe = (ctypes.c_size_t * 1)(1 << 46)             # 2^32 tiles per expert: launch_pack refuses
+        return L.uep_balance(ctx._h, ctypes.c_void_p(d_ids.data_ptr()), None, ctypes.c_void_p(count.data_ptr()),
+                             ctypes.byref(plan.c), ctypes.c_void_p(rep.data_ptr()), ctypes.c_void_p(rnk.data_ptr()),
+                             ctypes.c_void_p(off.data_ptr()), None, 1, srcs, bpe, dsts,
+                             ctypes.c_void_p(ws.data_ptr()), ctypes.c_void_p(stream.cuda_stream))
+
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    assert bad_call(st) == -2                             # UEP_ERR_UNSUPPORTED, eager
+    torch.cuda.synchronize()
+    lam, _ = oracle.histogram(ids.numpy(), E)
+    with torch.cuda.stream(st):
+        ctx.uep_balance(d_ids, None, count, plan, rep, rnk, off, None, [], [], ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(count.cpu().numpy(), lam)       # not doubled by the aborted call
+    g = torch.cuda.CUDAGraph()                            # the same inside a capture
+    with torch.cuda.stream(st):
+        with torch.cuda.graph(g, stream=st):
+            assert bad_call(st) == -2
+            ctx.uep_balance(d_ids, None, count, plan, rep, rnk, off, None, [], [], ws)
+    count.fill_(-1)
+    for _ in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(count.cpu().numpy(), lam)
+    o = oracle_chain(ids, None, E, R, ns, um)
+    assert np.array_equal(rep.cpu().numpy(), o[2]) and np.array_equal(off.cpu().numpy(), o[4])
