@@ -36,29 +36,37 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr int kMaxLog = UEP_MAX_R * UEP_MAX_NSLOT;      // 1024 accepted transfers at most
 constexpr int kPlanWarps = kPlanThreads / 32;
 constexpr int kLogPer = kMaxLog / kPlanThreads;        // log entries handled per thread when emitting
-static_assert(kLogPer * kPlanThreads == kMaxLog && UEP_MAX_E <= kPlanThreads && UEP_MAX_R < kPlanThreads, "plan emit");
-static_assert(kPlanThreads == 512, "rank order: threads per rank derived from 2^9");
+constexpr int kEPer = UEP_MAX_E / kPlanThreads;        // experts per thread in the emit scan (blocked)
+static_assert(kLogPer * kPlanThreads == kMaxLog && kEPer * kPlanThreads == UEP_MAX_E &&
+              UEP_MAX_R <= kPlanThreads, "plan setup / emit: one thread per rank, kEPer experts per thread");
+constexpr int kPlanLog2 = kPlanThreads == 512 ? 9 : 8;
+static_assert(kPlanThreads == (1 << kPlanLog2), "rank order: threads per rank derived from log2(kPlanThreads)");
 // CTAs (SMs) sharing one solve, so that the 63 probes of a round spread over many schedulers:
-// 8 CTAs = two probes per scheduler.  Measured on B200 (DSV3 shape): 4 / 8 / 16 CTAs give
-// 22.9 / 20.6 / 20.4 us of bisection, i.e. from 8 up the probes are bound by the latency of their
-// own dependent chain, not by issue slots, so the portable size 8 is the default
-// (UEP_PLAN_CLUSTER overrides; 16 needs the non-portable opt-in, set in init_plan_kernels).
+// 8 CTAs x 8 warps = one probe per warp, two per scheduler.  Measured on B200 (DSV3 shape): 4 / 8 /
+// 16 CTAs give 22.9 / 20.6 / 20.4 us of bisection, i.e. from 8 up the probes are bound by the
+// latency of their own dependent chain, not by issue slots, so the portable size 8 is used.
+// A CTA has 16 warps, 8 of which probe: at ~96 registers per thread it takes 48 K of an SM's
+// registers, which is deliberate — no rank_kernel / lookup_kernel CTA fits beside it, and a probe
+// sharing its SM with 16-32 streaming warps runs far slower (measured: a 256-thread, 24 K-register
+// version that co-resided with the rank kernel made the chain 5 us slower, 32.5 -> 37.5 us).
+constexpr int kWalkWarp = kPlanWarps > 8 ? 8 : 0;   // first warp without a probe (8 probing warps per CTA)
 constexpr int kPlanMaxNodes = 64;     // 2^6: six bisection levels speculated per round with 8 CTAs
 constexpr int kPcSmem = 2048;                           // phys_count staged in smem if R*P fits
 
 struct PlanSmem {
   int lam[UEP_MAX_E];
-  int elist[UEP_MAX_E];        // experts grouped by home rank, each group by lambda desc, id asc
+  int rexp[UEP_MAX_E];         // experts grouped by home rank, ascending id (static layout)
   int home[UEP_MAX_E];
   int main_phys[UEP_MAX_E];
+  int wpos[UEP_MAX_E];         // position of e among its home rank's experts in visit order
   int u_main[UEP_MAX_E];
   int n_rep[UEP_MAX_E];
   int first[UEP_MAX_E];
   int inst_off[UEP_MAX_E + 1];
   int ell[UEP_MAX_R];
-  int order[UEP_MAX_R];        // ranks by l_r desc, id asc
-  int roff[UEP_MAX_R + 1];
   int rload[UEP_MAX_R];
+  int rpos[UEP_MAX_R];         // visit position of rank r (ranks by l_r desc, id asc)
+  int roff[UEP_MAX_R + 1];
   // (padded: the probe reads one entry ahead of the one it is working on)
   int s_ell[UEP_MAX_R + 1];    // l_r in visit order
   int v_off[UEP_MAX_R + 2];    // CSR of the flat visit list: experts of the oi-th visited rank
@@ -68,12 +76,9 @@ struct PlanSmem {
   int log_n[2][kPlanMaxNodes]; // accepted transfers of the probe at each tree node (per round parity)
   int node_feas[2][kPlanMaxNodes];   // probe verdict per tree node, written by its owner to every CTA
   int pc[kPcSmem];
-  int warp_tmp[32];
-  unsigned long long scan_tmp[32];
-  int feas[32];
-  int lo, hi, n_probes, n_log, log_buf;
-  long long s_valid;
-  int max_ell;
+  int red_fan[kPlanWarps], red_grp[kPlanWarps];
+  unsigned long long scan_tmp[kPlanWarps];
+  int lo, hi, n_probes, n_log, log_buf, lo0, hi0, s_valid;
 };
 
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
@@ -85,24 +90,8 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
   return v;
 }
 
-// Block-wide inclusive scan of one value per thread (kPlanThreads). tmp: 32 ints of smem.
-__device__ __forceinline__ int block_incl_scan(int v, int* tmp) {
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  int s = warp_incl_scan(v, lane);
-  __syncthreads();
-  if (lane == 31) tmp[w] = s;
-  __syncthreads();
-  if (w == 0) {
-    int t = tmp[lane];
-    t = warp_incl_scan(t, lane);
-    tmp[lane] = t;
-  }
-  __syncthreads();
-  if (w > 0) s += tmp[w - 1];
-  return s;
-}
-
-// The same for a 64-bit value (two packed 32-bit sums).  tmp: 32 x 8 bytes of smem.
+// Block-wide inclusive scan of one 64-bit value per thread (two packed 32-bit sums), ONE barrier:
+// every warp scans the kPlanWarps warp totals itself.  tmp must not be in use by another scan.
 __device__ __forceinline__ unsigned long long block_incl_scan64(unsigned long long v, unsigned long long* tmp) {
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   unsigned long long s = v;
@@ -111,21 +100,16 @@ __device__ __forceinline__ unsigned long long block_incl_scan64(unsigned long lo
     const unsigned long long y = __shfl_up_sync(kFull, s, o);
     if (lane >= o) s += y;
   }
-  __syncthreads();
   if (lane == 31) tmp[w] = s;
   __syncthreads();
-  if (w == 0) {
-    unsigned long long t = (lane < kPlanWarps) ? tmp[lane] : 0ull;
+  unsigned long long t = (lane < kPlanWarps) ? tmp[lane] : 0ull;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const unsigned long long y = __shfl_up_sync(kFull, t, o);
-      if (lane >= o) t += y;
-    }
-    tmp[lane] = t;
+  for (int o = 1; o < kPlanWarps; o <<= 1) {
+    const unsigned long long y = __shfl_up_sync(kFull, t, o);
+    if (lane >= o) t += y;
   }
-  __syncthreads();
-  if (w > 0) s += tmp[w - 1];
-  return s;
+  const unsigned long long pre = __shfl_sync(kFull, t, (w + 31) & 31);     // total of the warps before w
+  return w > 0 ? s + pre : s;
 }
 
 // One greedy feasibility probe (Alg. 1 lines 6-20) by one warp.  All control flow is
@@ -134,6 +118,9 @@ __device__ __forceinline__ unsigned long long block_incl_scan64(unsigned long lo
 // visit list (s_ell / v_off / v_lam, sorted once per solve), the owner of the arg-max is the lane
 // whose key equals the reduced key (keys are unique: they carry the rank id), and its new key is
 // the old one minus delta << 8.  LOG: also record the accepted transfers {e, t, slot, delta}.
+// (Measured and dropped: keeping the top TWO keys so that the next arg-max is known without a
+// reduction on the chain — the warp issues in order and ptxas consumes the reduction's uniform
+// register right behind the CREDUX, so nothing overlaps: plan 15.1 -> 18.6 us.)
 template <int RPL, bool LOG>
 __device__ __forceinline__ bool probe(const PlanSmem& sm, const int tau, const int R,
                                       const int n_slot, const int u_min, const bool strict,
@@ -206,10 +193,10 @@ __device__ __forceinline__ bool probe(const PlanSmem& sm, const int tau, const i
   return true;
 }
 
-// LOWREG (uep_plan_batched): two CTAs per SM at 64 registers — a single solve is slower that way
-// (16.5 against 15.4 us), many solves at once are faster (1.13 against 1.52 us per layer for 32)
+// LOWREG (uep_plan_batched): up to four CTAs per SM at 64 registers — a single solve is slower
+// that way, many solves at once are faster
 template <int RPL, bool LOWREG>
-__global__ void __launch_bounds__(kPlanThreads, LOWREG ? 2 : 1)
+__global__ void __launch_bounds__(kPlanThreads, LOWREG ? (1024 / kPlanThreads) : 1)
 plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict__ g_home,
             const int32_t* __restrict__ g_main_phys, const int32_t* __restrict__ g_roff,
             const int32_t* __restrict__ g_rexp, uep_plan_out out, int E, int R, int n_slot, int M,
@@ -236,120 +223,110 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   // touch both ends of the parameter block now: the emit phase reads the plan's pointers on the
   // critical path, and a cold constant-cache line there costs several hundred cycles
   if (out.slot_expert == nullptr || out.scalars == nullptr || count_out == reinterpret_cast<int32_t*>(1)) return;
-  // ---- stage inputs ---------------------------------------------------------------------
+  // ---- setup, three barrier-separated phases after the wait -----------------------------------
   pdl_trigger();                   // the lookup kernel may start its plan-independent prologue
-  if (tid < E) {                   // static layout first: it does not depend on the histogram
-    sm.home[tid] = g_home[tid];
-    sm.main_phys[tid] = g_main_phys[tid];
-    sm.elist[tid] = g_rexp[tid];
+  // static layout first: it does not depend on the histogram (overlaps it under programmatic launch)
+  for (int e = tid; e < E; e += kPlanThreads) {
+    sm.home[e] = g_home[e];
+    sm.main_phys[e] = g_main_phys[e];
+    sm.rexp[e] = g_rexp[e];
   }
-  if (tid <= R) sm.roff[tid] = g_roff[tid];
+  for (int r = tid; r <= R; r += kPlanThreads) sm.roff[r] = g_roff[r];
+  __syncthreads();
   pdl_wait();                      // the histogram (preceding kernel) is complete
-  if (tid < E) sm.lam[tid] = acc ? __ldcg(acc + tid) : expert_count[tid];
-  __syncthreads();
-  // line 2: l_r
-  if (tid < R) {
-    int s = 0;
-    for (int i = sm.roff[tid]; i < sm.roff[tid + 1]; ++i) s += sm.lam[sm.elist[i]];
-    sm.ell[tid] = s;
-  }
-  __syncthreads();
-  // sum and max of l_r (R <= 256 -> first 8 warps)
+  // phase 1: lambda_e into shared memory, and line 2 (l_r) straight from global memory with
+  // independent loads (thread r sums its own experts: no barrier between lambda and l_r)
   {
-    int v = (tid < R) ? sm.ell[tid] : 0;
-    int sum = __reduce_add_sync(kFull, v);
-    int mx = __reduce_max_sync(kFull, v);
-    if (lane == 0) { sm.warp_tmp[warp] = sum; sm.feas[warp] = mx; }
-  }
-  __syncthreads();
-  if (warp == kPlanWarps - 1) {    // (the last warp has no expert to order below when E < kPlanThreads)
-    // per-warp partials -> totals with two warp reductions (S < 2^31: 32-bit sums are exact)
-    const int ps = (lane < kPlanWarps) ? sm.warp_tmp[lane] : 0;
-    const int pm = (lane < kPlanWarps) ? sm.feas[lane] : 0;
-    const unsigned sv = (unsigned)__reduce_add_sync(kFull, ps);
-    const int mx = __reduce_max_sync(kFull, pm);
-    if (lane == 0) {
-      sm.s_valid = (long long)sv;
-      sm.max_ell = mx;
-      // line 3 (S3): tau_lo = floor(beta * ceil(mean)), tau_hi = max l_r.  32-bit divisions where the
-      // operands fit (a 64-bit division is a ~300-cycle subroutine on this dependent path)
-      const unsigned mean_ceil = (sv + (unsigned)R - 1u) / (unsigned)R;
-      const unsigned long long prod = (unsigned long long)mean_ceil * (unsigned long long)beta_num;
-      const unsigned long long tl = (prod >> 32) == 0ull ? (unsigned long long)((unsigned)prod / (unsigned)beta_den)
-                                                         : prod / (unsigned long long)beta_den;
-      sm.lo = (int)min(tl, (unsigned long long)0x7fffffff);
-      sm.hi = mx;
-      sm.n_probes = 0;
-      sm.n_log = 0;
+    const int32_t* lam_g = acc ? acc + 0 : expert_count;
+    for (int e = tid; e < E; e += kPlanThreads) sm.lam[e] = __ldcg(lam_g + e);
+    if (tid < R) {
+      int s = 0;
+      const int a = sm.roff[tid], b = sm.roff[tid + 1];
+#pragma unroll 4
+      for (int i = a; i < b; ++i) s += __ldcg(lam_g + sm.rexp[i]);
+      sm.ell[tid] = s;
     }
   }
-  // rank order: position = number of ranks that come before (l desc, id asc).  gsz threads per
-  // rank (a power of two, all of the CTA's threads when R allows), each counting over a strided
-  // part of the ranks with independent loads, then a shuffle reduction inside the group.  (A warp
-  // per rank with a warp reduction each cost 500 cycles per rank, four ranks per warp in a row.)
+  __syncthreads();
+  // phase 2.  Every warp reduces the l_r itself (no second barrier for the bounds):
+  // line 3 (S3): tau_lo = floor(beta * ceil(mean)), tau_hi = max l_r; S < 2^24, so 32-bit sums are
+  // exact, and 32-bit divisions where the operands fit (a 64-bit division is a ~300-cycle
+  // subroutine on this dependent path)
   {
-    const int gsh = min(5, 9 - (32 - __clz(R - 1)));           // kPlanThreads = 2^9 >= R << gsh
+    int sum = 0, mx = 0;
+    for (int r = lane; r < R; r += 32) { const int v = sm.ell[r]; sum += v; mx = max(mx, v); }
+    sum = __reduce_add_sync(kFull, sum);
+    mx = __reduce_max_sync(kFull, mx);
+    const unsigned mean_ceil = ((unsigned)sum + (unsigned)R - 1u) / (unsigned)R;
+    const unsigned long long prod = (unsigned long long)mean_ceil * (unsigned long long)beta_num;
+    const unsigned long long tl = (prod >> 32) == 0ull ? (unsigned long long)((unsigned)prod / (unsigned)beta_den)
+                                                       : prod / (unsigned long long)beta_den;
+    if (tid == 0) {
+      sm.lo = sm.lo0 = (int)min(tl, (unsigned long long)0x7fffffff);
+      sm.hi = sm.hi0 = mx;
+      sm.s_valid = sum;
+      sm.n_probes = 0; sm.n_log = 0; sm.log_buf = -1;
+    }
+  }
+  // rank order (S5): visit position of rank r = number of ranks that come before it (l desc, id
+  // asc), and in the same pass the start of its experts in the flat visit list = number of experts
+  // of those ranks (no scan).  gsz threads per rank (a power of two), each over a strided part of
+  // the ranks with independent loads, then a shuffle reduction inside the group.
+  {
+    const int gsh = min(5, kPlanLog2 - (32 - __clz(R - 1)));   // kPlanThreads >= R << gsh
     const int gsz = 1 << gsh, r = tid >> gsh, sub = tid & (gsz - 1);
-    int cnt = 0;
+    int cnt = 0, off = 0, lr = 0;
     if (r < R) {
-      const int lr = sm.ell[r];
+      lr = sm.ell[r];
 #pragma unroll 4
       for (int q = sub; q < R; q += gsz) {
         const int lq = sm.ell[q];
-        cnt += (lq > lr || (lq == lr && q < r)) ? 1 : 0;
+        const bool before = lq > lr || (lq == lr && q < r);
+        cnt += before ? 1 : 0;
+        off += before ? sm.roff[q + 1] - sm.roff[q] : 0;
       }
     }
-    for (int o = gsz >> 1; o > 0; o >>= 1) cnt += __shfl_xor_sync(kFull, cnt, o);
-    if (r < R && sub == 0) sm.order[cnt] = r;
+    for (int o = gsz >> 1; o > 0; o >>= 1) {
+      cnt += __shfl_xor_sync(kFull, cnt, o);
+      off += __shfl_xor_sync(kFull, off, o);
+    }
+    if (r < R && sub == 0) { sm.rpos[r] = cnt; sm.s_ell[cnt] = lr; sm.v_off[cnt] = off; }
+    if (tid == 0) { sm.s_ell[R] = 0; sm.v_off[R] = E; sm.v_off[R + 1] = E; }    // read-ahead padding
   }
-  if (tid < E) {
-    // per-rank expert order: lambda desc, id asc; a thread per expert counts the experts of its
-    // home rank that come before it; positions into u_main (temp)
-    const int e = tid, h = sm.home[e], le = sm.lam[e];
+  // per-rank expert order (S5): lambda desc, id asc; a thread per expert counts the experts of its
+  // home rank that come before it
+  for (int e = tid; e < E; e += kPlanThreads) {
+    const int h = sm.home[e], le = sm.lam[e];
     const int a = sm.roff[h], b = sm.roff[h + 1];
     int cnt = 0;
 #pragma unroll 4
     for (int i = a; i < b; ++i) {
-      const int q = sm.elist[i];
+      const int q = sm.rexp[i];
       const int lq = sm.lam[q];
       cnt += (lq > le || (lq == le && q < e)) ? 1 : 0;
     }
-    sm.u_main[e] = a + cnt;
+    sm.wpos[e] = cnt;
   }
   __syncthreads();
-  if (tid < E) sm.elist[sm.u_main[tid]] = tid;
-  __syncthreads();
-  // flat visit list: ranks in visit order, each with its experts in visit order (S5)
-  {
-    const int r = (tid < R) ? sm.order[tid] : 0;
-    const int cnt = (tid < R) ? (sm.roff[r + 1] - sm.roff[r]) : 0;
-    const int inc = block_incl_scan(cnt, sm.warp_tmp);
-    if (tid < R) {
-      sm.s_ell[tid] = sm.ell[r];
-      sm.v_off[tid] = inc - cnt;
-      if (tid == R - 1) sm.v_off[R] = inc;
-      const int src = sm.roff[r];
-      for (int q = 0; q < cnt; ++q) {
-        const int e = sm.elist[src + q];
-        sm.v_e[inc - cnt + q] = e;
-        sm.v_lam[inc - cnt + q] = sm.lam[e];
-      }
-    }
-    if (tid == 0) sm.log_buf = -1;
-    if (tid < 2 * kPlanMaxNodes) (&sm.node_feas[0][0])[tid] = 0;    // an unprobed slot never reads as a verdict
-    // emit state, cleared here (off the path between the last probe and the plan's first store;
-    // no probe touches it): per-expert replica counts, first log entry, staged phys_count, and by
-    // CTA 0 the slot map in global memory (the emitting CTA writes it after a cluster barrier, or
-    // is CTA 0 itself when no round runs)
-    if (tid < E) { sm.u_main[tid] = sm.lam[tid]; sm.n_rep[tid] = 0; sm.first[tid] = 0x7fffffff; }
-    if (R * P <= kPcSmem) for (int i = tid; i < R * P; i += kPlanThreads) sm.pc[i] = 0;
-    if (crank == 0) {
-      int32_t* se = out.slot_expert + (size_t)batch_b * max(1, R * n_slot);
-      for (int i = tid; i < R * n_slot; i += kPlanThreads) se[i] = -1;
-    }
+  // phase 3: flat visit list (ranks in visit order, each with its experts in visit order), and the
+  // emit state cleared here, off the path between the last probe and the plan's first store (no
+  // probe touches it): per-expert replica counts, first log entry, staged phys_count, and by CTA 0
+  // the slot map in global memory (the emitting CTA writes it after a cluster
+  // barrier, or is CTA 0 itself when no round runs)
+  for (int e = tid; e < E; e += kPlanThreads) {
+    const int le = sm.lam[e];
+    const int p = sm.v_off[sm.rpos[sm.home[e]]] + sm.wpos[e];
+    sm.v_e[p] = e;
+    sm.v_lam[p] = le;
+    sm.u_main[e] = le; sm.n_rep[e] = 0; sm.first[e] = 0x7fffffff;
+  }
+  if (tid == 0) sm.v_lam[E] = 0;
+  if (R * P <= kPcSmem) for (int i = tid; i < R * P; i += kPlanThreads) sm.pc[i] = 0;
+  if (crank == 0) {
+    int32_t* se = out.slot_expert + (size_t)batch_b * max(1, R * n_slot);
+    for (int i = tid; i < R * n_slot; i += kPlanThreads) se[i] = -1;
   }
   __syncthreads();
-  const int tau_lo0 = sm.lo, tau_hi0 = sm.hi;
 
   // ---- bisection (S9): per round up to 2^levels - 1 nodes of the SEQUENTIAL bisection tree rooted
   // at the current [lo, hi) are probed speculatively, then the path the sequential search takes is
@@ -391,6 +368,16 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       const int jl = 31 - __clz(q);
       return ((1 << (bot_depth - 1)) << jl) + (q - (1 << jl));
     };
+    // the path walk below is done by the first warp that does not probe; everything of it that
+    // does not need the verdicts (which node each lane stands for) is computed before the barrier
+    const bool walker = warp == kWalkWarp;
+    int n0 = 0, n1 = 0, d0 = 0, d1 = 0;
+    bool s0 = false, s1 = false;
+    if (walker) {
+      n0 = node_of(lane); n1 = node_of(lane + 32);                 // lane i: the nodes of slots i and i + 32
+      s0 = n0 > 0 && (n0 & (n0 - 1)) == 0; s1 = n1 > 0 && (n1 & (n1 - 1)) == 0;   // all-left nodes: powers of two
+      d0 = 32 - __clz(n0); d1 = 32 - __clz(n1);                    // depth, root = 1
+    }
     const int slot = warp * csize + crank;
     const int node = node_of(slot);
     if (node >= 1) {
@@ -419,26 +406,23 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       }
     }
     if (csize > 1) cluster.sync(); else __syncthreads();
-    if (warp == 0) {
-      // walk the sequential path; lane i knows the nodes of slots i and i + 32.  A node on the
-      // path has a non-empty interval, so it was probed if it was speculated at all.
-      // (verdicts in registers: a step of the walk is two ballots, no shared-memory load)
-      const int n0 = node_of(lane), n1 = node_of(lane + 32);
+    if (walker) {
+      // walk the sequential path.  A node on the path has a non-empty interval, so it was probed if
+      // it was speculated at all.  (verdicts in registers: a step of the walk is two ballots, no
+      // shared-memory load)
       const bool f0 = sm.node_feas[buf][lane] != 0, f1 = sm.node_feas[buf][lane + 32] != 0;
       int nd = 1, l = lo, h = hi, np = sm.n_probes, last_feas = -1;
       {
         // the run of feasible verdicts at the head of the path (usually the whole path) in one
-        // step: the all-left nodes are the powers of two; they are speculated at every depth up
-        // to spine_depth, and the first infeasible one ends the run
+        // step: the all-left nodes are speculated at every depth up to spine_depth, and the first
+        // infeasible one ends the run
         const int spine_depth = spine ? depth_left : min(levels, depth_left);
-        const bool s0 = n0 > 0 && (n0 & (n0 - 1)) == 0, s1 = n1 > 0 && (n1 & (n1 - 1)) == 0;
-        const int d0 = 32 - __clz(n0), d1 = 32 - __clz(n1);          // depth, root = 1
         int dinf = spine_depth + 1;
         if (s0 && !f0) dinf = min(dinf, d0);
         if (s1 && !f1) dinf = min(dinf, d1);
         dinf = __reduce_min_sync(kFull, dinf);                       // depth of the first infeasible all-left node
         const int n_left = dinf - 1;                                 // feasible all-left nodes on the path
-        for (int q = 0; q < n_left; ++q) h = (l + h) >> 1;           // lines 5, 21-22, n_left times
+        h = l + ((h - l) >> n_left);                                 // lines 5, 21-22, n_left times: h <- floor((l+h)/2)
         np += n_left;
         nd = 1 << n_left;
         if (n_left > 0) {
@@ -485,7 +469,8 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   const int log_node = sm.log_buf;
   const int owner = log_node < 0 ? 0 : (log_node & (csize - 1));
   if (crank != owner) return;
-  if (acc && tid < E) count_out[tid] = sm.lam[tid];
+  const int n_probes = sm.n_probes;
+  if (acc) for (int e = tid; e < E; e += kPlanThreads) count_out[e] = sm.lam[e];
   uep_plan_out o = out;            // this instance's arrays (offset only here: the probes above
   if (batch_b != 0) {              // must not carry eleven pointers in registers)
     const size_t bb = (size_t)batch_b;
@@ -504,144 +489,168 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (o.U) o.U += bb * E * R;
   }
   const int log_buf = log_node < 0 ? 0 : 1 + (log_node >> csh);
-  if (warp == 0 && sm.n_probes > 0 && log_node < 0) {
-    int nl;
-    probe<RPL, true>(sm, tau, R, n_slot, u_min, strict, lane, logs, nl);
-    if (lane == 0) sm.n_log = nl;
-  }
-  const int4* lg = logs + (size_t)log_buf * log_cap;
   const int RP = R * P;
   const bool pc_in_smem = RP <= kPcSmem;
   int* pc = pc_in_smem ? sm.pc : o.phys_count;
-  if (!pc_in_smem) for (int i = tid; i < RP; i += kPlanThreads) pc[i] = 0;
-  if (o.U) for (int i = tid; i < E * R; i += kPlanThreads) o.U[i] = 0;
-  __syncthreads();
+  if (n_probes > 0 && log_node < 0) {                  // (rare; CTA-uniform condition)
+    if (warp == 0) {
+      int nl;
+      probe<RPL, true>(sm, tau, R, n_slot, u_min, strict, lane, logs, nl);
+      if (lane == 0) sm.n_log = nl;
+    }
+    __syncthreads();
+  }
+  if (!pc_in_smem || o.U) {                            // (rare: large R*P, or the dense test table)
+    if (!pc_in_smem) for (int i = tid; i < RP; i += kPlanThreads) pc[i] = 0;
+    if (o.U) for (int i = tid; i < E * R; i += kPlanThreads) o.U[i] = 0;
+    __syncthreads();
+  }
+  const int4* lg = logs + (size_t)log_buf * log_cap;
   const int n_log = sm.n_log;
 
-  // ---- emit (line 22 "materialize U~ into X" + cumulative reroute metadata, §5.2) ---------
+  // ---- emit (line 22 "materialize U~ into X" + cumulative reroute metadata, §5.2): four phases.
+  // Phase A, straight from the log (thread t owns the consecutive entries t*kLogPer ..): per-expert
+  // replica count / main quota / first entry, X, the replicas' phys_count and U
+  if (tid == 32) {                 // everything known once the bisection has ended: off the tail of the kernel
+    o.scalars[UEP_SC_TAU] = tau;
+    o.scalars[UEP_SC_N_REPLICAS] = n_log;
+    o.scalars[UEP_SC_N_PROBES] = n_probes;
+    o.scalars[UEP_SC_N_INVALID] = S_total - sm.s_valid;
+    o.scalars[UEP_SC_TAU_LO0] = sm.lo0;
+    o.scalars[UEP_SC_TAU_HI0] = sm.hi0;
+    for (int i = UEP_SC_N_GROUPS + 1; i < UEP_N_SCALARS; ++i) o.scalars[i] = 0;
+  }
+  int4 le[kLogPer];
+  int dsum = 0;
 #pragma unroll
   for (int j = 0; j < kLogPer; ++j) {
     const int l = tid * kLogPer + j;
+    le[j] = make_int4(0, 0, 0, 0);
     if (l < n_log) {
-      const int e = lg[l].x;
-      atomicSub(&sm.u_main[e], lg[l].w);
+      le[j] = lg[l];
+      const int e = le[j].x, t = le[j].y, sl = le[j].z, dd = le[j].w;
+      atomicSub(&sm.u_main[e], dd);
       atomicAdd(&sm.n_rep[e], 1);
       atomicMin(&sm.first[e], l);
+      o.slot_expert[t * n_slot + sl] = e;                           // X
+      pc[t * P + M + sl] = dd;
+      if (o.U) o.U[e * R + t] = dd;
+      dsum += dd;
     }
   }
   __syncthreads();
+  // Phase B: one block scan for both prefix sums — instances per expert (high word; <= E + R * n_slot;
+  // thread t owns the consecutive experts t*EP ..) and delta over the log (low word; <= S < 2^24, so
+  // it never carries) — and the main instances' phys_count
+  const int EP = (E + kPlanThreads - 1) / kPlanThreads;            // 1 or 2
+  int fan_mx = 0, n_grp = 0;
   {
-    // one block scan for both prefix sums: instances per expert (high word; <= E + R * n_slot) and
-    // delta over the log, kLogPer entries per thread (low word; <= S < 2^24, so it never carries)
-    int d[kLogPer], dsum = 0;
+    int v = 0;
 #pragma unroll
-    for (int j = 0; j < kLogPer; ++j) {
-      const int l = tid * kLogPer + j;
-      d[j] = (l < n_log) ? lg[l].w : 0;
-      dsum += d[j];
+    for (int q = 0; q < kEPer; ++q) {
+      const int e = tid * EP + q;
+      if (q < EP && e < E) v += 1 + sm.n_rep[e];
     }
-    const int v = (tid < E) ? (1 + sm.n_rep[tid]) : 0;
     const unsigned long long both =
         block_incl_scan64(((unsigned long long)v << 32) | (unsigned long long)(unsigned)dsum, sm.scan_tmp);
-    const int inc = (int)(both >> 32);
-    if (tid < E) sm.inst_off[tid] = inc - v;
-    if (tid == E - 1) sm.inst_off[E] = inc;
+    int pos = (int)(both >> 32) - v;
+#pragma unroll
+    for (int q = 0; q < kEPer; ++q) {
+      const int e = tid * EP + q;
+      if (q < EP && e < E) {
+        const int nr = sm.n_rep[e], um = sm.u_main[e], h = sm.home[e], mp = sm.main_phys[e];
+        sm.inst_off[e] = pos;
+        o.inst_off[e] = pos;
+        o.inst_rank[pos] = h;                                        // CSR entry of the main instance
+        o.inst_phys[pos] = mp;
+        o.inst_cum[pos] = um;
+        pc[h * P + mp] = um;
+        if (o.U) o.U[e * R + h] = um;
+        pos += 1 + nr;
+        fan_mx = max(fan_mx, 1 + nr);
+        n_grp += nr > 0 ? 1 : 0;
+        if (e == E - 1) { sm.inst_off[E] = pos; o.inst_off[E] = pos; }
+      }
+    }
     int run = (int)(unsigned)both - dsum;
 #pragma unroll
     for (int j = 0; j < kLogPer; ++j) {
       const int l = tid * kLogPer + j;
-      run += d[j];
+      run += le[j].w;
       if (l < n_log) sm.dscan[l] = run;
     }
+    fan_mx = __reduce_max_sync(kFull, fan_mx);
+    n_grp = __reduce_add_sync(kFull, n_grp);
+    if (lane == 0) { sm.red_fan[warp] = fan_mx; sm.red_grp[warp] = n_grp; }
   }
   __syncthreads();
-  for (int i = tid; i <= E; i += kPlanThreads) o.inst_off[i] = sm.inst_off[i];
-  int fan = 0;
-  if (tid < E) {
-    const int pos = sm.inst_off[tid], h = sm.home[tid], um = sm.u_main[tid];
-    o.inst_rank[pos] = h;
-    o.inst_phys[pos] = sm.main_phys[tid];
-    o.inst_cum[pos] = um;
-    pc[h * P + sm.main_phys[tid]] = um;
-    if (o.U) o.U[tid * R + h] = um;
-    fan = 1 + sm.n_rep[tid];
-  }
+  // Phase C: the replicas' CSR entries (S11: acceptance order) and, a thread per rank, the receive
+  // layout inside every rank (S13)
 #pragma unroll
   for (int j = 0; j < kLogPer; ++j) {
     const int l = tid * kLogPer + j;
     if (l < n_log) {
-      const int e = lg[l].x, t = lg[l].y, sl = lg[l].z, dd = lg[l].w;
+      const int e = le[j].x;
       const int f = sm.first[e];
-      const int pos = sm.inst_off[e] + 1 + (l - f);                 // S11: acceptance order
+      const int pos = sm.inst_off[e] + 1 + (l - f);
       const int before = (f > 0) ? sm.dscan[f - 1] : 0;
-      o.inst_rank[pos] = t;
-      o.inst_phys[pos] = M + sl;
+      o.inst_rank[pos] = le[j].y;
+      o.inst_phys[pos] = M + le[j].z;
       o.inst_cum[pos] = sm.u_main[e] + sm.dscan[l] - before;
-      o.slot_expert[t * n_slot + sl] = e;                           // X
-      pc[t * P + M + sl] = dd;
-      if (o.U) o.U[e * R + t] = dd;
     }
   }
   for (int i = E + n_log + tid; i < E + R * n_slot; i += kPlanThreads) {   // unused CSR tail
     o.inst_rank[i] = -1; o.inst_phys[i] = -1; o.inst_cum[i] = 0; o.inst_base[i] = 0;
   }
-  // max fan-out and number of replicated experts
-  {
-    int mf = __reduce_max_sync(kFull, fan);
-    int ng = __reduce_add_sync(kFull, (fan > 1) ? 1 : 0);
-    __syncthreads();                                                // pc complete
-    if (lane == 0) { sm.feas[warp] = mf; sm.warp_tmp[warp] = ng; }
-  }
-  // receive layout (S13): per rank exclusive prefix over its P physical slots
-  int load = 0;
-  if (tid < R) {
-    for (int q = 0; q < P; ++q) {
-      const int cnt = pc[tid * P + q];
-      o.phys_base[tid * P + q] = load;
-      if (pc_in_smem) { o.phys_count[tid * P + q] = cnt; pc[tid * P + q] = load; }
+  if (tid < R) {                   // receive layout of rank tid (S13): exclusive prefix over its P physical slots
+    int load = 0;
+    for (int x = 0; x < P; ++x) {
+      const int cnt = pc[tid * P + x];
+      o.phys_base[tid * P + x] = load;
+      if (pc_in_smem) { o.phys_count[tid * P + x] = cnt; pc[tid * P + x] = load; }
       load += cnt;
     }
     o.rank_load[tid] = load;
+    sm.rload[tid] = load;
+  }
+  if (tid == kPlanThreads - 32) {  // (a lane of the last warp: no rank to lay out unless R > kPlanThreads - 32)
+    int max_fan = 0, n_groups = 0;
+    for (int w = 0; w < kPlanWarps; ++w) { max_fan = max(max_fan, sm.red_fan[w]); n_groups += sm.red_grp[w]; }
+    o.scalars[UEP_SC_MAX_FANOUT] = max_fan;
+    o.scalars[UEP_SC_N_GROUPS] = n_groups;
   }
   __syncthreads();
-  // inst_base: offset of each instance's first token in its rank's receive buffer (S13)
+  // Phase D: inst_base = offset of each instance's first token in its rank's receive buffer (S13),
+  // and by the last warp the exclusive prefix over ranks
   {
     const int* pb = pc_in_smem ? pc : o.phys_base;      // bases (global ones are CTA-visible now)
-    if (tid < E) o.inst_base[sm.inst_off[tid]] = pb[sm.home[tid] * P + sm.main_phys[tid]];
+    for (int e = tid; e < E; e += kPlanThreads) o.inst_base[sm.inst_off[e]] = pb[sm.home[e] * P + sm.main_phys[e]];
 #pragma unroll
     for (int j = 0; j < kLogPer; ++j) {
       const int l = tid * kLogPer + j;
       if (l < n_log) {
-        const int e = lg[l].x;
-        o.inst_base[sm.inst_off[e] + 1 + (l - sm.first[e])] = pb[lg[l].y * P + M + lg[l].z];
+        const int e = le[j].x;
+        o.inst_base[sm.inst_off[e] + 1 + (l - sm.first[e])] = pb[le[j].y * P + M + le[j].z];
       }
     }
   }
-  int max_fan = 0, n_groups = 0;
-  if (tid == 0) for (int w = 0; w < kPlanWarps; ++w) { max_fan = max(max_fan, sm.feas[w]); n_groups += sm.warp_tmp[w]; }
-  __syncthreads();
-  {
-    const int inc = block_incl_scan(load, sm.warp_tmp);
-    if (tid < R) o.rank_base[tid] = inc - load;
-    if (tid == R - 1) o.rank_base[R] = inc;
-    const int mx = __reduce_max_sync(kFull, load);
-    __syncthreads();
-    if (lane == 0) sm.feas[warp] = mx;
-    __syncthreads();
-  }
-  if (tid == 0) {
-    int max_load = 0;
-    for (int w = 0; w < kPlanWarps; ++w) max_load = max(max_load, sm.feas[w]);
-    o.scalars[UEP_SC_TAU] = tau;
-    o.scalars[UEP_SC_N_REPLICAS] = n_log;
-    o.scalars[UEP_SC_MAX_LOAD] = max_load;
-    o.scalars[UEP_SC_MAX_FANOUT] = max_fan;
-    o.scalars[UEP_SC_N_PROBES] = sm.n_probes;
-    o.scalars[UEP_SC_N_INVALID] = (int)((long long)S_total - sm.s_valid);
-    o.scalars[UEP_SC_TAU_LO0] = tau_lo0;
-    o.scalars[UEP_SC_TAU_HI0] = tau_hi0;
-    o.scalars[UEP_SC_N_GROUPS] = n_groups;
-    for (int i = UEP_SC_N_GROUPS + 1; i < UEP_N_SCALARS; ++i) o.scalars[i] = 0;
+  if (warp == kPlanWarps - 1) {    // exclusive prefix over ranks (lane t owns the consecutive ranks t*RW ..) and the maximum
+    const int RW = (R + 31) >> 5;
+    int tot = 0, mxl = 0;
+    for (int q = 0; q < RW; ++q) {
+      const int r = lane * RW + q;
+      const int v = r < R ? sm.rload[r] : 0;
+      tot += v;
+      mxl = max(mxl, v);
+    }
+    const int inc = warp_incl_scan(tot, lane);
+    int base = inc - tot;
+    for (int q = 0; q < RW; ++q) {
+      const int r = lane * RW + q;
+      if (r < R) { o.rank_base[r] = base; base += sm.rload[r]; }
+    }
+    mxl = __reduce_max_sync(kFull, mxl);
+    if (lane == 31) { o.rank_base[R] = inc; o.scalars[UEP_SC_MAX_LOAD] = mxl; }
   }
 }
 
@@ -734,7 +743,9 @@ int init_plan_kernels(Ctx* c) {
   if (rc == UEP_OK) rc = init_plan_one<4>(max16);
   if (rc == UEP_OK) rc = init_plan_one<8>(max16);
   // 8 CTAs x 8 probing warps cover the 64 tree slots of a round (launch_plan_t: levels = 6); the
-  // path walk relies on every speculated slot having an owner, so the size is not configurable
+  // path walk relies on every speculated slot having an owner, so the size is not configurable.
+  // (The verdict table is deliberately NOT cleared during setup: a peer CTA whose probe exits
+  // early may already have written its verdict into this CTA's shared memory by then.)
   c->plan_cluster = 8;
   static_assert(8 * 8 >= kPlanMaxNodes, "every tree slot of a round needs a probing warp");
   (void)max16;

@@ -18,7 +18,7 @@ constexpr int kRemapThreads = 512;
 constexpr int kRemapWarps = kRemapThreads / 32;
 constexpr int kRemapItems = 16;          // slots per lane per round (register-resident)
 constexpr int kRemapRound = kRemapThreads * kRemapItems;   // 8192 slots per CTA
-constexpr int kPlanThreads = 512;       // 128 registers per thread for the probes (64 at 1024 threads cost 2 us)
+constexpr int kPlanThreads = 512;       // 16 warps per CTA (8 probe), ~96 registers: a whole SM's register file for two CTAs' worth
 constexpr int kPlanLevels = 6;           // bisection levels speculated per round (63 probes over a cluster of 8 CTAs)
 constexpr int kPackTile = 16 * 1024;     // bytes per bulk-copy tile
 constexpr int kPackStages = 8;           // shared-memory ring depth
