@@ -50,7 +50,8 @@ constexpr int kEMask = (1 << kPackedEBits) - 1;
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kRemapThreads, 2)
 rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len, int cpg,
-            int group_len, int32_t* __restrict__ packed, int32_t* __restrict__ prefix, int chunk0) {
+            int group_len, int32_t* __restrict__ packed, int32_t* __restrict__ prefix,
+            int32_t* __restrict__ counts, int chunk0) {
   extern __shared__ __align__(16) int smem[];
   int2* wrow = reinterpret_cast<int2*>(smem);
   pdl_trigger();                                 // prefix_kernel may be scheduled (it waits for this grid)
@@ -114,6 +115,7 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
       }
     }
     prefix[(size_t)(cb + 1) * E_pad + e] = run;
+    counts[(size_t)cb * E_pad + e] = run;     // row c of `counts` is never rewritten: the lookup reads it before prefix_kernel is done
   }
   __syncthreads();
 
@@ -186,7 +188,7 @@ int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool
   rank_kernel<<<n_launch < 0 ? chunks : n_launch, kRemapThreads, smem, s>>>(
       ids, c->S, c->cfg.E, c->E_pad, local ? c->l_chunk_len : c->r_chunk_len,
       local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S, ws_packed(c, ws),
-      ws_prefix(c, ws), chunk0);
+      ws_prefix(c, ws), ws_counts(c, ws), chunk0);
   UEP_CUDA_TRY(cudaGetLastError());
   count_launch(c);
   if (with_prefix) return launch_prefix(c, ws, s, local, /*pdl=*/true);
@@ -313,23 +315,43 @@ int launch_reroute(const Ctx* c, const uep_plan_out& plan, int32_t* n_inflight, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// lookup_kernel.  dynamic shared memory layout (ints):
-//   rec[E_pad] (int4) | base0[E_pad] | s_off[E_pad+4] | rbase[(R+7)&~3]
-//   | i_cum | i_base | i_rank (icap each) | wtot[36]
-//   | (STAGE) stg[kMaxChunk] (int2 {gate bits, out_gate index})
+// lookup_kernel.  One CTA per chunk, a thread handles kLkPairs PAIRS of consecutive slots (8-byte
+// loads and stores).  Everything that does not need the plan runs BEFORE griddepcontrol.wait (under
+// programmatic dependent launch it overlaps the planner): the loads of the packed ranks and gates,
+// the exclusive prefix el[e] of the chunk's per-expert counts (from rank_kernel's `counts` row),
+// and the staging of the gates in (expert, rank) order — a slot's staging position el[e] + rank in
+// chunk does not depend on the plan.  After the wait a CTA stages the plan, builds two 8-byte
+// records per expert for the instance that holds the chunk's first slot of that expert,
+//   rec[e]  = {db, thr << 17 | replica << 8 | rank}   offset = db + jl          while jl < thr
+//   grec[e] = {gbx, el[e] + thr}                      out_gate index = gbx + staged position
+// and makes two passes: slots in slot order (one random 8-byte record load, three coalesced 8-byte
+// stores per pair) and gates in staged order (consecutive positions of an expert go to consecutive
+// destinations: coalesced runs).  A slot or gate beyond the first instance's window walks the
+// expert's cumulative quotas.  (The first version staged {gate, destination} AFTER the wait with a
+// random 8-byte shared store per slot and used 16-byte records: 39 warp instructions per slot,
+// 11.5 us between the end of the planner and the last CTA at the DeepSeek-V3 shape.)
+// dynamic shared memory layout (ints):
+//   rec[E_pad] (int2) | grec[E_pad] (int2) | base0[E_pad] | el[E_pad+4] | s_off[E_pad+4]
+//   | rbase[(R+7)&~3] | i_cum | i_base | i_rank (icap each) | wtot[36] | (GATE) stg[kMaxChunk] (int2 {gate bits, e})
 // ------------------------------------------------------------------------------------------------
+constexpr int kLkPairs = kMaxChunk / 2 / kRemapThreads;       // pairs of slots per thread (8)
+constexpr int kLkThrMax = (1 << 14) - 1;                      // thr field of rec: 14 bits, > any rank in a chunk
+
 __host__ __device__ inline size_t lookup_smem_ints(int E_pad, int R, int inst_cap) {
-  return 4 * (size_t)E_pad + (size_t)E_pad + (E_pad + 4) + ((R + 7) & ~3) +
+  return 2 * (size_t)E_pad + 2 * (size_t)E_pad + (size_t)E_pad + 2 * (size_t)(E_pad + 4) + ((R + 7) & ~3) +
          3 * (size_t)((inst_cap + 3) & ~3) + 36;           // a multiple of 4: stg is 16-B aligned
 }
 __host__ __device__ inline size_t lookup_smem_bytes(int E_pad, int R, int inst_cap, bool stage) {
   return sizeof(int) * lookup_smem_ints(E_pad, R, inst_cap) + (stage ? sizeof(int2) * (size_t)kMaxChunk : 0);
 }
 
+__device__ __forceinline__ int ld_cg_i32(const int32_t* p) { return __ldcg(p); }
+
 template <typename GateT, bool STAGE, bool LOCAL>
 __global__ void __launch_bounds__(kRemapThreads, 2)
 lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate, int S, int E,
               int E_pad, int R, int inst_cap, int chunk_len, const int32_t* __restrict__ prefix,
+              const int32_t* __restrict__ counts,
               const int32_t* __restrict__ g_inst_off, const int32_t* __restrict__ g_inst_rank,
               const int32_t* __restrict__ g_inst_cum, const int32_t* __restrict__ g_inst_base,
               const int32_t* __restrict__ g_rank_base, int32_t* __restrict__ out_replica,
@@ -346,16 +368,18 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   // instance's base is inst_base + srcpre[r][.] (receive order: by source rank).  Everything else
   // is the same lookup.
   extern __shared__ __align__(16) int smem[];
-  int4* rec = reinterpret_cast<int4*>(smem);     // [E_pad] fast-path record per expert
-  int* base0 = reinterpret_cast<int*>(rec + E_pad);   // [E_pad] global rank of the chunk's first slot of e
-  int* s_off = base0 + E_pad;                    // [E_pad+4] CSR of instances
-  int* rbase = s_off + E_pad + 4;                // [(R+7)&~3] rank_base
+  int2* rec = reinterpret_cast<int2*>(smem);                 // [E_pad] slot-pass record per expert
+  int2* grec = rec + E_pad;                                  // [E_pad] gate-pass record per expert
+  int* base0 = reinterpret_cast<int*>(grec + E_pad);         // [E_pad] rank (plan numbering) of the chunk's first slot of e
+  int* el = base0 + E_pad;                                   // [E_pad+4] exclusive prefix of the chunk's counts over experts
+  int* s_off = el + E_pad + 4;                               // [E_pad+4] CSR of instances
+  int* rbase = s_off + E_pad + 4;                            // [(R+7)&~3] rank_base
   const int icap = (inst_cap + 3) & ~3;
   int* i_cum = rbase + ((R + 7) & ~3);           // cumulative quotas (row of the source rank when local)
   int* i_base = i_cum + icap;                    // inst_base (+ srcpre when local)
   int* i_rank = i_base + icap;
-  int* wtot = i_rank + icap;                     // [32] warp totals, [32] = chunk total
-  int2* stg = reinterpret_cast<int2*>(wtot + 36);     // staged {gate bits, out_gate index}, (expert, rank) order
+  int* wtot = i_rank + icap;                     // [32] warp totals
+  int2* stg = reinterpret_cast<int2*>(wtot + 36);     // staged {gate bits, expert}, (expert, rank) order
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int c = LOCAL ? (int)blockIdx.x + chunk0 : (int)blockIdx.x;
@@ -365,36 +389,68 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   const int clen = LOCAL ? (int)min(min((long long)chunk_len, (long long)group_len - (long long)sub * chunk_len),
                                     (long long)S - cbegin)
                          : (int)min((long long)chunk_len, (long long)S - cbegin);
-  const int items = (clen + kRemapThreads - 1) / kRemapThreads;
-  const bool full = (clen == items * kRemapThreads);
-  const int wbeg = warp * items * 32;
-  const int room = full ? 0x7fffffff : clen - wbeg - lane;
-  const bool has_gate = gate != nullptr;
-  const long long tbeg = cbegin + wbeg + lane;
-  packed += tbeg; out_replica += tbeg; out_rank += tbeg; out_offset += tbeg;
-  if (has_gate) gate += tbeg;
+  const bool has_gate = STAGE && gate != nullptr;
+  const bool even = (cbegin & 1) == 0;           // pairs are 8-byte aligned (always, unless a source rank's block is odd)
+  packed += cbegin; out_replica += cbegin; out_rank += cbegin; out_offset += cbegin;
+  if (has_gate) gate += cbegin;
 
-  int pv[kRemapItems];
-  GateT gv[kRemapItems];
+  // ---- plan-independent prologue ---------------------------------------------------------------
+  int2 pv[kLkPairs];
+  GateT gv[kLkPairs][2];
 #pragma unroll
-  for (int i = 0; i < kRemapItems; ++i) {
-    const bool in = (i < items) && (i * 32 < room);
-    pv[i] = in ? __ldg(packed + i * 32) : -1;
-    if (has_gate) gv[i] = in ? __ldg(gate + i * 32) : GateT(0);
+  for (int it = 0; it < kLkPairs; ++it) {
+    const int s0 = 2 * (it * kRemapThreads + tid);
+    pv[it] = make_int2(-1, -1);
+    if (s0 + 1 < clen && even) {
+      pv[it] = __ldcg(reinterpret_cast<const int2*>(packed + s0));
+    } else {
+      if (s0 < clen) pv[it].x = __ldcg(packed + s0);
+      if (s0 + 1 < clen) pv[it].y = __ldcg(packed + s0 + 1);
+    }
+    if (has_gate) {
+      gv[it][0] = s0 < clen ? __ldg(gate + s0) : GateT(0);
+      gv[it][1] = s0 + 1 < clen ? __ldg(gate + s0 + 1) : GateT(0);
+    }
+  }
+  // el[e]: exclusive prefix over experts of this chunk's counts (one thread per expert: E <= kRemapThreads)
+  {
+    const int n_own = (tid < E) ? __ldcg(counts + (size_t)c * E_pad + tid) : 0;
+    int inc = n_own;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int y = __shfl_up_sync(kFullMask, inc, o);
+      if (lane >= o) inc += y;
+    }
+    if (lane == 31) wtot[warp] = inc;
+    __syncthreads();
+    int pre = 0;
+    for (int w = 0; w < warp; ++w) pre += wtot[w];
+    if (tid < E) el[tid] = pre + inc - n_own;
+    if (tid == kRemapThreads - 1) el[E] = pre + inc;              // valid slots in this chunk (E < kRemapThreads or == : tid 511 holds the total)
+  }
+  __syncthreads();
+  if (has_gate) {                                            // gates into (expert, rank) order
+#pragma unroll
+    for (int it = 0; it < kLkPairs; ++it) {
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int pk = u ? pv[it].y : pv[it].x;
+        if (pk >= 0) {
+          const int e = pk & kEMask;
+          stg[el[e] + (pk >> kPackedEBits)] = make_int2((int)gv[it][u], e);
+        }
+      }
+    }
   }
 
-  // ---- everything above is independent of the plan and of prefix_kernel (the packed ranks were
-  // complete before prefix_kernel started): under programmatic dependent launch it overlaps the
-  // planner (uep_balance) or prefix_kernel (uep_remap); now wait for them ------------------------
+  // ---- everything above is independent of the plan and of prefix_kernel (rank_kernel's outputs were
+  // complete before prefix_kernel started); now wait for the planner / prefix_kernel ------------------
   pdl_wait();
-  // ---- chunk base ranks: row c of the exclusive prefix over chunks that prefix_kernel left.  Read
-  // AFTER the wait, in the same L2 round trip as the plan below: under stream capture the lookup's
-  // programmatic attribute makes its edge from prefix_kernel programmatic too, and only the wait
-  // guarantees that kernel's writes are visible.  (Reading the rows in the prologue was 0.3 us
-  // faster and never observed stale; reading them early and verifying after the wait measured the
-  // same as this.) ---------------------------------------------------------------------------------
+  // chunk base ranks: row c of the exclusive prefix over chunks that prefix_kernel left.  Read AFTER
+  // the wait, in the same L2 round trip as the plan: under stream capture the lookup's programmatic
+  // attribute makes its edge from prefix_kernel programmatic too, and only the wait guarantees that
+  // kernel's writes are visible.
   const int p_own = (tid < E) ? __ldcg(prefix + (size_t)c * E_pad + tid) : 0;
-  const int n_own = (tid < E) ? __ldcg(prefix + (size_t)(c + 1) * E_pad + tid) - p_own : 0;
   const int b0_own = (local && tid < E) ? p_own - __ldcg(prefix + (size_t)grp * cpg * E_pad + tid) : p_own;
   // uep_balance: the planner (now complete) has consumed the histogram's accumulator; clear it for
   // the next call
@@ -406,82 +462,62 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
     i_rank[p] = g_inst_rank[p];
     i_base[p] = g_inst_base[p] + (local ? __ldcg(srcpre + (size_t)grp * inst_cap + p) : 0);
   }
-  int el_inc = n_own;                            // inclusive scan of n_own over experts
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int y = __shfl_up_sync(kFullMask, el_inc, o);
-    if (lane >= o) el_inc += y;
-  }
-  if (lane == 31) wtot[warp] = el_inc;
   __syncthreads();
-  // rec[e] (E <= kRemapThreads: one thread per expert), in chunk-rank space: {cum - base0,
-  // dbase + base0, gbase + base0, staging base << 19 | replica << 8 | rank} of the instance
-  // holding the chunk's first slot of e, where dbase = inst_base - cum_prev (offset = dbase + j)
-  // and gbase = rank_base[rank] + dbase (out_gate index = gbase + j)
-  {
-    int pre = 0;
-    for (int w = 0; w < warp; ++w) pre += wtot[w];
-    if (tid < E) {
-      const int lo = s_off[tid], last = s_off[tid + 1] - 1, b0 = b0_own;
-      int p = lo;
-      while (p < last && i_cum[p] <= b0) ++p;
-      const int rk = i_rank[p];
-      const int d = i_base[p] - (p > lo ? i_cum[p - 1] : 0) + b0;
-      base0[tid] = b0;
-      rec[tid] = make_int4(i_cum[p] - b0, d, rbase[rk] + d,
-                           (int)(((unsigned)(pre + el_inc - n_own) << 19) | (unsigned)((p - lo) << 8) | (unsigned)rk));
-    }
-    if (tid == kRemapThreads - 1) wtot[32] = pre + el_inc;          // valid slots in this chunk
+  if (tid < E) {
+    const int lo = s_off[tid], last = s_off[tid + 1] - 1, b0 = b0_own;
+    int p = lo;
+    while (p < last && i_cum[p] <= b0) ++p;
+    const int rk = i_rank[p];
+    const int d = i_base[p] - (p > lo ? i_cum[p - 1] : 0) + b0;     // offset = d + rank in chunk
+    const int thr = min(i_cum[p] - b0, kLkThrMax);                  // ... while rank in chunk < thr
+    const int e0 = el[tid];
+    base0[tid] = b0;
+    rec[tid] = make_int2(d, (int)(((unsigned)thr << 17) | (unsigned)((p - lo) << 8) | (unsigned)rk));
+    grec[tid] = make_int2(rbase[rk] + d - e0, e0 + thr);
   }
   __syncthreads();
 
+  // a slot of expert e with rank jl in the chunk that lies beyond the first instance's window
+  auto walk = [&](int e, int jl, int rep0, int& rep, int& rk, int& db) {
+    const int b0 = base0[e], j = jl + b0;
+    int p = s_off[e] + rep0 + 1;
+    const int last = s_off[e + 1] - 1;             // cum[last] = lambda_e > j when ws matches plan
+    while (p < last && i_cum[p] <= j) ++p;
+    rk = i_rank[p];
+    db = i_base[p] - i_cum[p - 1] + b0;            // p > s_off[e]: cum_prev is the entry before
+    rep = p - s_off[e];
+  };
+
+  // ---- slot pass ----------------------------------------------------------------------------------
   int n_fly = 0;
-  // two slots at a time: their records are loaded before any of them stores to shared memory
-  // (the compiler cannot prove that the staging stores do not alias the records)
 #pragma unroll
-  for (int i0 = 0; i0 < kRemapItems; i0 += 2) {
-    if (i0 < items) {
-      int4 rc[2];
-#pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        const int pk = pv[i0 + u];
-        rc[u] = rec[pk >= 0 ? (pk & kEMask) : 0];
-      }
+  for (int it = 0; it < kLkPairs; ++it) {
+    const int s0 = 2 * (it * kRemapThreads + tid);
+    if (s0 < clen) {
+      int rep[2], rk[2], of[2];
 #pragma unroll
       for (int u = 0; u < 2; ++u) {
-        const int i = i0 + u;
-        if (i < items && i * 32 < room) {
-          const int pk = pv[i];
-          int rep = -1, rk = -1, of = -1;
-          if (pk >= 0) {
-            const int e = pk & kEMask, jl = pk >> kPackedEBits;
-            int db = rc[u].y, gb = rc[u].z;
-            const unsigned rw = (unsigned)rc[u].w;
-            rep = (int)((rw >> 8) & 0x7ffu);
-            rk = (int)(rw & 0xffu);
-            if (jl >= rc[u].x) {                         // past the first instance of this chunk's window
-              const int b0 = base0[e], j = jl + b0;
-              int p = s_off[e] + rep + 1;
-              const int last = s_off[e + 1] - 1;         // cum[last] = lambda_e > j when ws matches plan
-              while (p < last && i_cum[p] <= j) ++p;
-              rk = i_rank[p];
-              db = i_base[p] - i_cum[p - 1] + b0;          // p > s_off[e]: cum_prev is the entry before
-              gb = rbase[rk] + db; rep = p - s_off[e];
-            }
-            of = db + jl;
-            if (has_gate) {
-              if (STAGE) {
-                stg[(int)(rw >> 19) + jl] = make_int2((int)gv[i], gb + jl);
-              } else {
-                out_gate[gb + jl] = gv[i];
-              }
-            }
-          }
-          out_replica[i * 32] = rep;
-          out_rank[i * 32] = rk;
-          out_offset[i * 32] = of;
-          if (LOCAL) n_fly += (rk >= 0 && rk != grp) ? 1 : 0;
+        const int pk = u ? pv[it].y : pv[it].x;
+        rep[u] = -1; rk[u] = -1; of[u] = -1;
+        if (pk >= 0) {
+          const int e = pk & kEMask, jl = pk >> kPackedEBits;
+          const int2 rc = rec[e];
+          const unsigned w = (unsigned)rc.y;
+          int db = rc.x;
+          rep[u] = (int)((w >> 8) & 0x1ffu);
+          rk[u] = (int)(w & 0xffu);
+          if (jl >= (int)(w >> 17)) walk(e, jl, rep[u], rep[u], rk[u], db);
+          of[u] = db + jl;
+          if (LOCAL) n_fly += (rk[u] != grp) ? 1 : 0;
         }
+      }
+      if (s0 + 1 < clen && even) {
+        *reinterpret_cast<int2*>(out_replica + s0) = make_int2(rep[0], rep[1]);
+        *reinterpret_cast<int2*>(out_rank + s0) = make_int2(rk[0], rk[1]);
+        *reinterpret_cast<int2*>(out_offset + s0) = make_int2(of[0], of[1]);
+      } else {
+        out_replica[s0] = rep[0]; out_rank[s0] = rk[0]; out_offset[s0] = of[0];
+        if (s0 + 1 < clen) { out_replica[s0 + 1] = rep[1]; out_rank[s0 + 1] = rk[1]; out_offset[s0 + 1] = of[1]; }
       }
     }
   }
@@ -490,16 +526,21 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
     if (lane == 0 && n_fly) atomicAdd(n_inflight + grp, n_fly);
   }
 
-  if (STAGE && has_gate) {                               // staged gates leave as contiguous runs
-    __syncthreads();
-    const int n_valid = wtot[32];
-#pragma unroll
-    for (int i = 0; i < kRemapItems; ++i) {
-      const int lp = i * kRemapThreads + tid;
-      if (lp < n_valid) {
-        const int2 v = stg[lp];
-        out_gate[v.y] = (GateT)v.x;
+  // ---- gate pass: staged order, consecutive positions of an expert go to consecutive destinations ---
+  if (has_gate) {
+    const int n_valid = el[E];
+#pragma unroll 4
+    for (int ps = tid; ps < n_valid; ps += kRemapThreads) {
+      const int2 v = stg[ps];
+      const int2 g = grec[v.y];
+      int dst = g.x + ps;
+      if (ps >= g.y) {                                   // beyond the first instance's window
+        const int e = v.y, jl = ps - el[e];
+        int rep, rk, db;
+        walk(e, jl, (int)(((unsigned)rec[e].y >> 8) & 0x1ffu), rep, rk, db);
+        dst = rbase[rk] + db + jl;
       }
+      out_gate[dst] = (GateT)v.x;
     }
   }
 }
@@ -530,7 +571,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
   const int32_t* srcpre = cumq ? cumq + (size_t)g.R * inst_cap : nullptr;
   UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, k, (const int32_t*)ws_packed(c, ws), gate, c->S, g.E, c->E_pad,
                                   g.R, inst_cap, local ? c->l_chunk_len : c->r_chunk_len,
-                                  (const int32_t*)ws_prefix(c, ws),
+                                  (const int32_t*)ws_prefix(c, ws), (const int32_t*)ws_counts(c, ws),
                                   (const int32_t*)p.inst_off, (const int32_t*)p.inst_rank,
                                   (const int32_t*)p.inst_cum, (const int32_t*)p.inst_base,
                                   (const int32_t*)p.rank_base, out_replica, out_rank, out_offset,

@@ -199,7 +199,7 @@ void uep_destroy(uep_ctx* ctx) {
 size_t uep_workspace_bytes(const uep_ctx* ctx) {
   const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
   if (!c) return 0;
-  return (size_t)kWsHeaderBytes + ws_table_bytes(c) + ws_prefix_bytes(c) + ws_packed_bytes(c) +
+  return (size_t)kWsHeaderBytes + ws_table_bytes(c) + 2 * ws_prefix_bytes(c) + ws_packed_bytes(c) +
          sizeof(int32_t) * ws_reroute_ints(c);
 }
 

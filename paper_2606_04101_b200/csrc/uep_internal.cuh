@@ -177,13 +177,17 @@ inline size_t ws_reroute_ints(const Ctx* c) {             // cumq and srcpre: [R
 inline int32_t* ws_prefix(const Ctx* c, void* ws) {      // exclusive prefix over remap chunks (+ totals row)
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c));
 }
-inline int32_t* ws_packed(const Ctx* c, void* ws) {      // [S] packed (expert, rank in chunk)
+inline int32_t* ws_counts(const Ctx* c, void* ws) {      // per-chunk expert counts, row c = chunk c (never scanned)
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c) +
                                     ws_prefix_bytes(c));
 }
+inline int32_t* ws_packed(const Ctx* c, void* ws) {      // [S] packed (expert, rank in chunk)
+  return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c) +
+                                    2 * ws_prefix_bytes(c));
+}
 inline int32_t* ws_reroute(const Ctx* c, void* ws) {     // source-aware split tables (uep_remap_local)
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c) +
-                                    ws_prefix_bytes(c) + ws_packed_bytes(c));
+                                    2 * ws_prefix_bytes(c) + ws_packed_bytes(c));
 }
 
 }  // namespace uep
