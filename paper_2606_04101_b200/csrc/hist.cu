@@ -111,6 +111,10 @@ __global__ void hist_empty_kernel(int E, int E_pad, int32_t* table, int32_t* exp
 }
 
 int init_hist_kernels() {
+  int rc = prefer_max_smem(hist_kernel<false>);
+  if (rc == UEP_OK) rc = prefer_max_smem(hist_kernel<true>);
+  if (rc == UEP_OK) rc = prefer_max_smem(publish_kernel);
+  if (rc != UEP_OK) return rc;
   UEP_CUDA_TRY(cudaFuncSetAttribute(hist_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(sizeof(int) * (hist_smem_ints(UEP_MAX_E) + 4))));
   UEP_CUDA_TRY(cudaFuncSetAttribute(hist_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,

@@ -150,6 +150,7 @@ pack_kernel(PackArgs a, int E, int n_slot, int M, const int32_t* __restrict__ in
 }
 
 int init_pack_kernels() {
+  if (prefer_max_smem(pack_kernel) != UEP_OK) return UEP_ERR_CUDA;
   UEP_CUDA_TRY(cudaFuncSetAttribute(pack_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     kPackStages * kPackTile));
   return UEP_OK;

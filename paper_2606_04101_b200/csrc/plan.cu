@@ -719,6 +719,7 @@ static int init_plan_one(int& max16) {
   UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL, false>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
   UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(plan_kernel<RPL, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+  if (prefer_max_smem(plan_kernel<RPL, false>) != UEP_OK || prefer_max_smem(plan_kernel<RPL, true>) != UEP_OK) return UEP_ERR_CUDA;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(16);
   cfg.blockDim = dim3(kPlanThreads);

@@ -582,6 +582,18 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
 }
 
 int init_remap_kernels() {
+  int rc = prefer_max_smem(rank_kernel);
+  if (rc == UEP_OK) rc = prefer_max_smem(prefix_kernel);
+  if (rc == UEP_OK) rc = prefer_max_smem(reroute_kernel);
+  if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint32_t, true, false>);
+  if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint32_t, true, true>);
+  if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint32_t, false, false>);
+  if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint32_t, false, true>);
+  if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint16_t, true, false>);
+  if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint16_t, true, true>);
+  if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint16_t, false, false>);
+  if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint16_t, false, true>);
+  if (rc != UEP_OK) return rc;
   const int rank_bytes = (int)(sizeof(int2) * (size_t)kRemapWarps * UEP_MAX_E);
   const int bytes = (int)lookup_smem_bytes(UEP_MAX_E, UEP_MAX_R, UEP_MAX_E + UEP_MAX_R * UEP_MAX_NSLOT, true);
   UEP_CUDA_TRY(cudaFuncSetAttribute(rank_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rank_bytes));

@@ -73,6 +73,17 @@ struct PackArgs {
 
 int set_cuda_error(cudaError_t e);
 
+// An SM's L1 / shared-memory split is chosen for the kernels running on it; a kernel whose shared
+// memory does not fit into the current split waits until the SM has drained (measured: rank_kernel
+// CTAs, 32 KB, did not start beside hist_kernel CTAs, 33 KB, although registers and threads allowed
+// it — the histogram's split was 64 KB).  Every kernel that takes part in uep_balance therefore asks
+// for the largest shared-memory carveout; none of them depends on L1 hit rates.
+template <typename K>
+inline int prefer_max_smem(K kernel) {
+  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  return e == cudaSuccess ? UEP_OK : set_cuda_error(e);
+}
+
 // every CTA adds its counts to ws_acc(ws) with fire-and-forget reductions.  red = true
 // (uep_balance): the planner (launch_plan with acc) reads them there and publishes expert_count,
 // the lookup zeroes the accumulator again.  red = false: publish_kernel does both.
