@@ -217,15 +217,18 @@ int uep_remap_local(const uep_ctx* ctx, const int32_t* topk_ids, const void* gat
  * GPU g of G (G divides R, T % R == 0) owns the tokens of source ranks [g*R/G, (g+1)*R/G), i.e.
  * the contiguous slot range [g*S/G, (g+1)*S/G).  One layer is
  *   uep_shard_count   on every GPU: ranks its LOCAL slots inside their chunks and leaves this
- *                     shard's rows of the count table (per-chunk lambda: the rows of Lambda[R,E],
- *                     subdivided) in ws;
- *   an all-gather     of those rows, by the caller (NCCL / torch.distributed; the only exchange).
- *                     uep_shard_rows gives the byte range of shard g's rows inside ws: the ranges
- *                     of shards 0..G-1 are equal-sized, contiguous and in shard order, so an
- *                     in-place all-gather on ws[offset(0) .. offset(0) + G*bytes) does it;
- *   uep_shard_finish  on every GPU, redundantly and deterministically: prefix over the gathered
- *                     table, lambda_e = its totals row -> expert_count, the SAME plan everywhere,
- *                     then the lookup of the local slots with their GLOBAL stable ranks.
+ *                     shard's rows of the count matrix Lambda[R][E] (lambda_{r,e}: one row of E_pad
+ *                     int32 per source rank the shard owns) in ws;
+ *   an all-gather     of those rows, by the caller (NCCL / torch.distributed; the only exchange:
+ *                     4 * E_pad * R bytes in total, 64 KB at R = 64, E = 256).  uep_shard_rows gives
+ *                     the byte range of shard g's rows inside ws: the ranges of shards 0..G-1 are
+ *                     equal-sized, contiguous and in shard order, so an in-place all-gather on
+ *                     ws[offset(0) .. offset(0) + G*bytes) does it.  With G = 1 there is nothing to
+ *                     exchange and count -> finish is one capturable sequence;
+ *   uep_shard_finish  on every GPU, redundantly and deterministically: exclusive prefix of Lambda over
+ *                     source ranks (+ the shard's own per-chunk counts) = the GLOBAL stable rank base
+ *                     of every local chunk, lambda_e = the column sums -> expert_count, the SAME plan
+ *                     everywhere, then the lookup of the local slots.
  * The concatenation of the shards' outputs equals uep_remap on the whole input (global stable
  * order, S12), bit for bit; G = 1 is the whole problem.
  *   topk_ids_local / gate_local / out_*_local   DEVICE, the shard's S/G slots, 16-B aligned

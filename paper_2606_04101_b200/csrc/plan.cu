@@ -201,8 +201,11 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
             const int32_t* __restrict__ g_main_phys, const int32_t* __restrict__ g_roff,
             const int32_t* __restrict__ g_rexp, uep_plan_out out, int E, int R, int n_slot, int M,
             int P, int u_min, int beta_num, int beta_den, int strict_i, int S_total, int n_bufs,
-            int log_cap, int levels, const int32_t* __restrict__ acc, int32_t* __restrict__ count_out) {
+            int log_cap, int levels, const int32_t* __restrict__ acc, int32_t* __restrict__ count_out,
+            int acc_rows, int acc_pitch) {
   // acc != nullptr (uep_balance): lambda_e comes from the histogram's accumulator in the workspace
+  // (acc_rows == 1), or is the column sum of the gathered count matrix Lambda[acc_rows][acc_pitch] of
+  // the token-sharded path ("every rank solves the same plan" from the exchanged counts)
   // and the CTA that emits the plan also publishes it as expert_count (count_out)
   cg::cluster_group cluster = cg::this_cluster();
   const int csize = (int)cluster.num_blocks(), crank = (int)cluster.block_rank();
@@ -236,7 +239,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   pdl_wait();                      // the histogram (preceding kernel) is complete
   // phase 1: lambda_e into shared memory, and line 2 (l_r) straight from global memory with
   // independent loads (thread r sums its own experts: no barrier between lambda and l_r)
-  {
+  if (acc_rows <= 1) {
     const int32_t* lam_g = acc ? acc + 0 : expert_count;
     for (int e = tid; e < E; e += kPlanThreads) sm.lam[e] = __ldcg(lam_g + e);
     if (tid < R) {
@@ -244,6 +247,19 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       const int a = sm.roff[tid], b = sm.roff[tid + 1];
 #pragma unroll 4
       for (int i = a; i < b; ++i) s += __ldcg(lam_g + sm.rexp[i]);
+      sm.ell[tid] = s;
+    }
+  } else {                         // Alg. 1 line 2 in full: lambda_e = sum_r lambda_{r,e}
+    for (int e = tid; e < E; e += kPlanThreads) {
+      int s = 0;
+#pragma unroll 8
+      for (int r = 0; r < acc_rows; ++r) s += __ldcg(acc + (size_t)r * acc_pitch + e);
+      sm.lam[e] = s;
+    }
+    __syncthreads();
+    if (tid < R) {
+      int s = 0;
+      for (int i = sm.roff[tid]; i < sm.roff[tid + 1]; ++i) s += sm.lam[sm.rexp[i]];
       sm.ell[tid] = s;
     }
   }
@@ -658,7 +674,8 @@ constexpr size_t kLogBudget = 128 * 1024;     // shared memory for the accept lo
 
 template <int RPL>
 static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out& plan,
-                         cudaStream_t s, bool pdl, int n_inst, const int32_t* acc, int32_t* count_out) {
+                         cudaStream_t s, bool pdl, int n_inst, const int32_t* acc, int32_t* count_out,
+                         int acc_rows, int acc_pitch) {
   const uep_config& g = c->cfg;
   const int levels = 6;                                        // 63 nodes over kPlanCluster CTAs
   const int cluster = c->plan_cluster;
@@ -697,19 +714,19 @@ static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out&
                                   (const int32_t*)c->d_rexp, plan, g.E, g.R, g.n_slot, c->M, c->P,
                                   g.u_min, g.beta_num, g.beta_den,
                                   g.floor_mode == UEP_FLOOR_STRICT ? 1 : 0, c->S, n_bufs, log_cap,
-                                  levels, acc, count_out));
+                                  levels, acc, count_out, acc_rows, acc_pitch));
   count_launch(c);
   return UEP_OK;
 }
 
 int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
-                bool pdl, int n_inst, int32_t* acc, int32_t* count_out) {
+                bool pdl, int n_inst, int32_t* acc, int32_t* count_out, int acc_rows, int acc_pitch) {
   const int R = c->cfg.R;
   if (n_inst <= 0) return UEP_OK;
-  if (R <= 32) return launch_plan_t<1>(c, count, plan, s, pdl, n_inst, acc, count_out);
-  if (R <= 64) return launch_plan_t<2>(c, count, plan, s, pdl, n_inst, acc, count_out);
-  if (R <= 128) return launch_plan_t<4>(c, count, plan, s, pdl, n_inst, acc, count_out);
-  return launch_plan_t<8>(c, count, plan, s, pdl, n_inst, acc, count_out);
+  if (R <= 32) return launch_plan_t<1>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch);
+  if (R <= 64) return launch_plan_t<2>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch);
+  if (R <= 128) return launch_plan_t<4>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch);
+  return launch_plan_t<8>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch);
 }
 
 template <int RPL>

@@ -177,6 +177,50 @@ prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG) {
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Token-sharded path: what crosses GPUs is the count matrix
+// Lambda[R][E] (lambda_{r,e}: one row per source rank, 4*E_pad bytes each), not the per-chunk rows.
+//   shard_rows_kernel    a shard's rows of Lambda = the sums of its source ranks' chunk counts
+//                        (launched programmatically dependent on rank_kernel).
+// After the exchange nothing runs between it and the planner: plan_kernel adds up the columns of
+// Lambda (Alg. 1 line 2), and lookup_kernel (from_lambda) derives the global rank base of its chunk,
+// sum_{r' < r} Lambda[r'][e] + the counts of the source rank's earlier chunks, in its prologue.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(UEP_MAX_E)
+shard_rows_kernel(int E_pad, int cpg, int rank0, const int32_t* __restrict__ counts, int32_t* __restrict__ lambda) {
+  pdl_wait();                                   // rank_kernel complete
+  pdl_trigger();                                // (one GPU: the planner is next; the lookup behind it reads only
+                                                //  LOWER shards' rows of Lambda before its own wait)
+  const int r = rank0 + (int)blockIdx.x;
+  for (int e = threadIdx.x; e < E_pad; e += blockDim.x) {
+    int s = 0;
+    for (int q = 0; q < cpg; ++q) s += __ldcg(counts + (size_t)(r * cpg + q) * E_pad + e);
+    lambda[(size_t)r * E_pad + e] = s;
+  }
+}
+
+static void pdl_config(cudaLaunchConfig_t& cfg, cudaLaunchAttribute* attr, dim3 grid, dim3 block, cudaStream_t s, bool pdl) {
+  cfg = cudaLaunchConfig_t{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.stream = s;
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl ? 1 : 0;
+}
+
+int launch_shard_rows(const Ctx* c, void* ws, cudaStream_t s, int rank0, int n_ranks) {
+  if (c->S == 0) return UEP_OK;
+  cudaLaunchConfig_t cfg;
+  cudaLaunchAttribute attr[1];
+  pdl_config(cfg, attr, dim3(n_ranks), dim3(c->E_pad < 32 ? 32 : c->E_pad), s, /*pdl=*/true);
+  UEP_CUDA_TRY(cudaLaunchKernelEx(&cfg, shard_rows_kernel, c->E_pad, c->l_cpg, rank0,
+                                  (const int32_t*)ws_counts(c, ws), ws_lambda(c, ws)));
+  count_launch(c);
+  return UEP_OK;
+}
+
 // chunk0 / n_launch: the chunk range a token shard owns (uep_shard_count; `ids` is then the
 // virtual base of the global [S] array, only the shard's slots are dereferenced); n_launch < 0:
 // all chunks.  with_prefix = false leaves the raw per-chunk counts for the exchange step.
@@ -358,7 +402,8 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
               int32_t* __restrict__ out_rank, int32_t* __restrict__ out_offset,
               GateT* __restrict__ out_gate, int cpg, int group_len,
               const int32_t* __restrict__ cumq, const int32_t* __restrict__ srcpre,
-              int32_t* __restrict__ n_inflight, int32_t* __restrict__ acc_clear, int chunk0) {
+              int32_t* __restrict__ n_inflight, int32_t* __restrict__ acc_clear, int chunk0,
+              const int32_t* __restrict__ lambda) {
   // Token-sharded mode (LOCAL with cumq == nullptr): the grouped chunk geometry and
   // the per-source in-flight count of the source-aware mode, but GLOBAL ranks and the plan's own
   // cumulative quotas, on the chunks [chunk0, chunk0 + gridDim.x) that this GPU owns.
@@ -429,6 +474,18 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
     if (tid == kRemapThreads - 1) el[E] = pre + inc;              // valid slots in this chunk (E < kRemapThreads or == : tid 511 holds the total)
   }
   __syncthreads();
+  // token-sharded path: global rank of the chunk's first slot of e = the slots of e on the source
+  // ranks of LOWER shards (their rows of the gathered Lambda, complete before the planner in front of
+  // this kernel started) + those in this shard's earlier chunks (its own counts, complete since
+  // rank_kernel; this shard's own rows of Lambda may still be being written on one GPU); no prefix kernel
+  int p_lam = 0;
+  if (LOCAL && lambda != nullptr && tid < E) {
+    const int r_lo = chunk0 / cpg;
+#pragma unroll 8
+    for (int r = 0; r < r_lo; ++r) p_lam += __ldcg(lambda + (size_t)r * E_pad + tid);
+#pragma unroll 8
+    for (int ch = chunk0; ch < c; ++ch) p_lam += __ldcg(counts + (size_t)ch * E_pad + tid);
+  }
   if (has_gate) {                                            // gates into (expert, rank) order
 #pragma unroll
     for (int it = 0; it < kLkPairs; ++it) {
@@ -450,7 +507,7 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
   // the wait, in the same L2 round trip as the plan: under stream capture the lookup's programmatic
   // attribute makes its edge from prefix_kernel programmatic too, and only the wait guarantees that
   // kernel's writes are visible.
-  const int p_own = (tid < E) ? __ldcg(prefix + (size_t)c * E_pad + tid) : 0;
+  const int p_own = (LOCAL && lambda != nullptr) ? p_lam : (tid < E) ? __ldcg(prefix + (size_t)c * E_pad + tid) : 0;
   const int b0_own = (local && tid < E) ? p_own - __ldcg(prefix + (size_t)grp * cpg * E_pad + tid) : p_own;
   // uep_balance: the planner (now complete) has consumed the histogram's accumulator; clear it for
   // the next call
@@ -550,7 +607,7 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
                            int32_t* out_replica, int32_t* out_rank, int32_t* out_offset,
                            GateT* out_gate, void* ws, cudaStream_t s, bool pdl, bool local,
                            int32_t* n_inflight, int32_t* acc_clear, int chunk0, int n_launch,
-                           bool src_aware) {
+                           bool src_aware, bool from_lambda) {
   const uep_config& g = c->cfg;
   const int inst_cap = g.E + g.R * g.n_slot;
   const bool stage = gate != nullptr;
@@ -576,7 +633,8 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
                                   (const int32_t*)p.inst_cum, (const int32_t*)p.inst_base,
                                   (const int32_t*)p.rank_base, out_replica, out_rank, out_offset,
                                   out_gate, local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S,
-                                  cumq, srcpre, n_inflight, acc_clear, chunk0));
+                                  cumq, srcpre, n_inflight, acc_clear, chunk0,
+                                  from_lambda ? (const int32_t*)ws_lambda(c, ws) : (const int32_t*)nullptr));
   count_launch(c);
   return UEP_OK;
 }
@@ -611,15 +669,15 @@ int init_remap_kernels() {
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& p, int32_t* out_replica,
                   int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
                   bool pdl, bool local, int32_t* n_inflight, int32_t* acc_clear, int chunk0,
-                  int n_launch, bool src_aware) {
+                  int n_launch, bool src_aware, bool from_lambda) {
   if (c->S == 0) return UEP_OK;
   if (c->cfg.gate_dtype == UEP_GATE_BF16 && gate)
     return launch_lookup_t<uint16_t>(c, static_cast<const uint16_t*>(gate), p, out_replica, out_rank,
                                      out_offset, static_cast<uint16_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear,
-                                     chunk0, n_launch, src_aware);
+                                     chunk0, n_launch, src_aware, from_lambda);
   return launch_lookup_t<uint32_t>(c, static_cast<const uint32_t*>(gate), p, out_replica, out_rank,
                                    out_offset, static_cast<uint32_t*>(out_gate), ws, s, pdl, local, n_inflight, acc_clear,
-                                   chunk0, n_launch, src_aware);
+                                   chunk0, n_launch, src_aware, from_lambda);
 }
 
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& p,

@@ -199,8 +199,7 @@ void uep_destroy(uep_ctx* ctx) {
 size_t uep_workspace_bytes(const uep_ctx* ctx) {
   const Ctx* c = reinterpret_cast<const Ctx*>(ctx);
   if (!c) return 0;
-  return (size_t)kWsHeaderBytes + ws_table_bytes(c) + 2 * ws_prefix_bytes(c) + ws_packed_bytes(c) +
-         sizeof(int32_t) * ws_reroute_ints(c);
+  return ws_lambda_offset(c) + ws_lambda_bytes(c);
 }
 
 int uep_workspace_init(const uep_ctx* ctx, void* ws, void* stream) {
@@ -397,10 +396,11 @@ int uep_shard_rows(const uep_ctx* ctx, int32_t shard, int32_t n_shards, size_t* 
   ShardGeom g;
   int rc = shard_geom(c, shard, n_shards, &g);
   if (rc != UEP_OK) return rc;
-  // chunk ch's counts live in row ch + 1 of the prefix table (row 0 stays zero)
+  // the shard's rows of Lambda[R][E_pad] (one row per source rank: lambda_{r,e})
   const size_t row = sizeof(int32_t) * (size_t)c->E_pad;
-  *ws_byte_offset = (size_t)kWsHeaderBytes + ws_table_bytes(c) + row * (size_t)(g.chunk0 + 1);
-  *n_bytes = row * (size_t)g.chunks;
+  const int rps = c->cfg.R / n_shards;
+  *ws_byte_offset = ws_lambda_offset(c) + row * (size_t)(shard * rps);
+  *n_bytes = row * (size_t)rps;
   return UEP_OK;
 }
 
@@ -413,9 +413,12 @@ int uep_shard_count(const uep_ctx* ctx, int32_t shard, int32_t n_shards,
   if (rc != UEP_OK) return rc;
   if (c->S == 0) return UEP_OK;
   if (!topk_ids_local || !aligned16(topk_ids_local)) return UEP_ERR_INVALID_ARG;
-  return launch_rank(c, static_cast<const int32_t*>(virtual_base(topk_ids_local, g.slot0, 4)), ws,
-                     static_cast<cudaStream_t>(stream), /*local=*/true, g.chunk0, g.chunks,
-                     /*with_prefix=*/false);
+  rc = launch_rank(c, static_cast<const int32_t*>(virtual_base(topk_ids_local, g.slot0, 4)), ws,
+                   static_cast<cudaStream_t>(stream), /*local=*/true, g.chunk0, g.chunks,
+                   /*with_prefix=*/false);
+  const int rps = c->cfg.R / n_shards;
+  if (rc == UEP_OK) rc = launch_shard_rows(c, ws, static_cast<cudaStream_t>(stream), shard * rps, rps);
+  return rc;
 }
 
 int uep_shard_finish(const uep_ctx* ctx, int32_t shard, int32_t n_shards, const void* gate_local,
@@ -438,19 +441,19 @@ int uep_shard_finish(const uep_ctx* ctx, int32_t shard, int32_t n_shards, const 
   }
   const int rps = c->cfg.R / n_shards;
   if (n_inflight) UEP_CUDA_TRY(cudaMemsetAsync(n_inflight + shard * rps, 0, sizeof(int32_t) * rps, s));
-  rc = launch_prefix(c, ws, s, /*local=*/true);
-  // lambda_e = totals row of the scanned table; the planner publishes it as expert_count
-  int32_t* totals = ws_prefix(c, ws) + (size_t)c->l_chunks * c->E_pad;
-  // planner and lookup programmatically dependent on their predecessors (the lookup reads the prefix
-  // rows after its wait, i.e. after the planner, which itself waited for prefix_kernel)
-  if (rc == UEP_OK) rc = launch_plan(c, nullptr, *plan, s, /*pdl=*/true, 1, totals, expert_count);
+  // lambda_e = the column sums of the gathered Lambda: the planner adds them up itself and publishes
+  // expert_count; planner and lookup are programmatically dependent on their predecessors.  The lookup
+  // derives the GLOBAL rank base of each of its chunks from Lambda and its own chunk counts in its
+  // prologue, beside the planner: no kernel between the exchange and the planner
+  rc = launch_plan(c, nullptr, *plan, s, /*pdl=*/true, 1, ws_lambda(c, ws), expert_count, c->cfg.R, c->E_pad);
   const size_t gb = c->cfg.gate_dtype == UEP_GATE_BF16 ? 2 : 4;
   if (rc == UEP_OK)
     rc = launch_lookup(c, virtual_base(gate_local, g.slot0, gb), *plan,
                        static_cast<int32_t*>(virtual_base(out_replica_local, g.slot0, 4)),
                        static_cast<int32_t*>(virtual_base(out_rank_local, g.slot0, 4)),
                        static_cast<int32_t*>(virtual_base(out_offset_local, g.slot0, 4)), out_gate, ws, s, /*pdl=*/true,
-                       /*local=*/true, n_inflight, nullptr, g.chunk0, g.chunks, /*src_aware=*/false);
+                       /*local=*/true, n_inflight, nullptr, g.chunk0, g.chunks, /*src_aware=*/false,
+                       /*from_lambda=*/true);
   return rc;
 }
 

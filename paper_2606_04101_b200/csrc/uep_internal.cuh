@@ -90,17 +90,22 @@ inline int prefer_max_smem(K kernel) {
 int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws, cudaStream_t s,
                      bool red = false);
 int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
-                bool pdl = false, int n_inst = 1, int32_t* acc = nullptr, int32_t* count_out = nullptr);
+                bool pdl = false, int n_inst = 1, int32_t* acc = nullptr, int32_t* count_out = nullptr,
+                int acc_rows = 1, int acc_pitch = 0);
 // uep_remap = launch_rank (plan-independent: stable rank of every slot inside its chunk, packed
 // with the expert id into the workspace) + launch_lookup (plan-dependent: cumulative-quota lookup).
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local = false,
                 int chunk0 = 0, int n_launch = -1, bool with_prefix = true);
 int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local, bool pdl = false);
+// token-sharded path: the shard's rows of Lambda[R][E_pad] from its chunks' counts (after the exchange
+// the planner sums the matrix's columns and the lookup derives its chunk bases from it: no prefix kernel)
+int launch_shard_rows(const Ctx* c, void* ws, cudaStream_t s, int rank0, int n_ranks);
 int launch_reroute(const Ctx* c, const uep_plan_out& plan, int32_t* n_inflight, void* ws, cudaStream_t s);
 int launch_lookup(const Ctx* c, const void* gate, const uep_plan_out& plan, int32_t* out_replica,
                   int32_t* out_rank, int32_t* out_offset, void* out_gate, void* ws, cudaStream_t s,
                   bool pdl = false, bool local = false, int32_t* n_inflight = nullptr,
-                  int32_t* acc_clear = nullptr, int chunk0 = 0, int n_launch = -1, bool src_aware = true);
+                  int32_t* acc_clear = nullptr, int chunk0 = 0, int n_launch = -1, bool src_aware = true,
+                  bool from_lambda = false);
 int launch_remap(const Ctx* c, const int32_t* ids, const void* gate, const uep_plan_out& plan,
                  int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
                  void* ws, cudaStream_t s);
@@ -199,6 +204,14 @@ inline int32_t* ws_packed(const Ctx* c, void* ws) {      // [S] packed (expert, 
 inline int32_t* ws_reroute(const Ctx* c, void* ws) {     // source-aware split tables (uep_remap_local)
   return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + kWsHeaderBytes + ws_table_bytes(c) +
                                     2 * ws_prefix_bytes(c) + ws_packed_bytes(c));
+}
+inline size_t ws_lambda_offset(const Ctx* c) {           // Lambda[R][E_pad]: the count matrix of the token-sharded path
+  return ((size_t)kWsHeaderBytes + ws_table_bytes(c) + 2 * ws_prefix_bytes(c) + ws_packed_bytes(c) +
+          sizeof(int32_t) * ws_reroute_ints(c) + 255) & ~(size_t)255;
+}
+inline size_t ws_lambda_bytes(const Ctx* c) { return c->l_cpg ? sizeof(int32_t) * (size_t)c->cfg.R * c->E_pad : 0; }
+inline int32_t* ws_lambda(const Ctx* c, void* ws) {
+  return reinterpret_cast<int32_t*>(static_cast<unsigned char*>(ws) + ws_lambda_offset(c));
 }
 
 }  // namespace uep
