@@ -72,6 +72,59 @@ def test_world_size_2_gloo():
     assert shard.total_units(6, world) == 12
 
 
+def _lambda_worker(rank, world, port, q):
+    """Two ranks run the HOST side of the token-sharded path: each counts its own
+    source ranks' token blocks (here with the oracle, standing in for uep_shard_count), the rows of
+    Lambda[R][E_pad] are all-gathered in place, and every rank derives lambda_e and the global rank
+    base of every source rank from the gathered matrix."""
+    import numpy as np
+    import oracle
+    from paper_2606_04101_b200 import synth
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    T, k, E, R = 4096, 2, 13, 8                       # E_pad = 16
+    E_pad = (E + 3) // 4 * 4
+    ids = synth.zipf_topk_ids(T, k, E, 1.2, 7).numpy()
+    ids[5, 0] = -1                                     # an invalid id is in no row
+    rps, block = R // world, T // R
+    off0 = 4096                                        # byte offset of Lambda inside a workspace-shaped buffer
+    nb = rps * E_pad * 4
+    ws = torch.full((off0 + world * nb + 64,), 0xCD, dtype=torch.uint8)
+    mine = np.zeros((rps, E_pad), np.int32)
+    for j in range(rps):
+        r = rank * rps + j
+        mine[j, :E], _ = oracle.histogram(ids[r * block:(r + 1) * block], E)
+    ws[off0 + rank * nb: off0 + (rank + 1) * nb] = torch.from_numpy(mine.reshape(-1).view(np.uint8).copy())
+    shard.exchange_counts(ws, off0, nb, rank, world)
+    dist.barrier()
+    Lam = ws[off0: off0 + world * nb].numpy().view(np.int32).reshape(R, E_pad)
+    lam, bad = oracle.histogram(ids, E)
+    ok_tot = bool((Lam[:, :E].sum(axis=0) == lam).all()) and bad == 1
+    base = np.cumsum(Lam[:, :E], axis=0) - Lam[:, :E]                      # global rank base of (source rank, expert)
+    flat = ids.reshape(-1)
+    ok_base = all(int(base[r, e]) == int((flat[:r * block * k] == e).sum()) for r in range(R) for e in range(E))
+    q.put((rank, ok_tot, ok_base, nb, Lam.copy()))
+    dist.destroy_process_group()
+
+
+def test_lambda_rows_exchange_world_2():
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    ps = [ctx.Process(target=_lambda_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in ps:
+        p.start()
+    res = sorted((q.get(timeout=120) for _ in range(world)), key=lambda x: x[0])
+    for p in ps:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    import numpy as np
+    assert all(r[1] and r[2] for r in res)
+    assert res[0][3] == 4 * 16 * 8 // 2                                    # 4 * E_pad * R / G bytes per GPU
+    assert np.array_equal(res[0][4], res[1][4])                            # every rank holds the same matrix
+
+
 def test_single_process_paths():
     ws = torch.arange(64, dtype=torch.uint8)
     shard.exchange_counts(ws, 16, 32, 0, 1)                               # world 1: a no-op
