@@ -420,11 +420,13 @@ def run_token_sharded(c, rig, world, rank, device, stream, reps):
                     "of the plan latency), max over ranks; `value` is the weak-scaling instance-sharded number"}
 
 
-def roof(name, nbytes, dur_us, peak_gbs, peak_src, traffic, what):
+def roof(name, nbytes, dur_us, peak_gbs, peak_src, traffic, what, parts=None):
     a = nbytes / (dur_us * 1e-6) / 1e9 if dur_us > 0 else 0.0
+    parts = parts or [name]
+    tr = sum(traffic[k] for k in parts) if all(k in traffic for k in parts) else None
     return {"kernel": name, "bound": "hbm", "achieved": round(a, 1), "peak": peak_gbs, "unit": "GB/s",
             "frac": round(a / peak_gbs, 4), "frac_of_nominal_8TBs": round(a / 8000.0, 4),
-            "traffic": traffic.get(name), "bytes_per_launch": int(nbytes), "us_per_launch": round(dur_us, 2),
+            "traffic": tr, "bytes_per_launch": int(nbytes), "us_per_launch": round(dur_us, 2),
             "peak_source": peak_src, "achieved_is": what}
 
 
@@ -547,16 +549,17 @@ def run_uep(args):
     bytes_pack = [(n_grp[i] + n_rep[i]) * B for i in range(n_pack)]
     us = lambda ms, n: ms * 1e3 / n
     traffic, traffic_src = load_traffic(args)
-    rf = lambda name, nb, t, what: roof(name, nb, t, peak_gbs, peak_src, traffic, what)
+    rf = lambda name, nb, t, what, parts=None: roof(name, nb, t, peak_gbs, peak_src, traffic, what, parts)
 
     pack_us = us(pack_ms, n_pack)
     r_pack = rf("pack_kernel", sum(bytes_pack) / max(n_pack, 1), pack_us,
                 "algorithmic bytes per second; the peak is a torch copy_ measurement, so a streaming kernel can "
                 "read slightly above 1.0 (also given against the nominal 8 TB/s)")
     rooflines = [r_pack,
-                 rf("uep_remap (rank_kernel+prefix_kernel+lookup_kernel)", bytes_remap, us(remap_ms, n_inst), ALGO),
+                 rf("uep_remap (rank_kernel+prefix_kernel+lookup_kernel)", bytes_remap, us(remap_ms, n_inst), ALGO,
+                    ["rank_kernel", "prefix_kernel", "lookup_kernel"]),
                  rf("lookup_kernel", bytes_remap, us(lookup_ms, n_inst), ALGO),
-                 rf("rank_kernel+prefix_kernel", 8 * S, us(rank_ms, n_inst), ALGO),
+                 rf("rank_kernel+prefix_kernel", 8 * S, us(rank_ms, n_inst), ALGO, ["rank_kernel", "prefix_kernel"]),
                  rf("hist_kernel", bytes_hist, us(hist_ms, n_inst), ALGO)]
     red_bytes = statistics.mean(2 * (n_grp[i] + n_rep[i]) for i in range(n_red)) * g_elems * 4
     result = {
