@@ -202,7 +202,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
             const int32_t* __restrict__ g_rexp, uep_plan_out out, int E, int R, int n_slot, int M,
             int P, int u_min, int beta_num, int beta_den, int strict_i, int S_total, int n_bufs,
             int log_cap, int levels, const int32_t* __restrict__ acc, int32_t* __restrict__ count_out,
-            int acc_rows, int acc_pitch) {
+            int acc_rows, int acc_pitch, int32_t* __restrict__ zero_ptr, int zero_n) {
   // acc != nullptr (uep_balance): lambda_e comes from the histogram's accumulator in the workspace
   // (acc_rows == 1), or is the column sum of the gathered count matrix Lambda[acc_rows][acc_pitch] of
   // the token-sharded path ("every rank solves the same plan" from the exchanged counts)
@@ -235,6 +235,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     sm.rexp[e] = g_rexp[e];
   }
   for (int r = tid; r <= R; r += kPlanThreads) sm.roff[r] = g_roff[r];
+  if (acc_rows > 1) for (int e = tid; e < E; e += kPlanThreads) sm.lam[e] = 0;
+  // (token-sharded path: the per-source in-flight counters the lookup behind this kernel adds to;
+  // it does so only after its own wait for this kernel, so clearing them anywhere in here is in time)
+  if (blockIdx.x == 0) for (int i = tid; i < zero_n; i += kPlanThreads) zero_ptr[i] = 0;
   __syncthreads();
   pdl_wait();                      // the histogram (preceding kernel) is complete
   // phase 1: lambda_e into shared memory, and line 2 (l_r) straight from global memory with
@@ -250,11 +254,16 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
       sm.ell[tid] = s;
     }
   } else {                         // Alg. 1 line 2 in full: lambda_e = sum_r lambda_{r,e}
-    for (int e = tid; e < E; e += kPlanThreads) {
+    // (kPlanThreads / Ecap threads per expert, each over a strided part of the rows with independent
+    // loads, combined in shared memory: sm.lam was cleared before the wait)
+    int ecap = 32;
+    while (ecap < E) ecap <<= 1;
+    const int parts = kPlanThreads / ecap, e = tid % ecap, part = tid / ecap;   // ecap <= UEP_MAX_E <= kPlanThreads
+    if (e < E) {
       int s = 0;
-#pragma unroll 8
-      for (int r = 0; r < acc_rows; ++r) s += __ldcg(acc + (size_t)r * acc_pitch + e);
-      sm.lam[e] = s;
+#pragma unroll 16
+      for (int r = part; r < acc_rows; r += parts) s += __ldcg(acc + (size_t)r * acc_pitch + e);
+      atomicAdd(&sm.lam[e], s);
     }
     __syncthreads();
     if (tid < R) {
@@ -675,7 +684,7 @@ constexpr size_t kLogBudget = 128 * 1024;     // shared memory for the accept lo
 template <int RPL>
 static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out& plan,
                          cudaStream_t s, bool pdl, int n_inst, const int32_t* acc, int32_t* count_out,
-                         int acc_rows, int acc_pitch) {
+                         int acc_rows, int acc_pitch, int32_t* zero_ptr, int zero_n) {
   const uep_config& g = c->cfg;
   const int levels = 6;                                        // 63 nodes over kPlanCluster CTAs
   const int cluster = c->plan_cluster;
@@ -714,19 +723,20 @@ static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out&
                                   (const int32_t*)c->d_rexp, plan, g.E, g.R, g.n_slot, c->M, c->P,
                                   g.u_min, g.beta_num, g.beta_den,
                                   g.floor_mode == UEP_FLOOR_STRICT ? 1 : 0, c->S, n_bufs, log_cap,
-                                  levels, acc, count_out, acc_rows, acc_pitch));
+                                  levels, acc, count_out, acc_rows, acc_pitch, zero_ptr, zero_n));
   count_launch(c);
   return UEP_OK;
 }
 
 int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
-                bool pdl, int n_inst, int32_t* acc, int32_t* count_out, int acc_rows, int acc_pitch) {
+                bool pdl, int n_inst, int32_t* acc, int32_t* count_out, int acc_rows, int acc_pitch,
+                int32_t* zero_ptr, int zero_n) {
   const int R = c->cfg.R;
   if (n_inst <= 0) return UEP_OK;
-  if (R <= 32) return launch_plan_t<1>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch);
-  if (R <= 64) return launch_plan_t<2>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch);
-  if (R <= 128) return launch_plan_t<4>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch);
-  return launch_plan_t<8>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch);
+  if (R <= 32) return launch_plan_t<1>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch, zero_ptr, zero_n);
+  if (R <= 64) return launch_plan_t<2>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch, zero_ptr, zero_n);
+  if (R <= 128) return launch_plan_t<4>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch, zero_ptr, zero_n);
+  return launch_plan_t<8>(c, count, plan, s, pdl, n_inst, acc, count_out, acc_rows, acc_pitch, zero_ptr, zero_n);
 }
 
 template <int RPL>

@@ -188,9 +188,8 @@ prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG) {
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(UEP_MAX_E)
 shard_rows_kernel(int E_pad, int cpg, int rank0, const int32_t* __restrict__ counts, int32_t* __restrict__ lambda) {
-  pdl_wait();                                   // rank_kernel complete
-  pdl_trigger();                                // (one GPU: the planner is next; the lookup behind it reads only
-                                                //  LOWER shards' rows of Lambda before its own wait)
+  pdl_wait();                                   // rank_kernel complete.  (No early trigger: on one GPU the planner
+                                                // is next, and the lookup behind IT reads Lambda in its prologue)
   const int r = rank0 + (int)blockIdx.x;
   for (int e = threadIdx.x; e < E_pad; e += blockDim.x) {
     int s = 0;
@@ -474,17 +473,16 @@ lookup_kernel(const int32_t* __restrict__ packed, const GateT* __restrict__ gate
     if (tid == kRemapThreads - 1) el[E] = pre + inc;              // valid slots in this chunk (E < kRemapThreads or == : tid 511 holds the total)
   }
   __syncthreads();
-  // token-sharded path: global rank of the chunk's first slot of e = the slots of e on the source
-  // ranks of LOWER shards (their rows of the gathered Lambda, complete before the planner in front of
-  // this kernel started) + those in this shard's earlier chunks (its own counts, complete since
-  // rank_kernel; this shard's own rows of Lambda may still be being written on one GPU); no prefix kernel
+  // token-sharded path: global rank of the chunk's first slot of e = the slots of e on lower source
+  // ranks (rows of the gathered Lambda; complete before the planner in front of this kernel started:
+  // neither the all-gather nor shard_rows_kernel triggers early) + those in the source rank's earlier
+  // chunks (own counts); no prefix kernel.  (Summing the counts of ALL earlier chunks of the shard
+  // instead — up to 292 dependent L2 loads per thread on one GPU — took longer than the planner.)
   int p_lam = 0;
   if (LOCAL && lambda != nullptr && tid < E) {
-    const int r_lo = chunk0 / cpg;
 #pragma unroll 8
-    for (int r = 0; r < r_lo; ++r) p_lam += __ldcg(lambda + (size_t)r * E_pad + tid);
-#pragma unroll 8
-    for (int ch = chunk0; ch < c; ++ch) p_lam += __ldcg(counts + (size_t)ch * E_pad + tid);
+    for (int r = 0; r < grp; ++r) p_lam += __ldcg(lambda + (size_t)r * E_pad + tid);
+    for (int q = 0; q < sub; ++q) p_lam += __ldcg(counts + (size_t)(grp * cpg + q) * E_pad + tid);
   }
   if (has_gate) {                                            // gates into (expert, rank) order
 #pragma unroll

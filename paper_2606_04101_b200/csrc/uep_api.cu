@@ -440,12 +440,12 @@ int uep_shard_finish(const uep_ctx* ctx, int32_t shard, int32_t n_shards, const 
     return launch_plan(c, expert_count, *plan, s);
   }
   const int rps = c->cfg.R / n_shards;
-  if (n_inflight) UEP_CUDA_TRY(cudaMemsetAsync(n_inflight + shard * rps, 0, sizeof(int32_t) * rps, s));
   // lambda_e = the column sums of the gathered Lambda: the planner adds them up itself and publishes
   // expert_count; planner and lookup are programmatically dependent on their predecessors.  The lookup
   // derives the GLOBAL rank base of each of its chunks from Lambda and its own chunk counts in its
   // prologue, beside the planner: no kernel between the exchange and the planner
-  rc = launch_plan(c, nullptr, *plan, s, /*pdl=*/true, 1, ws_lambda(c, ws), expert_count, c->cfg.R, c->E_pad);
+  rc = launch_plan(c, nullptr, *plan, s, /*pdl=*/true, 1, ws_lambda(c, ws), expert_count, c->cfg.R, c->E_pad,
+                   n_inflight ? n_inflight + shard * rps : nullptr, n_inflight ? rps : 0);
   const size_t gb = c->cfg.gate_dtype == UEP_GATE_BF16 ? 2 : 4;
   if (rc == UEP_OK)
     rc = launch_lookup(c, virtual_base(gate_local, g.slot0, gb), *plan,

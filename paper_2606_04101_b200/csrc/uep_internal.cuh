@@ -91,7 +91,7 @@ int launch_histogram(const Ctx* c, const int32_t* ids, int32_t* count, void* ws,
                      bool red = false);
 int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cudaStream_t s,
                 bool pdl = false, int n_inst = 1, int32_t* acc = nullptr, int32_t* count_out = nullptr,
-                int acc_rows = 1, int acc_pitch = 0);
+                int acc_rows = 1, int acc_pitch = 0, int32_t* zero_ptr = nullptr, int zero_n = 0);
 // uep_remap = launch_rank (plan-independent: stable rank of every slot inside its chunk, packed
 // with the expert id into the workspace) + launch_lookup (plan-dependent: cumulative-quota lookup).
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local = false,
