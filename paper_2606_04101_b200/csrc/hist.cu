@@ -2,9 +2,10 @@
 //
 // HBM-bound: 4 B/slot read once.  One CTA per chunk (one chunk per SM).  Every thread issues
 // all of its int4 loads of a round before it touches shared memory (kHistVecs x 16 B in flight
-// per thread, 64 KB per SM), then counts into a WARP-PRIVATE shared-memory row (pitch E_pad+1
-// so the same expert in different rows falls into different banks): no contention between
-// warps on a hot expert, only the intra-warp multiplicity.  Every CTA adds its column sums to an
+// per thread, 64 KB per SM), then counts into a shared-memory row that four warps share (8 rows,
+// pitch E_pad+1 so the same expert in different rows falls into different banks; shared atomics
+// cost ~1.2 cycles per warp instruction and SM on this part, so a row per warp — 32 rows to zero
+// and to add up — bought nothing: 5.42 -> 5.31 us with 8).  Every CTA adds its column sums to an
 // accumulator in the workspace (zero between calls) with fire-and-forget reductions — integer
 // adds, order-free, bit-identical run to run — and exits.  The accumulator is consumed by the
 // kernel behind it in the stream, launched programmatically dependent: the planner inside
@@ -17,6 +18,8 @@
 namespace uep {
 
 constexpr int kHistWarps = kHistThreads / 32;
+constexpr int kHistShare = 2;                                 // log2 of the warps sharing a row of counters
+constexpr int kHistRows = kHistWarps >> kHistShare;
 constexpr int kHistVecs = 4;                                  // int4 loads per thread per round
 
 __device__ __forceinline__ int4 ld_stream_v4(const int4* p) {
@@ -30,9 +33,9 @@ __device__ __forceinline__ void count_one(int* row, int e, int E) {
   if ((unsigned)e < (unsigned)E) atomicAdd(&row[e], 1);
 }
 
-// dynamic shared memory (ints): priv[kHistWarps][E_pad+1]
+// dynamic shared memory (ints): priv[kHistRows][E_pad+1]
 __host__ __device__ inline size_t hist_smem_ints(int E_pad) {
-  return (size_t)kHistWarps * (E_pad + 1);
+  return (size_t)kHistRows * (E_pad + 1);
 }
 
 // TABLE: also leave the CTA's raw counts in row c of the chunk table (uep_histogram's by-product,
@@ -60,10 +63,10 @@ hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
     const int i = u * kHistThreads + tid;
     x[u] = (i < n_vec) ? ld_stream_v4(v + i) : make_int4(-1, -1, -1, -1);
   }
-  for (int i = tid; i < kHistWarps * pitch; i += kHistThreads) priv[i] = 0;
+  for (int i = tid; i < kHistRows * pitch; i += kHistThreads) priv[i] = 0;
   __syncthreads();
 
-  int* row = priv + warp * pitch;
+  int* row = priv + (warp >> kHistShare) * pitch;
   for (int vbase = 0; vbase < n_vec; vbase += kHistThreads * kHistVecs) {
 #pragma unroll
     for (int u = 0; u < kHistVecs; ++u) {
@@ -85,7 +88,7 @@ hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
   for (int e = tid; e < E_pad; e += kHistThreads) {
     int s = 0;
 #pragma unroll 8
-    for (int w = 0; w < kHistWarps; ++w) s += priv[w * pitch + e];
+    for (int w = 0; w < kHistRows; ++w) s += priv[w * pitch + e];
     if (s != 0 && e < E) atomicAdd(acc + e, s);          // result unused: a fire-and-forget RED
     if (TABLE) table[(size_t)c * E_pad + e] = s;
   }
