@@ -1105,3 +1105,62 @@ def test_balance_failure_mid_chain_leaves_stream_and_workspace_usable():
     assert np.array_equal(count.cpu().numpy(), lam)
     o = oracle_chain(ids, None, E, R, ns, um)
     assert np.array_equal(rep.cpu().numpy(), o[2]) and np.array_equal(off.cpu().numpy(), o[4])
+
+
+def test_many_replays_with_changing_ids_on_one_workspace_full_size():
+    """The lookup reads rank_kernel's outputs (packed ranks, chunk counts) in its prologue, before its
+    griddepcontrol.wait: that rests on rank_kernel's grid being complete (prefix_kernel waits for it
+    before it lets the lookup start) and on loads that bypass L1.  Stress it: ONE graph of three
+    different calls (uep_balance, uep_remap, uep_balance) on ONE workspace at the DeepSeek-V3 shape,
+    replayed six times with the ids and gates rewritten before every replay, each result checked
+    against the oracle — a stale read of the previous replay's ranks or counts would show."""
+    c = synth.CONFIGS["dsv3_prefill"]
+    T, k, E, R, ns, um = c["T"], c["k"], c["E"], c["R"], c["n_slot"], c["u_min"]
+    ctx = binding.Context(T, k, E, R, ns, um)
+    ws = ctx.new_workspace()
+    d_ids = [torch.zeros((T, k), dtype=torch.int32, device=DEV) for _ in range(3)]
+    d_gate = [torch.zeros((T, k), dtype=torch.float32, device=DEV) for _ in range(3)]
+    outs = []
+    for b in range(3):
+        rep, rnk, off, og = ctx.new_outputs(d_gate[b])
+        outs.append(dict(count=torch.zeros(E, dtype=torch.int32, device=DEV), plan=ctx.new_plan(), rep=rep, rnk=rnk,
+                         off=off, og=og))
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+
+    def run_all():
+        for b in (0, 1, 2):
+            o = outs[b]
+            if b == 1:                                   # remap alone, on the plan of its own ids
+                ctx.uep_histogram(d_ids[b], o["count"], ws)
+                ctx.uep_plan(o["count"], o["plan"], ws)
+                ctx.uep_remap(d_ids[b], d_gate[b], o["plan"], o["rep"], o["rnk"], o["off"], o["og"], ws)
+            else:
+                ctx.uep_balance(d_ids[b], d_gate[b], o["count"], o["plan"], o["rep"], o["rnk"], o["off"], o["og"],
+                                [], [], ws)
+
+    with torch.cuda.stream(stream):
+        run_all()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            run_all()
+    torch.cuda.synchronize()
+    for it in range(6):
+        host = []
+        for b in range(3):
+            ids = synth.zipf_topk_ids(T, k, E, 0.6 + 0.25 * ((it + b) % 5), 5000 + 10 * it + b, device=DEV)
+            gate = synth.gates_uniform_renorm(T, k, 70 + 10 * it + b, device=DEV)
+            d_ids[b].copy_(ids); d_gate[b].copy_(gate)
+            host.append((ids.cpu(), gate.cpu()))
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        for b in range(3):
+            lam, p, rep, rnk, off, og = oracle_chain(host[b][0], host[b][1], E, R, ns, um)
+            o = outs[b]
+            assert np.array_equal(o["count"].cpu().numpy(), lam), (it, b)
+            assert np.array_equal(o["rep"].cpu().numpy(), rep), (it, b)
+            assert np.array_equal(o["rnk"].cpu().numpy(), rnk), (it, b)
+            assert np.array_equal(o["off"].cpu().numpy(), off), (it, b)
+            nv = int(p.rank_base[-1])
+            assert np.array_equal(o["og"].cpu().view(torch.int32).numpy().view(np.uint32)[:nv], og[:nv]), (it, b)
