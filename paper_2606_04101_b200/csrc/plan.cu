@@ -273,26 +273,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     }
   }
   __syncthreads();
-  // phase 2.  Every warp reduces the l_r itself (no second barrier for the bounds):
-  // line 3 (S3): tau_lo = floor(beta * ceil(mean)), tau_hi = max l_r; S < 2^24, so 32-bit sums are
-  // exact, and 32-bit divisions where the operands fit (a 64-bit division is a ~300-cycle
-  // subroutine on this dependent path)
-  {
-    int sum = 0, mx = 0;
-    for (int r = lane; r < R; r += 32) { const int v = sm.ell[r]; sum += v; mx = max(mx, v); }
-    sum = __reduce_add_sync(kFull, sum);
-    mx = __reduce_max_sync(kFull, mx);
-    const unsigned mean_ceil = ((unsigned)sum + (unsigned)R - 1u) / (unsigned)R;
-    const unsigned long long prod = (unsigned long long)mean_ceil * (unsigned long long)beta_num;
-    const unsigned long long tl = (prod >> 32) == 0ull ? (unsigned long long)((unsigned)prod / (unsigned)beta_den)
-                                                       : prod / (unsigned long long)beta_den;
-    if (tid == 0) {
-      sm.lo = sm.lo0 = (int)min(tl, (unsigned long long)0x7fffffff);
-      sm.hi = sm.hi0 = mx;
-      sm.s_valid = sum;
-      sm.n_probes = 0; sm.n_log = 0; sm.log_buf = -1;
-    }
-  }
+  // phase 2
   // rank order (S5): visit position of rank r = number of ranks that come before it (l desc, id
   // asc), and in the same pass the start of its experts in the flat visit list = number of experts
   // of those ranks (no scan).  gsz threads per rank (a power of two), each over a strided part of
@@ -333,6 +314,26 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     sm.wpos[e] = cnt;
   }
   __syncthreads();
+  // line 3 (S3), by the last warp alone beside the scatter below (it has no expert to place unless
+  // E > kPlanThreads - 32; on every warp's path in phase 2 these two divisions cost ~950 cycles):
+  // tau_lo = floor(beta * ceil(mean)), tau_hi = max l_r; S < 2^24, so 32-bit sums are exact, and
+  // 32-bit divisions where the operands fit (a 64-bit division is a ~300-cycle subroutine)
+  if (warp == kPlanWarps - 1) {
+    int sum = 0, mx = 0;
+    for (int r = lane; r < R; r += 32) { const int v = sm.ell[r]; sum += v; mx = max(mx, v); }
+    sum = __reduce_add_sync(kFull, sum);
+    mx = __reduce_max_sync(kFull, mx);
+    const unsigned mean_ceil = ((unsigned)sum + (unsigned)R - 1u) / (unsigned)R;
+    const unsigned long long prod = (unsigned long long)mean_ceil * (unsigned long long)beta_num;
+    const unsigned long long tl = (prod >> 32) == 0ull ? (unsigned long long)((unsigned)prod / (unsigned)beta_den)
+                                                       : prod / (unsigned long long)beta_den;
+    if (lane == 0) {
+      sm.lo = sm.lo0 = (int)min(tl, (unsigned long long)0x7fffffff);
+      sm.hi = sm.hi0 = mx;
+      sm.s_valid = sum;
+      sm.n_probes = 0; sm.n_log = 0; sm.log_buf = -1;
+    }
+  }
   // phase 3: flat visit list (ranks in visit order, each with its experts in visit order), and the
   // emit state cleared here, off the path between the last probe and the plan's first store (no
   // probe touches it): per-expert replica counts, first log entry, staged phys_count, and by CTA 0
@@ -609,8 +610,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     if (lane == 0) { sm.red_fan[warp] = fan_mx; sm.red_grp[warp] = n_grp; }
   }
   __syncthreads();
-  // Phase C: the replicas' CSR entries (S11: acceptance order) and, a thread per rank, the receive
-  // layout inside every rank (S13)
+  // Phase C: the replicas' CSR entries (S11: acceptance order) and, by the last warp, the receive layout
 #pragma unroll
   for (int j = 0; j < kLogPer; ++j) {
     const int l = tid * kLogPer + j;
@@ -627,26 +627,45 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   for (int i = E + n_log + tid; i < E + R * n_slot; i += kPlanThreads) {   // unused CSR tail
     o.inst_rank[i] = -1; o.inst_phys[i] = -1; o.inst_cum[i] = 0; o.inst_base[i] = 0;
   }
-  if (tid < R) {                   // receive layout of rank tid (S13): exclusive prefix over its P physical slots
-    int load = 0;
-    for (int x = 0; x < P; ++x) {
-      const int cnt = pc[tid * P + x];
-      o.phys_base[tid * P + x] = load;
-      if (pc_in_smem) { o.phys_count[tid * P + x] = cnt; pc[tid * P + x] = load; }
-      load += cnt;
+  if (warp == kPlanWarps - 1) {    // (the last warp: it has log entries above only when more than 960 transfers were accepted)
+    // receive layout (S13): per rank the exclusive prefix over its P physical slots (lane t owns the
+    // consecutive ranks t*RW ..), then the exclusive prefix over ranks and the maximum — beside the
+    // other warps' CSR stores, so that the last phase is the instance bases alone
+    const int RW = (R + 31) >> 5;
+    int tot = 0, mxl = 0;
+    for (int q = 0; q < RW; ++q) {
+      const int r = lane * RW + q;
+      if (r < R) {
+        int load = 0;
+        for (int x = 0; x < P; ++x) {
+          const int cnt = pc[r * P + x];
+          o.phys_base[r * P + x] = load;
+          if (pc_in_smem) { o.phys_count[r * P + x] = cnt; pc[r * P + x] = load; }
+          load += cnt;
+        }
+        o.rank_load[r] = load;
+        sm.rload[r] = load;
+        tot += load;
+        mxl = max(mxl, load);
+      }
     }
-    o.rank_load[tid] = load;
-    sm.rload[tid] = load;
+    const int inc = warp_incl_scan(tot, lane);
+    int base = inc - tot;
+    for (int q = 0; q < RW; ++q) {
+      const int r = lane * RW + q;
+      if (r < R) { o.rank_base[r] = base; base += sm.rload[r]; }
+    }
+    mxl = __reduce_max_sync(kFull, mxl);
+    if (lane == 31) { o.rank_base[R] = inc; o.scalars[UEP_SC_MAX_LOAD] = mxl; }
   }
-  if (tid == kPlanThreads - 32) {  // (a lane of the last warp: no rank to lay out unless R > kPlanThreads - 32)
+  if (tid == kPlanThreads - 64) {  // (a lane of the last warp but one)
     int max_fan = 0, n_groups = 0;
     for (int w = 0; w < kPlanWarps; ++w) { max_fan = max(max_fan, sm.red_fan[w]); n_groups += sm.red_grp[w]; }
     o.scalars[UEP_SC_MAX_FANOUT] = max_fan;
     o.scalars[UEP_SC_N_GROUPS] = n_groups;
   }
   __syncthreads();
-  // Phase D: inst_base = offset of each instance's first token in its rank's receive buffer (S13),
-  // and by the last warp the exclusive prefix over ranks
+  // Phase D: inst_base = offset of each instance's first token in its rank's receive buffer (S13)
   {
     const int* pb = pc_in_smem ? pc : o.phys_base;      // bases (global ones are CTA-visible now)
     for (int e = tid; e < E; e += kPlanThreads) o.inst_base[sm.inst_off[e]] = pb[sm.home[e] * P + sm.main_phys[e]];
@@ -658,24 +677,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
         o.inst_base[sm.inst_off[e] + 1 + (l - sm.first[e])] = pb[le[j].y * P + M + le[j].z];
       }
     }
-  }
-  if (warp == kPlanWarps - 1) {    // exclusive prefix over ranks (lane t owns the consecutive ranks t*RW ..) and the maximum
-    const int RW = (R + 31) >> 5;
-    int tot = 0, mxl = 0;
-    for (int q = 0; q < RW; ++q) {
-      const int r = lane * RW + q;
-      const int v = r < R ? sm.rload[r] : 0;
-      tot += v;
-      mxl = max(mxl, v);
-    }
-    const int inc = warp_incl_scan(tot, lane);
-    int base = inc - tot;
-    for (int q = 0; q < RW; ++q) {
-      const int r = lane * RW + q;
-      if (r < R) { o.rank_base[r] = base; base += sm.rload[r]; }
-    }
-    mxl = __reduce_max_sync(kFull, mxl);
-    if (lane == 31) { o.rank_base[R] = inc; o.scalars[UEP_SC_MAX_LOAD] = mxl; }
   }
 }
 
