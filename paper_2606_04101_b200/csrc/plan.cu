@@ -567,7 +567,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   __syncthreads();
   // Phase B: one block scan for both prefix sums — instances per expert (high word; <= E + R * n_slot;
   // thread t owns the consecutive experts t*EP ..) and delta over the log (low word; <= S < 2^24, so
-  // it never carries) — and the main instances' phys_count
+  // it never carries); behind it the main instances' CSR entries and, by the last warp, the receive layout
   const int EP = (E + kPlanThreads - 1) / kPlanThreads;            // 1 or 2
   int fan_mx = 0, n_grp = 0;
   {
@@ -575,7 +575,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
 #pragma unroll
     for (int q = 0; q < kEPer; ++q) {
       const int e = tid * EP + q;
-      if (q < EP && e < E) v += 1 + sm.n_rep[e];
+      if (q < EP && e < E) {
+        v += 1 + sm.n_rep[e];
+        pc[sm.home[e] * P + sm.main_phys[e]] = sm.u_main[e];        // complete before the scan's barrier: the
+      }                                                             // last warp lays out the receive buffers behind it
     }
     const unsigned long long both =
         block_incl_scan64(((unsigned long long)v << 32) | (unsigned long long)(unsigned)dsum, sm.scan_tmp);
@@ -590,7 +593,6 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
         o.inst_rank[pos] = h;                                        // CSR entry of the main instance
         o.inst_phys[pos] = mp;
         o.inst_cum[pos] = um;
-        pc[h * P + mp] = um;
         if (o.U) o.U[e * R + h] = um;
         pos += 1 + nr;
         fan_mx = max(fan_mx, 1 + nr);
@@ -609,28 +611,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     n_grp = __reduce_add_sync(kFull, n_grp);
     if (lane == 0) { sm.red_fan[warp] = fan_mx; sm.red_grp[warp] = n_grp; }
   }
-  __syncthreads();
-  // Phase C: the replicas' CSR entries (S11: acceptance order) and, by the last warp, the receive layout
-#pragma unroll
-  for (int j = 0; j < kLogPer; ++j) {
-    const int l = tid * kLogPer + j;
-    if (l < n_log) {
-      const int e = le[j].x;
-      const int f = sm.first[e];
-      const int pos = sm.inst_off[e] + 1 + (l - f);
-      const int before = (f > 0) ? sm.dscan[f - 1] : 0;
-      o.inst_rank[pos] = le[j].y;
-      o.inst_phys[pos] = M + le[j].z;
-      o.inst_cum[pos] = sm.u_main[e] + sm.dscan[l] - before;
-    }
-  }
-  for (int i = E + n_log + tid; i < E + R * n_slot; i += kPlanThreads) {   // unused CSR tail
-    o.inst_rank[i] = -1; o.inst_phys[i] = -1; o.inst_cum[i] = 0; o.inst_base[i] = 0;
-  }
-  if (warp == kPlanWarps - 1) {    // (the last warp: it has log entries above only when more than 960 transfers were accepted)
+  if (warp == kPlanWarps - 1) {    // (the last warp: no expert above unless E > kPlanThreads - 32)
     // receive layout (S13): per rank the exclusive prefix over its P physical slots (lane t owns the
     // consecutive ranks t*RW ..), then the exclusive prefix over ranks and the maximum — beside the
-    // other warps' CSR stores, so that the last phase is the instance bases alone
+    // other warps' CSR entries of the main instances; every phys_count was final at the scan's barrier
     const int RW = (R + 31) >> 5;
     int tot = 0, mxl = 0;
     for (int q = 0; q < RW; ++q) {
@@ -658,25 +642,32 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     mxl = __reduce_max_sync(kFull, mxl);
     if (lane == 31) { o.rank_base[R] = inc; o.scalars[UEP_SC_MAX_LOAD] = mxl; }
   }
+  __syncthreads();
+  // Phase C (last): the replicas' CSR entries (S11: acceptance order) and every instance's base
+  const int* pb = pc_in_smem ? pc : o.phys_base;        // bases (global ones are CTA-visible now)
+#pragma unroll
+  for (int j = 0; j < kLogPer; ++j) {
+    const int l = tid * kLogPer + j;
+    if (l < n_log) {
+      const int e = le[j].x;
+      const int f = sm.first[e];
+      const int pos = sm.inst_off[e] + 1 + (l - f);
+      const int before = (f > 0) ? sm.dscan[f - 1] : 0;
+      o.inst_rank[pos] = le[j].y;
+      o.inst_phys[pos] = M + le[j].z;
+      o.inst_cum[pos] = sm.u_main[e] + sm.dscan[l] - before;
+      o.inst_base[pos] = pb[le[j].y * P + M + le[j].z];             // S13: first token's offset in the rank's buffer
+    }
+  }
+  for (int e = tid; e < E; e += kPlanThreads) o.inst_base[sm.inst_off[e]] = pb[sm.home[e] * P + sm.main_phys[e]];
+  for (int i = E + n_log + tid; i < E + R * n_slot; i += kPlanThreads) {   // unused CSR tail
+    o.inst_rank[i] = -1; o.inst_phys[i] = -1; o.inst_cum[i] = 0; o.inst_base[i] = 0;
+  }
   if (tid == kPlanThreads - 64) {  // (a lane of the last warp but one)
     int max_fan = 0, n_groups = 0;
     for (int w = 0; w < kPlanWarps; ++w) { max_fan = max(max_fan, sm.red_fan[w]); n_groups += sm.red_grp[w]; }
     o.scalars[UEP_SC_MAX_FANOUT] = max_fan;
     o.scalars[UEP_SC_N_GROUPS] = n_groups;
-  }
-  __syncthreads();
-  // Phase D: inst_base = offset of each instance's first token in its rank's receive buffer (S13)
-  {
-    const int* pb = pc_in_smem ? pc : o.phys_base;      // bases (global ones are CTA-visible now)
-    for (int e = tid; e < E; e += kPlanThreads) o.inst_base[sm.inst_off[e]] = pb[sm.home[e] * P + sm.main_phys[e]];
-#pragma unroll
-    for (int j = 0; j < kLogPer; ++j) {
-      const int l = tid * kLogPer + j;
-      if (l < n_log) {
-        const int e = le[j].x;
-        o.inst_base[sm.inst_off[e] + 1 + (l - sm.first[e])] = pb[le[j].y * P + M + le[j].z];
-      }
-    }
   }
 }
 
