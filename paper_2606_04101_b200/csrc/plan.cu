@@ -76,6 +76,7 @@ struct PlanSmem {
   int log_n[2][kPlanMaxNodes]; // accepted transfers of the probe at each tree node (per round parity)
   int node_feas[2][kPlanMaxNodes];   // probe verdict per tree node, written by its owner to every CTA
   int pc[kPcSmem];
+  int pbase[kPcSmem];          // exclusive prefix of pc inside each rank (S13)
   int red_fan[kPlanWarps], red_grp[kPlanWarps];
   unsigned long long scan_tmp[kPlanWarps];
   int lo, hi, n_probes, n_log, log_buf, lo0, hi0, s_valid;
@@ -611,40 +612,22 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
     n_grp = __reduce_add_sync(kFull, n_grp);
     if (lane == 0) { sm.red_fan[warp] = fan_mx; sm.red_grp[warp] = n_grp; }
   }
-  if (warp == kPlanWarps - 1) {    // (the last warp: no expert above unless E > kPlanThreads - 32)
-    // receive layout (S13): per rank the exclusive prefix over its P physical slots (lane t owns the
-    // consecutive ranks t*RW ..), then the exclusive prefix over ranks and the maximum — beside the
-    // other warps' CSR entries of the main instances; every phys_count was final at the scan's barrier
-    const int RW = (R + 31) >> 5;
-    int tot = 0, mxl = 0;
-    for (int q = 0; q < RW; ++q) {
-      const int r = lane * RW + q;
-      if (r < R) {
-        int load = 0;
-        for (int x = 0; x < P; ++x) {
-          const int cnt = pc[r * P + x];
-          o.phys_base[r * P + x] = load;
-          if (pc_in_smem) { o.phys_count[r * P + x] = cnt; pc[r * P + x] = load; }
-          load += cnt;
-        }
-        o.rank_load[r] = load;
-        sm.rload[r] = load;
-        tot += load;
-        mxl = max(mxl, load);
-      }
-    }
-    const int inc = warp_incl_scan(tot, lane);
-    int base = inc - tot;
-    for (int q = 0; q < RW; ++q) {
-      const int r = lane * RW + q;
-      if (r < R) { o.rank_base[r] = base; base += sm.rload[r]; }
-    }
-    mxl = __reduce_max_sync(kFull, mxl);
-    if (lane == 31) { o.rank_base[R] = inc; o.scalars[UEP_SC_MAX_LOAD] = mxl; }
+  // receive layout (S13), an entry (rank, physical slot) per thread, handed out from the LAST thread
+  // down so that it runs beside the expert threads' CSR stores: the slot's base is the sum of the
+  // counts in front of it in its rank (independent loads, P - 1 at most); the thread of a rank's last
+  // slot also has the rank's load.  Every phys_count was final at the scan's barrier.
+  int* pbs = pc_in_smem ? sm.pbase : o.phys_base;
+  for (int i = kPlanThreads - 1 - tid; i < RP; i += kPlanThreads) {
+    const int r = i / P, x = i - r * P;
+    int base = 0;
+    for (int y = 0; y < x; ++y) base += pc[r * P + y];
+    pbs[i] = base;
+    if (pc_in_smem) { o.phys_base[i] = base; o.phys_count[i] = pc[i]; }
+    if (x == P - 1) { const int load = base + pc[i]; o.rank_load[r] = load; sm.rload[r] = load; }
   }
   __syncthreads();
   // Phase C (last): the replicas' CSR entries (S11: acceptance order) and every instance's base
-  const int* pb = pc_in_smem ? pc : o.phys_base;        // bases (global ones are CTA-visible now)
+  const int* pb = pbs;                                  // bases (global ones are CTA-visible now)
 #pragma unroll
   for (int j = 0; j < kLogPer; ++j) {
     const int l = tid * kLogPer + j;
@@ -662,6 +645,22 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   for (int e = tid; e < E; e += kPlanThreads) o.inst_base[sm.inst_off[e]] = pb[sm.home[e] * P + sm.main_phys[e]];
   for (int i = E + n_log + tid; i < E + R * n_slot; i += kPlanThreads) {   // unused CSR tail
     o.inst_rank[i] = -1; o.inst_phys[i] = -1; o.inst_cum[i] = 0; o.inst_base[i] = 0;
+  }
+  if (warp == kPlanWarps - 1) {    // exclusive prefix over the rank loads and their maximum (lane t: ranks t*RW ..)
+    const int RW = (R + 31) >> 5;
+    int tot = 0, mxl = 0;
+    for (int q = 0; q < RW; ++q) {
+      const int r = lane * RW + q;
+      if (r < R) { tot += sm.rload[r]; mxl = max(mxl, sm.rload[r]); }
+    }
+    const int inc = warp_incl_scan(tot, lane);
+    int base = inc - tot;
+    for (int q = 0; q < RW; ++q) {
+      const int r = lane * RW + q;
+      if (r < R) { o.rank_base[r] = base; base += sm.rload[r]; }
+    }
+    mxl = __reduce_max_sync(kFull, mxl);
+    if (lane == 31) { o.rank_base[R] = inc; o.scalars[UEP_SC_MAX_LOAD] = mxl; }
   }
   if (tid == kPlanThreads - 64) {  // (a lane of the last warp but one)
     int max_fan = 0, n_groups = 0;
