@@ -306,6 +306,31 @@ int uep_balance_host(const uep_ctx* ctx, const int32_t* topk_ids_host, const voi
                      int32_t* scalars_host, int32_t n_tensors, const void* const* src,
                      const size_t* bytes_per_expert, void* const* dst, void* ws, void* stream);
 
+/* Histogram for callers that cannot allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same lambda_e as uep_histogram (Alg. 1 line 2,
+ * PAPER.md:250; ids outside [0,E) skipped, S14) with NO context and NO workspace.  The
+ * per-CTA count rows that uep_histogram keeps in the caller's workspace live in a fixed array in
+ * the library's device image (192 rows x UEP_MAX_E int32 = 384 KB on every GPU that loads the
+ * library, until the process exits).  The call allocates nothing: no cudaMalloc / cudaFree and no
+ * allocating library routine, on the first call or later.
+ *   topk_ids      DEVICE int32 [n_slots], 16-byte aligned (may be NULL when n_slots == 0)
+ *   n_slots       0 .. UEP_STATIC_MAX_SLOTS; beyond it UEP_ERR_UNSUPPORTED, nothing launched
+ *   E             1 .. UEP_MAX_E; outside it UEP_ERR_UNSUPPORTED, nothing launched
+ *   expert_count  DEVICE int32 [E], out, 16-byte aligned
+ * Two kernels on `stream` of the CURRENT device, asynchronous.  uep_static_last_error() gives the
+ * text of the last rejection on this thread (which limit, which value).  The first call on a device
+ * resolves the array's address there (cudaGetSymbolAddress, once per device); make that call — or
+ * uep_histogram_static_setup(), with the device current — outside stream capture.
+ * ALL calls on a device share the one array, and it keeps the last call's rows (every row a call
+ * reads it has written itself, nothing needs clearing): calls that OVERLAP on the GPU — different
+ * streams without an ordering between them, or a graph replayed concurrently with itself — race.
+ * Calls ordered on one stream, or by events, are safe. */
+#define UEP_STATIC_MAX_SLOTS (1 << 24)
+int uep_histogram_static_setup(void);
+int uep_histogram_static(const int32_t* topk_ids, long long n_slots, int32_t E, int32_t* expert_count,
+                         void* stream);
+const char* uep_static_last_error(void);
+
 /* Number of kernels launched through this context so far (host-side count, all entry points).
  * The bench reports the difference over its timed region as gpu_launches. */
 unsigned long long uep_launch_count(const uep_ctx* ctx);

@@ -28,7 +28,9 @@ EXPORTS = ["uep_create", "uep_destroy", "uep_workspace_bytes", "uep_workspace_in
            "uep_remap_lookup", "uep_remap_inverse", "uep_relay_plan", "uep_pack", "uep_grad_reduce",
            "uep_balance",
            "uep_balance_host", "uep_strerror", "uep_last_cuda_error", "uep_get_launch_info",
-           "uep_launch_count"]
+           "uep_launch_count", "uep_histogram_static", "uep_histogram_static_setup",
+           "uep_static_last_error"]
+STATIC_MAX_SLOTS = 1 << 24
 
 
 class UepError(RuntimeError):
@@ -80,6 +82,7 @@ def lib():
         L.uep_last_cuda_error.restype = ctypes.c_char_p
         L.uep_destroy.restype = None
         L.uep_launch_count.restype = ctypes.c_ulonglong
+        L.uep_static_last_error.restype = ctypes.c_char_p
         _lib = L
     return _lib
 
@@ -91,6 +94,29 @@ def _check(rc: int):
         if rc == -3:
             msg += " — " + L.uep_last_cuda_error().decode()
         raise UepError(f"libuep rc={rc}: {msg}")
+
+
+def _check_static(rc: int):
+    if rc != 0:
+        L = lib()
+        msg = L.uep_static_last_error().decode() or L.uep_strerror(rc).decode()
+        if rc == -3:
+            msg += " — " + L.uep_last_cuda_error().decode()
+        raise UepError(f"libuep rc={rc}: {msg}")
+
+
+def uep_histogram_static_setup():
+    """Resolve the static scratch on the current device (once per device, outside capture)."""
+    _check_static(lib().uep_histogram_static_setup())
+
+
+def uep_histogram_static(topk_ids, E, expert_count, stream=None, n_slots=None):
+    """lambda_e without context or workspace; the library allocates nothing (include/uep.h).
+    topk_ids: int32 device tensor (or None with n_slots=0); expert_count: int32 [E] device tensor."""
+    n = (0 if topk_ids is None else topk_ids.numel()) if n_slots is None else int(n_slots)
+    _check_static(lib().uep_histogram_static(_ptr(topk_ids), ctypes.c_longlong(n), ctypes.c_int32(E),
+                                             _ptr(expert_count), _stream(stream)))
+    return expert_count
 
 
 def _ptr(t):
