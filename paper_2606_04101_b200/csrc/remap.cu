@@ -46,12 +46,45 @@ constexpr unsigned kFullMask = 0xffffffffu;
 constexpr int kEMask = (1 << kPackedEBits) - 1;
 
 // ------------------------------------------------------------------------------------------------
-// rank_kernel.  dynamic shared memory: wrow[kRemapWarps][E_pad] (int2 {mask, count})
+// rank_kernel.  Two ways to the same packed words (expert | stable rank inside the chunk << 9):
+//
+// FAST (W > 0), for routing as top-k produces it — a token names an expert at most once.  Then the
+// slots of expert e in the chunk are one per token, in token order, and the rank of slot (t, e) is
+// the number of tokens before t that name e: a bitmap per expert over the chunk's tokens
+// (B[e][W] words), one shared-memory atomicOr per slot (commutative: no order-dependent atomic
+// anywhere), an exclusive prefix of the words' popcounts per expert (P[e][W], 16 bit), and
+// rank = P[e][w] + popc(B[e][w] & bits below t).  Every slot of a thread is independent of the
+// others (no warp-synchronous steps).  An atomicOr that finds its bit already set has met a token
+// that names an expert twice: the CTA then falls back to the general way below.
+// dynamic shared memory: B[E_pad][W] (int32) | P[E_pad][W] (uint16)
+//
+// GENERAL (any ids; W == 0 when the bitmaps do not fit or k is 1): every warp owns a row of cells
+// {peer mask, count} per expert and ranks its span in steps of 32 slots (lanes in order): atomicOr
+// of the lane's bit, read, the lowest peer adds the popcount and clears the mask.
+// dynamic shared memory: wrow[kRemapWarps][E_pad] (int2 {mask, count})
 // ------------------------------------------------------------------------------------------------
+constexpr size_t kRankFastSmem = 96 * 1024;        // two CTAs per SM beside the other kernels of the chain
+
+// words per expert row of the token bitmaps for chunks of chunk_len slots, 0 = general way only
+inline int rank_fast_words(int chunk_len, int k, int E_pad) {
+  if (k < 2 || k > 64) return 0;                   // (k = 1: one slot per token, nothing to gain; the division by
+  const int toks = chunk_len / k + 2;              //  multiplication below is exact for slot * k < 2^32)
+  const int W = ((toks + 31) / 32) | 1;            // odd pitch: rows of different experts start in different banks
+  return (size_t)E_pad * W * 6 <= kRankFastSmem ? W : 0;
+}
+inline size_t rank_smem_bytes(int E_pad, int W) {
+  const size_t general = sizeof(int2) * (size_t)kRemapWarps * E_pad, fast = (size_t)E_pad * W * 6 + 16;
+  return general > fast ? general : fast;
+}
+
+// BITMAPS = false is the general way alone, with the code the compiler makes for it alone (uep_balance
+// launches that one: 42 registers, so that a CTA fits beside the planner's 512 x 80 on one SM; inside
+// the BITMAPS = true kernel the general loop comes out at 39 instructions per step instead of 30).
+template <bool BITMAPS>
 __global__ void __launch_bounds__(kRemapThreads, 2)
 rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len, int cpg,
             int group_len, int32_t* __restrict__ packed, int32_t* __restrict__ prefix,
-            int32_t* __restrict__ counts, int chunk0) {
+            int32_t* __restrict__ counts, int chunk0, int W, unsigned k_magic) {
   extern __shared__ __align__(16) int smem[];
   int2* wrow = reinterpret_cast<int2*>(smem);
   pdl_trigger();                                 // prefix_kernel may be scheduled (it waits for this grid)
@@ -75,6 +108,64 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
 #pragma unroll
   for (int i = 0; i < kRemapItems; ++i)
     ev[i] = (i < items && i * 32 < room) ? __ldg(ids + i * 32) : -1;
+
+  if (BITMAPS && W > 0) {
+    int* B = smem;
+    unsigned short* P = reinterpret_cast<unsigned short*>(B + E_pad * W);
+    {
+      int4* z = reinterpret_cast<int4*>(B);                            // E_pad % 4 == 0
+      for (int i = tid; i < E_pad * W / 4; i += kRemapThreads) z[i] = make_int4(0, 0, 0, 0);
+    }
+    __syncthreads();
+    // token of slot g (global index) = g / k = umulhi(g, ceil(2^32 / k)), exact for g * k < 2^32
+    const unsigned tok0 = __umulhi((unsigned)cbegin, k_magic);
+    const unsigned g0 = (unsigned)cbegin + (unsigned)(wbeg + lane);
+    unsigned dup = 0;
+    const unsigned B_s = smem_u32(B);
+#pragma unroll
+    for (int i = 0; i < kRemapItems; ++i) {
+      if (i >= items) break;                                            // (CTA-uniform)
+      const unsigned e = (unsigned)ev[i];
+      const bool valid = e < (unsigned)E;                               // (a slot beyond the chunk holds -1)
+      const unsigned lt = __umulhi(g0 + 32u * i, k_magic) - tok0;       // token inside the chunk
+      const unsigned bit = 1u << (lt & 31u);
+      unsigned old = 0;                                                 // (a predicated atomic, no branch per slot)
+      asm volatile("{ .reg .pred p; setp.ne.u32 p, %4, 0; @p atom.shared.or.b32 %0, [%1], %2; @!p mov.u32 %0, %3; }"
+                   : "=r"(old) : "r"(B_s + 4u * (e * (unsigned)W + (lt >> 5))), "r"(bit), "r"(0u), "r"((unsigned)valid) : "memory");
+      dup |= old & bit;
+      ev[i] = valid ? (int)(e | (lt << kPackedEBits)) : -1;
+    }
+    if (!__syncthreads_or(dup != 0u)) {
+      // per expert: exclusive prefix of the words' popcounts; the total is the chunk's count of e
+      for (int e = tid; e < E_pad; e += kRemapThreads) {
+        int run = 0;
+#pragma unroll 4
+        for (int w = 0; w < W; ++w) {
+          P[e * W + w] = (unsigned short)run;
+          run += __popc((unsigned)B[e * W + w]);
+        }
+        prefix[(size_t)(cb + 1) * E_pad + e] = run;     // (rows of e >= E are all zero)
+        counts[(size_t)cb * E_pad + e] = run;
+      }
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < kRemapItems; ++i) {
+        if (i >= items) break;                                          // (CTA-uniform)
+        const int pk = ev[i];
+        const unsigned up = (unsigned)max(pk, 0);                       // (-1: cell 0, result unused)
+        const unsigned e = up & (unsigned)kEMask, lt = up >> kPackedEBits;
+        const unsigned idx = e * (unsigned)W + (lt >> 5);
+        const int r = (int)P[idx] + __popc((unsigned)B[idx] & ((1u << (lt & 31u)) - 1u));
+        if (i * 32 < room) packed[i * 32] = pk >= 0 ? (int)(e | ((unsigned)r << kPackedEBits)) : -1;
+      }
+      return;
+    }
+    // a token names an expert twice: redo the chunk the general way (the barrier above ordered every
+    // atomicOr before the cells below are cleared)
+#pragma unroll
+    for (int i = 0; i < kRemapItems; ++i) ev[i] = ev[i] < 0 ? -1 : (ev[i] & kEMask);
+  }
+
   {
     int4* z = reinterpret_cast<int4*>(wrow);
     for (int i = tid; i < kRemapWarps * E_pad / 2; i += kRemapThreads) z[i] = make_int4(0, 0, 0, 0);
@@ -223,15 +314,24 @@ int launch_shard_rows(const Ctx* c, void* ws, cudaStream_t s, int rank0, int n_r
 // chunk0 / n_launch: the chunk range a token shard owns (uep_shard_count; `ids` is then the
 // virtual base of the global [S] array, only the shard's slots are dereferenced); n_launch < 0:
 // all chunks.  with_prefix = false leaves the raw per-chunk counts for the exchange step.
+// bitmaps = false (uep_balance): the general way.  There the kernel shares its SMs with the planner,
+// its end is set by when its second wave of CTAs gets onto the SMs (after the histogram's CTAs
+// leave), not by its instruction stream, and the bitmap way's higher issue rate slows the planner's
+// probes on the SMs they share (measured, A/B on one box: chain 29.4 -> 29.9 us with it; rank + prefix alone
+// 12.3 -> 10.9 us).
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local, int chunk0,
-                int n_launch, bool with_prefix) {
+                int n_launch, bool with_prefix, bool bitmaps) {
   if (c->S == 0) return UEP_OK;
   const int chunks = local ? c->l_chunks : c->r_chunks;
-  const size_t smem = sizeof(int2) * (size_t)kRemapWarps * c->E_pad;
-  rank_kernel<<<n_launch < 0 ? chunks : n_launch, kRemapThreads, smem, s>>>(
-      ids, c->S, c->cfg.E, c->E_pad, local ? c->l_chunk_len : c->r_chunk_len,
+  const int clen = local ? c->l_chunk_len : c->r_chunk_len, k = c->cfg.k;
+  const int W = bitmaps ? rank_fast_words(clen, k, c->E_pad) : 0;
+  const unsigned k_magic = W > 0 ? 0xffffffffu / (unsigned)k + 1u : 0u;      // ceil(2^32 / k), k >= 2
+  const size_t smem = rank_smem_bytes(c->E_pad, W);
+  auto kern = W > 0 ? rank_kernel<true> : rank_kernel<false>;
+  kern<<<n_launch < 0 ? chunks : n_launch, kRemapThreads, smem, s>>>(
+      ids, c->S, c->cfg.E, c->E_pad, clen,
       local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S, ws_packed(c, ws),
-      ws_prefix(c, ws), ws_counts(c, ws), chunk0);
+      ws_prefix(c, ws), ws_counts(c, ws), chunk0, W, k_magic);
   UEP_CUDA_TRY(cudaGetLastError());
   count_launch(c);
   if (with_prefix) return launch_prefix(c, ws, s, local, /*pdl=*/true);
@@ -638,7 +738,8 @@ static int launch_lookup_t(const Ctx* c, const GateT* gate, const uep_plan_out& 
 }
 
 int init_remap_kernels() {
-  int rc = prefer_max_smem(rank_kernel);
+  int rc = prefer_max_smem(rank_kernel<false>);
+  if (rc == UEP_OK) rc = prefer_max_smem(rank_kernel<true>);
   if (rc == UEP_OK) rc = prefer_max_smem(prefix_kernel);
   if (rc == UEP_OK) rc = prefer_max_smem(reroute_kernel);
   if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint32_t, true, false>);
@@ -650,9 +751,10 @@ int init_remap_kernels() {
   if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint16_t, false, false>);
   if (rc == UEP_OK) rc = prefer_max_smem(lookup_kernel<uint16_t, false, true>);
   if (rc != UEP_OK) return rc;
-  const int rank_bytes = (int)(sizeof(int2) * (size_t)kRemapWarps * UEP_MAX_E);
+  const int rank_bytes = (int)std::max(sizeof(int2) * (size_t)kRemapWarps * UEP_MAX_E, kRankFastSmem + 16);
   const int bytes = (int)lookup_smem_bytes(UEP_MAX_E, UEP_MAX_R, UEP_MAX_E + UEP_MAX_R * UEP_MAX_NSLOT, true);
-  UEP_CUDA_TRY(cudaFuncSetAttribute(rank_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, rank_bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(rank_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, rank_bytes));
+  UEP_CUDA_TRY(cudaFuncSetAttribute(rank_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, rank_bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   UEP_CUDA_TRY(cudaFuncSetAttribute(lookup_kernel<uint32_t, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));

@@ -547,7 +547,7 @@ static int balance_impl(const uep_ctx* ctx, const int32_t* topk_ids, const void*
   UEP_BAL_RC(launch_histogram(c, topk_ids, expert_count, ws, s, /*red=*/true));
   UEP_BAL_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
   forked = (rc == UEP_OK && ce == cudaSuccess);
-  UEP_BAL_RC(launch_rank(c, topk_ids, ws, c->side));
+  UEP_BAL_RC(launch_rank(c, topk_ids, ws, c->side, /*local=*/false, 0, -1, /*with_prefix=*/true, /*bitmaps=*/false));
   UEP_BAL_TRY(cudaEventRecord(c->ev_rank, c->side));
   // planner and lookup are launched programmatically dependent on their predecessor: their
   // prologues (static layout; packed ranks, gates) overlap it
