@@ -192,7 +192,10 @@ int uep_remap(const uep_ctx* ctx, const int32_t* topk_ids, const void* gate,
  *                     concurrently with uep_histogram / uep_plan on another stream.
  *   uep_remap_lookup  plan-DEPENDENT: needs ws after uep_remap_rank on the same topk_ids, and
  *                     the plan of those ids.  Same outputs and argument rules as uep_remap.
- * uep_remap(...) == uep_remap_rank(...) then uep_remap_lookup(...) on one stream. */
+ * uep_remap(...) == uep_remap_rank(...) then uep_remap_lookup(...) on one stream.
+ * uep_remap_rank accepts any ids.  When every token names an expert at most once (what top-k
+ * routing produces) and 2 <= k <= 64 it ranks with per-expert token bitmaps, which is faster; a
+ * token that repeats an expert sends its chunk through the general method.  Same result either way. */
 int uep_remap_rank(const uep_ctx* ctx, const int32_t* topk_ids, void* ws, void* stream);
 int uep_remap_lookup(const uep_ctx* ctx, const void* gate, const uep_plan_out* plan,
                      int32_t* out_replica, int32_t* out_rank, int32_t* out_offset, void* out_gate,
