@@ -480,20 +480,24 @@ def run_uep(args):
 
     # ---- stage timing: graph-captured chains over all instances (L2-cold by rotation) --------
     reps = 5
+    # Every timed graph holds at least 32 calls (the instances in order, as many rounds as that takes),
+    # so that the gap between two graph launches — harness, not layer — weighs the same whatever
+    # --steps is (with 20 instances in a graph of 20 calls it added 0.5 us per call to the chain).
+    g_rounds = max(1, -(-32 // n_inst))
+    order = [i for _ in range(g_rounds) for i in range(n_inst)]
+
+    def timed(fn):
+        ms, mn = time_graph(capture([lambda i=i: fn(i) for i in order], stream), stream, reps)
+        return ms / g_rounds, mn / g_rounds       # per round over the n_inst instances
+
     # the chain is uep_balance without state tensors: histogram -> plan -> lookup on the stream,
     # the rank half of the remap forked beside histogram + plan (as the library schedules it)
-    chain = capture([lambda i=i: rig.balance(i, with_pack=False) for i in range(n_inst)], stream)
-    g_rank = capture([lambda i=i: rig.rank(i) for i in range(n_inst)], stream)
-    g_lookup = capture([lambda i=i: rig.lookup(i) for i in range(n_inst)], stream)
-    g_hist = capture([lambda i=i: rig.hist(i) for i in range(n_inst)], stream)
-    g_plan = capture([lambda i=i: rig.plan(i) for i in range(n_inst)], stream)
-    g_remap = capture([lambda i=i: rig.remap(i) for i in range(n_inst)], stream)
-    chain_ms, chain_min = time_graph(chain, stream, reps)
-    hist_ms, _ = time_graph(g_hist, stream, reps)
-    plan_ms, _ = time_graph(g_plan, stream, reps)
-    remap_ms, _ = time_graph(g_remap, stream, reps)
-    rank_ms, _ = time_graph(g_rank, stream, reps)
-    lookup_ms, _ = time_graph(g_lookup, stream, reps)
+    chain_ms, chain_min = timed(lambda i: rig.balance(i, with_pack=False))
+    hist_ms, _ = timed(rig.hist)
+    plan_ms, _ = timed(rig.plan)
+    remap_ms, _ = timed(rig.remap)
+    rank_ms, _ = timed(rig.rank)
+    lookup_ms, _ = timed(rig.lookup)
     n_pack = min(n_inst, 8)
     g_pack = capture([lambda i=i: rig.pack(i) for i in range(n_pack)], stream)
     pack_ms, _ = time_graph(g_pack, stream, 3, warm=1)
@@ -579,6 +583,7 @@ def run_uep(args):
                     "n_replicas_mean": round(statistics.mean(n_rep), 1),
                     "max_fanout_max": max(int(s[binding.SC_MAX_FANOUT]) for s in sc),
                     "n_probes_mean": round(statistics.mean(int(s[binding.SC_N_PROBES]) for s in sc), 1)},
+        "calls_per_timed_graph": n_inst * g_rounds,
         "batched_plan": {"instances": n_inst, "us_total": round(bplan_ms * 1e3, 2),
                          "us_per_layer": round(bplan_ms * 1e3 / n_inst, 3),
                          "note": "uep_plan_batched: one launch, one 8-CTA cluster per instance"},
