@@ -670,7 +670,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   }
 }
 
-constexpr size_t kLogBudget = 128 * 1024;     // shared memory for the accept logs of one round
+constexpr size_t kLogBudget = 144 * 1024;     // shared memory for the accept logs of one round (9 x 1024 entries: R = 256, N_slot = 4)
 
 template <int RPL>
 static int launch_plan_t(const Ctx* c, const int32_t* count, const uep_plan_out& plan,
