@@ -727,9 +727,9 @@ def test_long_fuzz_opt_in():
     """The walk of test_random_shapes_fuzz for a time budget, with token counts up to 300 000 (many
     chunks, instance boundaries inside chunks) and, through the bodies of the NEXT-row tests, random
     arguments for uep_remap_local, the token-sharded path, relay plans and the gradient reduce.
-    Run at the end of round 2 with UEP_FUZZ_SECONDS=600 on one B200: 19 920 chain cases and 987
-    sets of NEXT-row cases, no mismatch (earlier developer runs of the same walks: 40 340 and
-    11 726 cases; the only rejections there were shard slices that are not 16-byte aligned,
+    Last run, at the final sources of round 2 with UEP_FUZZ_SECONDS=900 on one B200: 42 320 chain
+    cases and 2 091 sets of NEXT-row cases, no mismatch (earlier developer runs of similar walks
+    rejected only shard slices that are not 16-byte aligned,
     UEP_ERR_INVALID_ARG as include/uep.h states — this walk keeps them aligned)."""
     import random
     import time
