@@ -726,7 +726,7 @@ def test_random_shapes_fuzz(seed):
 def test_long_fuzz_opt_in():
     """The walk of test_random_shapes_fuzz for a time budget, with token counts up to 300 000 (many
     chunks, instance boundaries inside chunks) and, through the bodies of the NEXT-row tests, random
-    arguments for uep_remap_local, the token-sharded path, relay plans and the gradient reduce.
+    arguments for uep_remap_local, the token-sharded path and relay plans.
     Last run, at the final sources of round 2 with UEP_FUZZ_SECONDS=900 on one B200: 42 320 chain
     cases and 2 091 sets of NEXT-row cases, no mismatch (earlier developer runs of similar walks
     rejected only shard slices that are not 16-byte aligned,
