@@ -361,7 +361,8 @@ def run_token_sharded(c, rig, world, rank, device, stream, reps):
     import torch
     import torch.distributed as dist
     from paper_2606_04101_b200 import binding, shard
-    n = min(4, rig.n_inst)
+    n = min(8, rig.n_inst)
+    rounds = max(1, -(-32 // n))            # at least 32 steps per timed graph, as for the other stages
     S = c["T"] * c["k"]
     Sl = S // world
     ids_l, gate_l = [], []
@@ -383,9 +384,9 @@ def run_token_sharded(c, rig, world, rank, device, stream, reps):
     if dist.is_available() and dist.is_initialized():
         dist.barrier()
     try:                                    # count -> exchange -> finish is one capturable sequence
-        g = capture([lambda i=i: layers[i].step(ids_l[i], gate_l[i]) for i in range(n)], stream)
+        g = capture([lambda i=i: layers[i].step(ids_l[i], gate_l[i]) for _ in range(rounds) for i in range(n)], stream)
         ms, _ = time_graph(g, stream, reps)
-        ms /= n
+        ms /= n * rounds
     except Exception:                       # a process group that cannot be captured: time as launched
         use_graph = False
         torch.cuda.synchronize(device)

@@ -219,9 +219,11 @@ int uep_remap_local(const uep_ctx* ctx, const int32_t* topk_ids, const void* gat
  * exchanges the count matrix ... every rank solves the same plan").
  * GPU g of G (G divides R, T % R == 0) owns the tokens of source ranks [g*R/G, (g+1)*R/G), i.e.
  * the contiguous slot range [g*S/G, (g+1)*S/G).  One layer is
- *   uep_shard_count   on every GPU: ranks its LOCAL slots inside their chunks and leaves this
- *                     shard's rows of the count matrix Lambda[R][E] (lambda_{r,e}: one row of E_pad
- *                     int32 per source rank the shard owns) in ws;
+ *   uep_shard_count   on every GPU: one counting pass over its LOCAL slots leaves this shard's rows
+ *                     of the count matrix Lambda[R][E] (lambda_{r,e}: one row of E_pad int32 per
+ *                     source rank the shard owns) in ws, on `stream`; the stable ranks of the slots,
+ *                     which only uep_shard_finish needs, are computed beside it on the context's
+ *                     internal side stream (forked from `stream` here);
  *   an all-gather     of those rows, by the caller (NCCL / torch.distributed; the only exchange:
  *                     4 * E_pad * R bytes in total, 64 KB at R = 64, E = 256).  uep_shard_rows gives
  *                     the byte range of shard g's rows inside ws: the ranges of shards 0..G-1 are
@@ -240,6 +242,10 @@ int uep_remap_local(const uep_ctx* ctx, const int32_t* topk_ids, const void* gat
  *   n_inflight   DEVICE int32 [R] or NULL: entries of this shard's source ranks are set to the
  *                number of their slots that leave the rank
  *   ws           sized by uep_workspace_bytes (of the whole problem), initialised once
+ * uep_shard_finish joins the side stream's work in front of its lookup, so the pair uses the context's
+ * side stream and events like uep_balance: issue uep_shard_count / uep_shard_finish of one context from
+ * one host thread at a time, call them on the SAME `stream`, and under stream capture put both into
+ * the same capture (a capture that ends after uep_shard_count alone ends with an un-joined fork).
  * Errors: UEP_ERR_UNSUPPORTED if T % R != 0; UEP_ERR_INVALID_ARG if G does not divide R, g is
  * out of range, or a pointer is NULL / misaligned. */
 int uep_shard_count(const uep_ctx* ctx, int32_t shard, int32_t n_shards,

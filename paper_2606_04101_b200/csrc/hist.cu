@@ -105,6 +105,58 @@ publish_kernel(int E, int32_t* __restrict__ acc, int32_t* __restrict__ expert_co
   }
 }
 
+// Token-sharded path: the count rows of the GROUPED chunks (chunk cb = sub-chunk cb % cpg
+// of source rank cb / cpg, never across two source ranks' blocks) without the ranks — the quick half
+// of uep_shard_count, so that the rows for the exchange are ready after one pass over the ids while
+// rank_kernel works beside it.  Same counting scheme as hist_kernel; a chunk may start anywhere, so the
+// 16-byte loads begin at the first aligned slot.  Row cb of `counts` gets the chunk's counts.
+constexpr int kShThreads = 512;                               // two CTAs per SM: the 256 chunks of the DeepSeek-V3 shape in one wave
+constexpr int kShRows = (kShThreads / 32) >> kHistShare;
+__global__ void __launch_bounds__(kShThreads, 2)
+shard_hist_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len, int cpg,
+                  int group_len, int32_t* __restrict__ counts, int chunk0) {
+  extern __shared__ __align__(16) int hsm[];
+  const int pitch = E_pad + 1;
+  int* priv = hsm;
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const int cb = (int)blockIdx.x + chunk0;
+  pdl_trigger();
+  const int grp = cb / cpg, sub = cb - grp * cpg;
+  const long long cbegin = (long long)grp * group_len + (long long)sub * chunk_len;
+  const int clen = (int)min(min((long long)chunk_len, (long long)group_len - (long long)sub * chunk_len),
+                            (long long)S - cbegin);
+  for (int i = tid; i < kShRows * pitch; i += kShThreads) priv[i] = 0;
+  __syncthreads();
+  int* row = priv + (warp >> kHistShare) * pitch;
+  const int32_t* p = ids + cbegin;
+  const int lead = min(clen, (int)(((16u - (unsigned)(reinterpret_cast<uintptr_t>(p) & 15u)) & 15u) >> 2));
+  if (tid < lead) count_one(row, p[tid], E);
+  const int4* v = reinterpret_cast<const int4*>(p + lead);
+  const int n_vec = (clen - lead) >> 2;
+  for (int vbase = 0; vbase < n_vec; vbase += kShThreads * kHistVecs) {     // all loads of a round in flight first
+    int4 x[kHistVecs];
+#pragma unroll
+    for (int u = 0; u < kHistVecs; ++u) {
+      const int i = vbase + u * kShThreads + tid;
+      x[u] = (i < n_vec) ? ld_stream_v4(v + i) : make_int4(-1, -1, -1, -1);
+    }
+#pragma unroll
+    for (int u = 0; u < kHistVecs; ++u) {
+      count_one(row, x[u].x, E); count_one(row, x[u].y, E);
+      count_one(row, x[u].z, E); count_one(row, x[u].w, E);
+    }
+  }
+  const int t0 = lead + (n_vec << 2);
+  if (tid < clen - t0) count_one(row, p[t0 + tid], E);
+  __syncthreads();
+  for (int e = tid; e < E_pad; e += kShThreads) {
+    int s = 0;
+#pragma unroll 8
+    for (int w = 0; w < kShRows; ++w) s += priv[w * pitch + e];
+    counts[(size_t)cb * E_pad + e] = s;
+  }
+}
+
 // S == 0: nothing to read; zero the counts and the single table row.
 __global__ void hist_empty_kernel(int E, int E_pad, int32_t* table, int32_t* expert_count) {
   for (int e = threadIdx.x; e < E_pad; e += blockDim.x) {
@@ -117,11 +169,24 @@ int init_hist_kernels() {
   int rc = prefer_max_smem(hist_kernel<false>);
   if (rc == UEP_OK) rc = prefer_max_smem(hist_kernel<true>);
   if (rc == UEP_OK) rc = prefer_max_smem(publish_kernel);
+  if (rc == UEP_OK) rc = prefer_max_smem(shard_hist_kernel);
   if (rc != UEP_OK) return rc;
+  UEP_CUDA_TRY(cudaFuncSetAttribute(shard_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)(sizeof(int) * (hist_smem_ints(UEP_MAX_E) + 4))));
   UEP_CUDA_TRY(cudaFuncSetAttribute(hist_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(sizeof(int) * (hist_smem_ints(UEP_MAX_E) + 4))));
   UEP_CUDA_TRY(cudaFuncSetAttribute(hist_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(sizeof(int) * (hist_smem_ints(UEP_MAX_E) + 4))));
+  return UEP_OK;
+}
+
+int launch_shard_hist(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, int chunk0, int n_launch) {
+  if (c->S == 0 || n_launch <= 0) return UEP_OK;
+  const size_t smem = sizeof(int) * (hist_smem_ints(c->E_pad) + 4);
+  shard_hist_kernel<<<n_launch, kShThreads, smem, s>>>(ids, c->S, c->cfg.E, c->E_pad, c->l_chunk_len, c->l_cpg,
+                                                        c->l_group_len, ws_counts(c, ws), chunk0);
+  UEP_CUDA_TRY(cudaGetLastError());
+  count_launch(c);
   return UEP_OK;
 }
 

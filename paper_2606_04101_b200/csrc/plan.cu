@@ -228,7 +228,10 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   // critical path, and a cold constant-cache line there costs several hundred cycles
   if (out.slot_expert == nullptr || out.scalars == nullptr || count_out == reinterpret_cast<int32_t*>(1)) return;
   // ---- setup, three barrier-separated phases after the wait -----------------------------------
-  pdl_trigger();                   // the lookup kernel may start its plan-independent prologue
+  // the lookup kernel may start its plan-independent prologue.  Token-sharded path (acc_rows > 1): only
+  // after the wait below — that prologue reads the gathered Lambda rows, which the kernels in front of
+  // this one (shard_rows_kernel, the all-gather) are still writing until then
+  if (acc_rows <= 1) pdl_trigger();
   // static layout first: it does not depend on the histogram (overlaps it under programmatic launch)
   for (int e = tid; e < E; e += kPlanThreads) {
     sm.home[e] = g_home[e];
@@ -242,6 +245,7 @@ plan_kernel(const int32_t* __restrict__ expert_count, const int32_t* __restrict_
   if (blockIdx.x == 0) for (int i = tid; i < zero_n; i += kPlanThreads) zero_ptr[i] = 0;
   __syncthreads();
   pdl_wait();                      // the histogram (preceding kernel) is complete
+  if (acc_rows > 1) pdl_trigger();
   // phase 1: lambda_e into shared memory, and line 2 (l_r) straight from global memory with
   // independent loads (thread r sums its own experts: no barrier between lambda and l_r)
   if (acc_rows <= 1) {

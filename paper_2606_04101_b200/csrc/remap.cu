@@ -84,10 +84,13 @@ template <bool BITMAPS>
 __global__ void __launch_bounds__(kRemapThreads, 2)
 rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_len, int cpg,
             int group_len, int32_t* __restrict__ packed, int32_t* __restrict__ prefix,
-            int32_t* __restrict__ counts, int chunk0, int W, unsigned k_magic) {
+            int32_t* __restrict__ counts, int chunk0, int W, unsigned k_magic, int early_trigger) {
   extern __shared__ __align__(16) int smem[];
   int2* wrow = reinterpret_cast<int2*>(smem);
-  pdl_trigger();                                 // prefix_kernel may be scheduled (it waits for this grid)
+  // prefix_kernel may be scheduled (it waits for this grid).  Not when the kernel behind this one is
+  // the lookup itself (uep_shard_count: under stream capture the lookup's edge from this kernel is
+  // programmatic, and its prologue reads what this kernel writes)
+  if (early_trigger) pdl_trigger();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
   const int cb = (int)blockIdx.x + chunk0;       // chunk0 > 0: a token shard's CTAs (uep_shard_count)
@@ -145,7 +148,7 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
           run += __popc((unsigned)B[e * W + w]);
         }
         prefix[(size_t)(cb + 1) * E_pad + e] = run;     // (rows of e >= E are all zero)
-        counts[(size_t)cb * E_pad + e] = run;
+        if (counts) counts[(size_t)cb * E_pad + e] = run;
       }
       __syncthreads();
 #pragma unroll
@@ -206,7 +209,7 @@ rank_kernel(const int32_t* __restrict__ ids, int S, int E, int E_pad, int chunk_
       }
     }
     prefix[(size_t)(cb + 1) * E_pad + e] = run;
-    counts[(size_t)cb * E_pad + e] = run;     // row c of `counts` is never rewritten: the lookup reads it before prefix_kernel is done
+    if (counts) counts[(size_t)cb * E_pad + e] = run;     // row c of `counts` is never rewritten: the lookup reads it before prefix_kernel is done
   }
   __syncthreads();
 
@@ -279,8 +282,9 @@ prefix_kernel(int32_t* __restrict__ prefix, int n_rows, int CG) {
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(UEP_MAX_E)
 shard_rows_kernel(int E_pad, int cpg, int rank0, const int32_t* __restrict__ counts, int32_t* __restrict__ lambda) {
-  pdl_wait();                                   // rank_kernel complete.  (No early trigger: on one GPU the planner
-                                                // is next, and the lookup behind IT reads Lambda in its prologue)
+  pdl_trigger();                                // the planner behind this kernel may be placed and run its static
+                                                // set-up; it lets the lookup start only after its own wait for this grid
+  pdl_wait();                                   // shard_hist_kernel complete
   const int r = rank0 + (int)blockIdx.x;
   for (int e = threadIdx.x; e < E_pad; e += blockDim.x) {
     int s = 0;
@@ -320,7 +324,7 @@ int launch_shard_rows(const Ctx* c, void* ws, cudaStream_t s, int rank0, int n_r
 // probes on the SMs they share (measured, A/B on one box: chain 29.4 -> 29.9 us with it; rank + prefix alone
 // 12.3 -> 10.9 us).
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local, int chunk0,
-                int n_launch, bool with_prefix, bool bitmaps) {
+                int n_launch, bool with_prefix, bool bitmaps, bool write_counts) {
   if (c->S == 0) return UEP_OK;
   const int chunks = local ? c->l_chunks : c->r_chunks;
   const int clen = local ? c->l_chunk_len : c->r_chunk_len, k = c->cfg.k;
@@ -331,7 +335,7 @@ int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool
   kern<<<n_launch < 0 ? chunks : n_launch, kRemapThreads, smem, s>>>(
       ids, c->S, c->cfg.E, c->E_pad, clen,
       local ? c->l_cpg : c->r_chunks, local ? c->l_group_len : c->S, ws_packed(c, ws),
-      ws_prefix(c, ws), ws_counts(c, ws), chunk0, W, k_magic);
+      ws_prefix(c, ws), write_counts ? ws_counts(c, ws) : nullptr, chunk0, W, k_magic, write_counts ? 1 : 0);
   UEP_CUDA_TRY(cudaGetLastError());
   count_launch(c);
   if (with_prefix) return launch_prefix(c, ws, s, local, /*pdl=*/true);

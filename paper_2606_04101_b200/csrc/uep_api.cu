@@ -413,11 +413,35 @@ int uep_shard_count(const uep_ctx* ctx, int32_t shard, int32_t n_shards,
   if (rc != UEP_OK) return rc;
   if (c->S == 0) return UEP_OK;
   if (!topk_ids_local || !aligned16(topk_ids_local)) return UEP_ERR_INVALID_ARG;
-  rc = launch_rank(c, static_cast<const int32_t*>(virtual_base(topk_ids_local, g.slot0, 4)), ws,
-                   static_cast<cudaStream_t>(stream), /*local=*/true, g.chunk0, g.chunks,
-                   /*with_prefix=*/false);
+  // The rows the exchange needs come from one quick counting pass over the shard's ids
+  // (shard_hist_kernel -> shard_rows_kernel on `stream`); the stable ranks, which only the lookup of
+  // uep_shard_finish needs, are made beside it on the context's side stream (forked here, joined in
+  // uep_shard_finish: the same scheme as uep_balance, and the general rank kernel for the same
+  // reason).  Before: rank kernel, then the rows from its counts, all in front of the exchange
+  // (token-sharded step 35.7 us at G = 1 on the DeepSeek-V3 shape).
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int32_t* vids = static_cast<const int32_t*>(virtual_base(topk_ids_local, g.slot0, 4));
   const int rps = c->cfg.R / n_shards;
-  if (rc == UEP_OK) rc = launch_shard_rows(c, ws, static_cast<cudaStream_t>(stream), shard * rps, rps);
+  cudaError_t ce = cudaSuccess;
+  bool forked = false;
+#define UEP_SH_TRY(expr) do { if (rc == UEP_OK && ce == cudaSuccess) ce = (expr); } while (0)
+#define UEP_SH_RC(expr) do { if (rc == UEP_OK && ce == cudaSuccess) rc = (expr); } while (0)
+  UEP_SH_TRY(cudaEventRecord(c->ev_fork, s));
+  UEP_SH_RC(launch_shard_hist(c, vids, ws, s, g.chunk0, g.chunks));       // launched first: its CTAs take the SMs first
+  UEP_SH_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+  forked = (rc == UEP_OK && ce == cudaSuccess);
+  UEP_SH_RC(launch_rank(c, vids, ws, c->side, /*local=*/true, g.chunk0, g.chunks, /*with_prefix=*/false,
+                        /*bitmaps=*/false, /*write_counts=*/false));
+  UEP_SH_TRY(cudaEventRecord(c->ev_rank, c->side));
+  UEP_SH_RC(launch_shard_rows(c, ws, s, shard * rps, rps));
+#undef UEP_SH_TRY
+#undef UEP_SH_RC
+  if (rc == UEP_OK && ce == cudaSuccess) return UEP_OK;
+  if (ce != cudaSuccess) rc = set_cuda_error(ce);
+  if (forked) {                  // join what was forked: an enclosing capture stays valid
+    if (cudaEventRecord(c->ev_join, c->side) == cudaSuccess) cudaStreamWaitEvent(s, c->ev_join, 0);
+  }
+  cudaGetLastError();
   return rc;
 }
 
@@ -447,6 +471,9 @@ int uep_shard_finish(const uep_ctx* ctx, int32_t shard, int32_t n_shards, const 
   rc = launch_plan(c, nullptr, *plan, s, /*pdl=*/true, 1, ws_lambda(c, ws), expert_count, c->cfg.R, c->E_pad,
                    n_inflight ? n_inflight + shard * rps : nullptr, n_inflight ? rps : 0);
   const size_t gb = c->cfg.gate_dtype == UEP_GATE_BF16 ? 2 : 4;
+  // join the rank kernel that uep_shard_count left on the side stream (also when the planner's launch
+  // failed: a capture must not end with an un-joined fork)
+  if (cudaStreamWaitEvent(s, c->ev_rank, 0) != cudaSuccess && rc == UEP_OK) rc = set_cuda_error(cudaGetLastError());
   if (rc == UEP_OK)
     rc = launch_lookup(c, virtual_base(gate_local, g.slot0, gb), *plan,
                        static_cast<int32_t*>(virtual_base(out_replica_local, g.slot0, 4)),

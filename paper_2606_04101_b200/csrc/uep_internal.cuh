@@ -95,7 +95,10 @@ int launch_plan(const Ctx* c, const int32_t* count, const uep_plan_out& plan, cu
 // uep_remap = launch_rank (plan-independent: stable rank of every slot inside its chunk, packed
 // with the expert id into the workspace) + launch_lookup (plan-dependent: cumulative-quota lookup).
 int launch_rank(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, bool local = false,
-                int chunk0 = 0, int n_launch = -1, bool with_prefix = true, bool bitmaps = true);
+                int chunk0 = 0, int n_launch = -1, bool with_prefix = true, bool bitmaps = true,
+                bool write_counts = true);
+// token-sharded path: the grouped chunks' count rows alone (hist.cu)
+int launch_shard_hist(const Ctx* c, const int32_t* ids, void* ws, cudaStream_t s, int chunk0, int n_launch);
 int launch_prefix(const Ctx* c, void* ws, cudaStream_t s, bool local, bool pdl = false);
 // token-sharded path: the shard's rows of Lambda[R][E_pad] from its chunks' counts (after the exchange
 // the planner sums the matrix's columns and the lookup derives its chunk bases from it: no prefix kernel)

@@ -660,6 +660,51 @@ def test_token_sharded_path_matches_global_remap(T, k, E, R, n_slot, s, G, gate_
         assert (np.delete(got, np.s_[g * rps:(g + 1) * rps]) == -3).all()
 
 
+def test_token_sharded_step_captured_as_its_first_use_full_size():
+    """uep_shard_count forks the rank kernel onto the context's side stream and uep_shard_finish joins
+    it in front of the lookup.  Under stream capture that join is a PROGRAMMATIC edge (the lookup is
+    launched with the programmatic attribute), so the rank kernel must not trigger early there: the
+    lookup's prologue reads what it writes.  A fresh context, workspace never used, the step captured
+    without an eager run in front of it (stale ranks of an earlier identical run would hide a race),
+    four layers in one graph, replayed twice with new ids each time; every output against the oracle."""
+    from paper_2606_04101_b200 import shard as shard_mod
+    T, k, E, R, n_slot, um, n = 262144, 8, 256, 64, 2, 1024, 4
+    ctx = binding.Context(T, k, E, R, n_slot, um, gate_dtype=binding.GATE_F32)
+    layers = [shard_mod.TokenShardedLayer(ctx, 0, 1) for _ in range(n)]       # four layers, one context
+    d_ids = [torch.empty(T * k, dtype=torch.int32, device=DEV) for _ in range(n)]
+    d_gate = [torch.empty(T * k, dtype=torch.float32, device=DEV) for _ in range(n)]
+    for L in layers:
+        L.out_gate = torch.zeros(T * k, dtype=torch.float32, device=DEV)
+    st = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(st):
+        with torch.cuda.graph(g, stream=st):
+            for i, L in enumerate(layers):
+                L.step(d_ids[i], d_gate[i])
+    for rep in range(2):
+        ins = []
+        for i in range(n):
+            ids = synth.zipf_topk_ids(T, k, E, 1.0, 900 + 10 * rep + i)
+            gate = synth.gates_uniform_renorm(T, k, 900 + 10 * rep + i)
+            d_ids[i].copy_(ids.reshape(-1))
+            d_gate[i].copy_(gate.reshape(-1))
+            ins.append((ids, gate))
+            for t in (layers[i].out_replica, layers[i].out_rank, layers[i].out_offset):
+                t.fill_(-9)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            g.replay()
+        torch.cuda.synchronize()
+        for (ids, gate), L in zip(ins, layers):
+            lam, p, o_rep, o_rnk, o_off, o_og = oracle_chain(ids, gate, E, R, n_slot, um)
+            assert np.array_equal(L.expert_count.cpu().numpy()[:E], lam)
+            assert np.array_equal(L.out_replica.cpu().numpy().reshape(T, k), o_rep)
+            assert np.array_equal(L.out_rank.cpu().numpy().reshape(T, k), o_rnk)
+            assert np.array_equal(L.out_offset.cpu().numpy().reshape(T, k), o_off)
+            nv = int(p.rank_base[-1])
+            assert np.array_equal(L.out_gate.view(torch.int32).cpu().numpy().view(np.uint32)[:nv], o_og[:nv])
+
+
 def test_token_shard_argument_errors():
     ctx = binding.Context(4096, 2, 16, 4, 1, 64)
     ws = ctx.new_workspace()
